@@ -1,0 +1,177 @@
+/* bits.h -- C ABI of libbits_b200: the data-parallel hot path of the BITS method
+ * (Binary Interval Search, arXiv 1208.3407) on one NVIDIA B200 (sm_100a).
+ *
+ * The path (PAPER.md = /root/reference/PAPER.md; see DESIGN.md for the readings taken):
+ *   place   PAPER.md:155-157 (Sec. 3.2)  random re-placement of one interval set per Monte Carlo
+ *           round: uniform random starts, lengths kept, chromosome ends respected.
+ *   sort    PAPER.md:117-125 (Algorithm 2 COUNTER, "Sort(B_S); Sort(B_E)"), :101 (Sec. 2.1):
+ *           B's starts and B's ends sorted ascending, each on its own.
+ *   search  PAPER.md:93-99 (Algorithm 1 ICOUNT), :103-107: per query interval a,
+ *           first = #{b in B : b.start <= a.end}, last = #{b in B : b.end < a.start},
+ *           c(a) = first - last  (closed intervals).
+ *   reduce  PAPER.md:111, :115, Algorithm 2: total = sum over a in A of c(a).
+ *
+ * Conventions
+ *   - Coordinates are 0-based CLOSED intervals [start, end], start <= end, already projected to
+ *     the 1-D genome: chromosome c occupies [off[c], off[c+1]-1].
+ *   - "dev" pointers are CUDA device pointers owned by the caller; "host" pointers are ordinary
+ *     host memory.  The library never allocates or frees device memory, and never writes to
+ *     its inputs: all scratch lives in the caller's workspace (size from bits_workspace_bytes,
+ *     256-byte aligned).  Workspace contents are undefined on entry and on return.
+ *   - `stream` is a cudaStream_t (NULL = the legacy default stream).  The device-pointer entry
+ *     points validate on the host, enqueue on `stream` and return; outputs are valid once the
+ *     caller has synchronised the stream.  The *_host entry points copy in, run, copy out and
+ *     synchronise `stream` before they return.
+ *   - Every function returns a bits_status (0 = BITS_OK); no exceptions, no printing, no exit.
+ *     On error no output is defined.  There is no CPU fallback: without a usable CUDA device
+ *     the compute entry points return BITS_ERR_CUDA.
+ *   - Sizes: n_a, n_b < 2^32.  Degenerate sizes are legal: n_a == 0 or n_b == 0 gives total 0,
+ *     all per-interval counts 0 and all round counts 0.
+ *   - All results are integers: per-interval counts uint32, totals and round counts uint64.
+ */
+#ifndef BITS_B200_H_
+#define BITS_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  BITS_OK = 0,
+  BITS_ERR_NULL = 1,          /* a required pointer is NULL */
+  BITS_ERR_SIZE = 2,          /* n_a or n_b >= 2^32, or n_rounds / round_begin overflow uint32 */
+  BITS_ERR_GENOME = 3,        /* offset table: off[0] != 0, not strictly ascending, or n_chrom == 0 */
+  BITS_ERR_NO_PLACEMENT = 4,  /* an interval of the permuted set is as long as every chromosome */
+  BITS_ERR_WORKSPACE = 5,     /* workspace NULL, misaligned (256 B) or smaller than required */
+  BITS_ERR_FLAGS = 6,         /* unknown flag bit, bad `which`, bad `fn`, bad `tail` */
+  BITS_ERR_MALFORMED = 7,     /* BITS_VALIDATE: some start > end */
+  BITS_ERR_CUDA = 8           /* a CUDA call failed (including: no device) */
+} bits_status;
+
+/* flags */
+enum {
+  BITS_B_SORTED = 1u,   /* b_start / b_end already are B_S / B_E: each ascending on its own.  The
+                           sort step is skipped (the arrays are read in place). */
+  BITS_VALIDATE = 2u    /* check start <= end for every interval of A and B first; synchronises
+                           the stream once.  Without it malformed input gives undefined counts. */
+};
+
+/* `which` of bits_mc_rounds: the set that is re-placed each round */
+enum {
+  BITS_PERMUTE_A = 0,   /* queries re-placed; B sorted once (BASELINE.json configs[2]) */
+  BITS_PERMUTE_B = 1    /* the searched set re-placed and re-sorted every round
+                           (BASELINE.json configs[4]) */
+};
+
+/* `fn` of bits_workspace_bytes */
+enum {
+  BITS_FN_COUNT = 0,
+  BITS_FN_COUNT_PER_INTERVAL = 1,
+  BITS_FN_MC_ROUNDS = 2,
+  BITS_FN_PLACE = 3,
+  BITS_FN_SORT = 4
+};
+
+/* Bytes of device workspace `fn` needs for these sizes (device-pointer entry points).
+ * `which` matters only for BITS_FN_MC_ROUNDS; n_chrom only for MC_ROUNDS and PLACE; for
+ * BITS_FN_SORT n_b is the key count (n_a ignored).  Add bits_host_staging_bytes for *_host.
+ * Returns 0 for an unknown fn. */
+size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which,
+                            uint32_t flags);
+
+/* Extra device bytes the *_host variant of `fn` needs to stage its inputs and outputs. */
+size_t bits_host_staging_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_rounds);
+
+/* Counting problem (Algorithm 2):
+ *   *total_out = |{(a,b) in A x B : a.start <= b.end and a.end >= b.start}|.
+ * a_start, a_end: dev uint32[n_a]; b_start, b_end: dev uint32[n_b]; total_out: dev uint64[1]. */
+int bits_count(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+               const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+               uint32_t flags, void* workspace, size_t workspace_bytes,
+               uint64_t* total_out, void* stream);
+
+/* Per-interval counting (Algorithm 1):
+ *   counts_out[i] = c(a_i), in A's input order (dev uint32[n_a]);
+ *   *total_out = sum_i c(a_i) (dev uint64[1]; may be NULL). */
+int bits_count_per_interval(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                            const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                            uint32_t flags, void* workspace, size_t workspace_bytes,
+                            uint32_t* counts_out, uint64_t* total_out, void* stream);
+
+/* Monte Carlo rounds (Sec. 3.2; procedure in DESIGN.md "Monte Carlo"):
+ *   *observed_out = total(A, B);
+ *   for k in [0, n_rounds): r = round_begin + k; the permuted set P (A or B, by `which`) is
+ *   re-placed with Philox4x32-10: interval i draws counter (i >> 1, r, which, 0) under key
+ *   (seed lo32, seed hi32), takes the 64 bits x = out[2h] | out[2h+1] << 32 with h = i & 1,
+ *   u = (x * V) >> 64 where V = sum_c max(L_c - d_i, 0) counts the valid starts for its span
+ *   d_i = end_i - start_i, and start' = the u-th valid start in chromosome-table order,
+ *   end' = start' + d_i.  round_counts_out[k] = total(A', B) or total(A, B'), B' re-sorted.
+ * Results depend only on (seed, r, i): any split of the rounds over calls is bit-identical.
+ * chrom_offsets: HOST uint32[n_chrom + 1], off[0] = 0, strictly ascending, off[n_chrom] = G <= 2^32-1
+ * (read before the call returns).  Every interval of the permuted set must satisfy end < G.
+ * observed_out: dev uint64[1]; round_counts_out: dev uint64[n_rounds].
+ * Synchronises `stream` once (the longest span of the permuted set is checked against the
+ * longest chromosome: BITS_ERR_NO_PLACEMENT). */
+int bits_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                   const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                   const uint32_t* chrom_offsets, uint32_t n_chrom, int which, uint64_t seed,
+                   uint32_t round_begin, uint32_t n_rounds,
+                   uint32_t flags, void* workspace, size_t workspace_bytes,
+                   uint64_t* observed_out, uint64_t* round_counts_out, void* stream);
+
+/* One placement step on its own (the "place" row of the path; same arithmetic as inside
+ * bits_mc_rounds): spans dev uint32[n] -> start_out, end_out dev uint32[n] for round `round`,
+ * stream tag `tag` (0 for A, 1 for B).  Spans must be shorter than the longest chromosome. */
+int bits_place(const uint32_t* spans, uint64_t n, const uint32_t* chrom_offsets, uint32_t n_chrom,
+               uint64_t seed, uint32_t round, uint32_t tag,
+               void* workspace, size_t workspace_bytes,
+               uint32_t* start_out, uint32_t* end_out, void* stream);
+
+/* One sort step on its own (the "sort" row: Algorithm 2's Sort(B_S)):
+ * keys_out = keys_in ascending (dev uint32[n] each, must not overlap). */
+int bits_sort_u32(const uint32_t* keys_in, uint32_t* keys_out, uint64_t n,
+                  void* workspace, size_t workspace_bytes, void* stream);
+
+/* Host-buffer variants: same semantics, every array argument is a HOST pointer (pinned memory
+ * makes the copies asynchronous).  workspace is still a device pointer and must hold
+ * bits_workspace_bytes(fn, ...) + bits_host_staging_bytes(fn, ...) bytes.  They copy the inputs
+ * to the device, run the path, copy the outputs back and synchronise `stream`. */
+int bits_count_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                    const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                    uint32_t flags, void* workspace, size_t workspace_bytes,
+                    uint64_t* total_out, void* stream);
+int bits_count_per_interval_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                                 const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                                 uint32_t flags, void* workspace, size_t workspace_bytes,
+                                 uint32_t* counts_out, uint64_t* total_out, void* stream);
+int bits_mc_rounds_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                        const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                        const uint32_t* chrom_offsets, uint32_t n_chrom, int which, uint64_t seed,
+                        uint32_t round_begin, uint32_t n_rounds,
+                        uint32_t flags, void* workspace, size_t workspace_bytes,
+                        uint64_t* observed_out, uint64_t* round_counts_out, void* stream);
+
+/* Empirical p-value from the integer outputs (host pointers; reading R13 -- the paper
+ * prints only log2(observed/median)):
+ *   tail 0: (#{r : count_r >= observed} + 1) / (n_rounds + 1)      (enrichment)
+ *   tail 1: (#{r : count_r <= observed} + 1) / (n_rounds + 1)      (depletion)
+ * Returns NaN for a bad tail or a NULL array with n_rounds > 0. */
+double bits_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n_rounds, int tail);
+
+/* Kernels launched by this library in this process since load (for bench.py's gpu_launches). */
+uint64_t bits_launch_count(void);
+
+/* Tuning knobs for design studies (bench.py --study); returns BITS_ERR_FLAGS for an unknown
+ * name.  They never change results.  Names are listed in DESIGN.md "Knobs". */
+int bits_set_option(const char* name, int64_t value);
+
+const char* bits_strerror(int status);
+const char* bits_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BITS_B200_H_ */

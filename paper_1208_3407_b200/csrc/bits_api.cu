@@ -1,0 +1,625 @@
+// bits_api.cu -- the C ABI of libbits_b200 (include/bits.h): argument checks, workspace carving
+// and kernel launches.  Every step of the path (place, sort, search, reduce) runs in the kernels
+// of this directory; there is no CPU fallback.
+#include <math.h>
+#include <string.h>
+
+#include "common.cuh"
+#include "philox_place.cuh"
+#include "place_kernels.cuh"
+#include "radix_sort.cuh"
+#include "search.cuh"
+
+namespace bits {
+
+unsigned long long g_launches = 0;
+
+struct Options {
+  int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
+  int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
+  int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
+};
+static Options g_opt;
+
+constexpr int kSMs = 148;
+
+// ---------------------------------------------------------------------------------------------
+// Workspace: a bump allocator that is run twice -- once with base == nullptr to size, once to carve.
+struct Carver {
+  char* base;
+  size_t used = 0;
+  explicit Carver(void* b) : base(static_cast<char*>(b)) {}
+  template <typename T>
+  T* take(uint64_t count) {
+    used = align_up(used, 256);
+    T* p = base ? reinterpret_cast<T*>(base + used) : nullptr;
+    used += count * sizeof(T);
+    return p;
+  }
+};
+
+// Buffers for sorting a pair of equally long arrays (starts and ends), plus their bucket indices.
+struct SortCtx {
+  uint32_t n = 0, n_tiles = 0;
+  uint32_t* buf[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [array][0 = result "Y", 1 = temp "X"]
+  uint32_t* hist[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};  // [parity][array] -> uint32[4][256]
+  uint64_t* status[2] = {nullptr, nullptr};
+  uint32_t* ticket = nullptr;                                       // uint32[2]
+  uint32_t* idx[2] = {nullptr, nullptr};
+  uint32_t shift = 31;
+  void carve(Carver& c, uint64_t n_keys, bool with_index) {
+    n = (uint32_t)n_keys;
+    n_tiles = rs::num_tiles(n_keys);
+    const uint64_t padded = align_up(n_keys + kPad, 64);
+    for (int a = 0; a < 2; ++a)
+      for (int b = 0; b < 2; ++b) buf[a][b] = c.take<uint32_t>(padded);
+    for (int p = 0; p < 2; ++p)
+      for (int a = 0; a < 2; ++a) hist[p][a] = c.take<uint32_t>(rs::kPasses * rs::kRadix);
+    for (int a = 0; a < 2; ++a) status[a] = c.take<uint64_t>((uint64_t)n_tiles * rs::kRadix);
+    ticket = c.take<uint32_t>(64);
+    shift = index_shift_for(n_keys);
+    if (with_index)
+      for (int a = 0; a < 2; ++a) idx[a] = c.take<uint32_t>(index_entries(shift));
+  }
+};
+
+struct Small {            // small device scalars
+  uint32_t* max_span;     // [1]
+  uint32_t* bad;          // [1]
+  uint32_t* chrom;        // [n_chrom + 1]
+  void carve(Carver& c, uint32_t n_chrom) {
+    max_span = c.take<uint32_t>(64);
+    bad = max_span ? max_span + 1 : nullptr;
+    chrom = c.take<uint32_t>((uint64_t)n_chrom + 1);
+  }
+};
+
+struct Layout {
+  Small small;
+  SortCtx b;              // the searched set
+  SortCtx q;              // PERMUTE_B: A's ends (array 0) and starts (array 1), sorted once
+  uint32_t* spans = nullptr;
+  size_t bytes = 0;
+};
+
+static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which) {
+  Layout L;
+  Carver c(ws);
+  L.small.carve(c, n_chrom);
+  switch (fn) {
+    case BITS_FN_COUNT:
+    case BITS_FN_COUNT_PER_INTERVAL:
+      L.b.carve(c, n_b, true);
+      break;
+    case BITS_FN_MC_ROUNDS:
+      L.b.carve(c, n_b, true);
+      if (which == BITS_PERMUTE_A) {
+        L.spans = c.take<uint32_t>(align_up(n_a, 4) + 4);
+      } else {
+        L.spans = c.take<uint32_t>(align_up(n_b, 4) + 4);
+        L.q.carve(c, n_a, false);
+      }
+      break;
+    case BITS_FN_PLACE:
+      break;
+    case BITS_FN_SORT:
+      L.b.carve(c, n_b, false);
+      break;
+    default:
+      break;
+  }
+  L.bytes = align_up(c.used, 256);
+  return L;
+}
+
+static inline bool ws_ok(const void* ws, size_t have, size_t need) {
+  return ws != nullptr && ((uintptr_t)ws & 255) == 0 && have >= need;
+}
+
+static inline int grid_for(uint64_t threads_needed, int block) {
+  const uint64_t blocks = ceil_div(threads_needed, block);
+  const uint64_t cap = (uint64_t)kSMs * (uint64_t)g_opt.grid_mult;
+  return (int)(blocks < cap ? (blocks ? blocks : 1) : cap);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Sort of a pair of arrays: src -> X -> Y -> X -> Y, so the result lands in Y.  `hist` must
+// already hold the four digit histograms of both arrays.  `epoch` is advanced per pass.
+struct SortPlan {
+  const uint32_t* src[2];
+  uint32_t* x[2];
+  uint32_t* y[2];
+  const uint32_t* hist[2];
+  uint64_t* status[2];
+  uint32_t* ticket;
+  uint32_t n, n_tiles;
+  int n_arrays;
+};
+
+static int launch_sort_passes(const SortPlan& p, uint32_t* epoch, cudaStream_t st) {
+  for (int pass = 0; pass < rs::kPasses; ++pass) {
+    rs::SortPassArgs a;
+    for (int k = 0; k < 2; ++k) {
+      const int kk = k < p.n_arrays ? k : 0;
+      a.arr[k].src = pass == 0 ? p.src[kk] : ((pass & 1) ? p.x[kk] : p.y[kk]);
+      a.arr[k].dst = (pass & 1) ? p.y[kk] : p.x[kk];
+      a.arr[k].hist = p.hist[kk] + pass * rs::kRadix;
+      a.arr[k].status = p.status[kk];
+      a.arr[k].ticket = p.ticket + k;
+    }
+    a.n = p.n; a.n_tiles = p.n_tiles; a.shift = 8 * pass; a.epoch = (*epoch)++;
+    rs::onesweep_pass_kernel<<<dim3(p.n_tiles, p.n_arrays), rs::kThreads, 0, st>>>(a);
+    BITS_LAUNCH_CHECK();
+  }
+  return BITS_OK;
+}
+
+static int launch_histogram(const uint32_t* k0, const uint32_t* k1, uint32_t* h0, uint32_t* h1, uint32_t n,
+                            int n_arrays, cudaStream_t st) {
+  rs::HistArgs h;
+  h.keys[0] = k0; h.keys[1] = n_arrays > 1 ? k1 : k0;
+  h.hist[0] = h0; h.hist[1] = n_arrays > 1 ? h1 : h0;
+  h.n = n;
+  rs::histogram_kernel<<<dim3(grid_for(ceil_div(n, 4), 512), n_arrays), 512, 0, st>>>(h);
+  BITS_LAUNCH_CHECK();
+  return BITS_OK;
+}
+
+// Clear the sort bookkeeping of a context (once per library call); epochs restart at 1.
+static int reset_sort_ctx(const SortCtx& c, cudaStream_t st) {
+  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[1][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[1][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.status[0], 0, sizeof(uint64_t) * (uint64_t)c.n_tiles * rs::kRadix, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.status[1], 0, sizeof(uint64_t) * (uint64_t)c.n_tiles * rs::kRadix, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.ticket, 0, sizeof(uint32_t) * 64, st));
+  return BITS_OK;
+}
+
+static SortPlan plan_for(const SortCtx& c, const uint32_t* src0, const uint32_t* src1, int parity) {
+  SortPlan p;
+  p.src[0] = src0; p.src[1] = src1;
+  for (int a = 0; a < 2; ++a) {
+    p.x[a] = c.buf[a][1]; p.y[a] = c.buf[a][0];
+    p.hist[a] = c.hist[parity][a];
+    p.status[a] = c.status[a];
+  }
+  p.ticket = c.ticket;
+  p.n = c.n; p.n_tiles = c.n_tiles; p.n_arrays = 2;
+  return p;
+}
+
+static int launch_build_index(const SortCtx& c, cudaStream_t st) {
+  IndexArgs ia;
+  ia.keys[0] = c.buf[0][0]; ia.keys[1] = c.buf[1][0];
+  ia.idx[0] = c.idx[0]; ia.idx[1] = c.idx[1];
+  ia.n = c.n; ia.shift = c.shift;
+  const uint64_t threads = (uint64_t)c.n + 1 > (uint64_t)kPad ? (uint64_t)c.n + 1 : (uint64_t)kPad;
+  build_index_kernel<<<dim3((unsigned)ceil_div(threads, 256), 2), 256, 0, st>>>(ia);
+  BITS_LAUNCH_CHECK();
+  return BITS_OK;
+}
+
+// B_S, B_E (+ indices) from the caller's b_start / b_end.  Result: c.buf[0][0], c.buf[1][0].
+static int setup_searched_set(const SortCtx& c, const uint32_t* b_start, const uint32_t* b_end, uint32_t flags,
+                              uint32_t* epoch, cudaStream_t st) {
+  if (flags & BITS_B_SORTED) {
+    BITS_CUDA_TRY(cudaMemcpyAsync(c.buf[0][0], b_start, sizeof(uint32_t) * (size_t)c.n, cudaMemcpyDeviceToDevice, st));
+    BITS_CUDA_TRY(cudaMemcpyAsync(c.buf[1][0], b_end, sizeof(uint32_t) * (size_t)c.n, cudaMemcpyDeviceToDevice, st));
+  } else {
+    BITS_TRY(launch_histogram(b_start, b_end, c.hist[0][0], c.hist[0][1], c.n, 2, st));
+    const SortPlan p = plan_for(c, b_start, b_end, 0);
+    BITS_TRY(launch_sort_passes(p, epoch, st));
+  }
+  return launch_build_index(c, st);
+}
+
+static inline SortedSet sorted_set(const SortCtx& c, int a) {
+  SortedSet s;
+  s.keys = c.buf[a][0]; s.idx = c.idx[a]; s.n = c.n; s.shift = c.shift;
+  return s;
+}
+
+static int launch_count(const uint32_t* a_start, const uint32_t* a_end, uint32_t n_a, const SortCtx& b,
+                        uint32_t* counts, uint64_t* total, cudaStream_t st) {
+  const bool vec = (((uintptr_t)a_start | (uintptr_t)a_end | (uintptr_t)counts) & 15) == 0;
+  const int grid = grid_for(ceil_div(n_a, 4), 256);
+  if (vec)
+    count_kernel<true><<<grid, 256, 0, st>>>(a_start, a_end, n_a, sorted_set(b, 0), sorted_set(b, 1), counts,
+                                             reinterpret_cast<unsigned long long*>(total));
+  else
+    count_kernel<false><<<grid, 256, 0, st>>>(a_start, a_end, n_a, sorted_set(b, 0), sorted_set(b, 1), counts,
+                                              reinterpret_cast<unsigned long long*>(total));
+  BITS_LAUNCH_CHECK();
+  return BITS_OK;
+}
+
+static int validate_inputs(const uint32_t* a_start, const uint32_t* a_end, uint32_t n_a, const uint32_t* b_start,
+                           const uint32_t* b_end, uint32_t n_b, uint32_t* bad, cudaStream_t st) {
+  BITS_CUDA_TRY(cudaMemsetAsync(bad, 0, sizeof(uint32_t), st));
+  if (n_a) { validate_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(a_start, a_end, n_a, bad); BITS_LAUNCH_CHECK(); }
+  if (n_b) { validate_kernel<<<grid_for(n_b, 256), 256, 0, st>>>(b_start, b_end, n_b, bad); BITS_LAUNCH_CHECK(); }
+  uint32_t h = 0;
+  BITS_CUDA_TRY(cudaMemcpyAsync(&h, bad, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  BITS_CUDA_TRY(cudaStreamSynchronize(st));
+  return h ? BITS_ERR_MALFORMED : BITS_OK;
+}
+
+static int check_common(const void* a_start, const void* a_end, uint64_t n_a, const void* b_start, const void* b_end,
+                        uint64_t n_b, uint32_t flags) {
+  if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (flags & ~(uint32_t)(BITS_B_SORTED | BITS_VALIDATE)) return BITS_ERR_FLAGS;
+  if (n_a && (!a_start || !a_end)) return BITS_ERR_NULL;
+  if (n_b && (!b_start || !b_end)) return BITS_ERR_NULL;
+  return BITS_OK;
+}
+
+static int count_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                      const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* ws, size_t ws_bytes, int fn,
+                      uint32_t* counts_out, uint64_t* total_out, cudaStream_t st) {
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (fn == BITS_FN_COUNT && !total_out) return BITS_ERR_NULL;
+  if (fn == BITS_FN_COUNT_PER_INTERVAL && n_a && !counts_out) return BITS_ERR_NULL;
+  const Layout L = make_layout(ws, fn, n_a, n_b, 0, 0);
+  if (!ws_ok(ws, ws_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
+  if (flags & BITS_VALIDATE)
+    BITS_TRY(validate_inputs(a_start, a_end, (uint32_t)n_a, b_start, b_end, (uint32_t)n_b, L.small.bad, st));
+  if (total_out) BITS_CUDA_TRY(cudaMemsetAsync(total_out, 0, sizeof(uint64_t), st));
+  if (n_a == 0) return BITS_OK;
+  if (n_b == 0) {
+    if (counts_out) BITS_CUDA_TRY(cudaMemsetAsync(counts_out, 0, sizeof(uint32_t) * (size_t)n_a, st));
+    return BITS_OK;
+  }
+  uint32_t epoch = 1;
+  BITS_TRY(reset_sort_ctx(L.b, st));
+  BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
+  return launch_count(a_start, a_end, (uint32_t)n_a, L.b, counts_out, total_out, st);
+}
+
+// ---------------------------------------------------------------------------------------------
+static int check_genome(const uint32_t* off, uint32_t n_chrom, ChromTable* t, uint32_t* l_max) {
+  if (!off) return BITS_ERR_NULL;
+  if (n_chrom == 0 || off[0] != 0) return BITS_ERR_GENOME;
+  uint32_t lmin = 0xffffffffu, lmax = 0;
+  for (uint32_t c = 0; c < n_chrom; ++c) {
+    if (off[c + 1] <= off[c]) return BITS_ERR_GENOME;
+    const uint32_t L = off[c + 1] - off[c];
+    lmin = L < lmin ? L : lmin;
+    lmax = L > lmax ? L : lmax;
+  }
+  t->n_chrom = n_chrom;
+  t->l_min = lmin;
+  t->genome = off[n_chrom];
+  uint32_t s = 0;
+  if (n_chrom > 1) { s = 1; while ((uint64_t)s * 2 <= n_chrom - 1) s *= 2; }
+  t->step0 = s;
+  *l_max = lmax;
+  return BITS_OK;
+}
+
+static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* end_out, uint32_t n, uint32_t round,
+                        uint32_t tag, const PhiloxKeys& key, const ChromTable& chrom, bool vec, uint32_t* hist_s,
+                        uint32_t* hist_e, uint32_t* zero_s, uint32_t* zero_e, cudaStream_t st) {
+  PlaceArgs a;
+  a.spans = spans; a.start_out = start_out; a.end_out = end_out; a.n = n; a.round = round; a.tag = tag;
+  a.key = key; a.chrom = chrom; a.hist_start = hist_s; a.hist_end = hist_e; a.zero_a = zero_s; a.zero_b = zero_e;
+  const int grid = grid_for(ceil_div(n, 4), 256);
+  if (hist_s) {
+    if (vec) place_kernel<true, true><<<grid, 256, 0, st>>>(a); else place_kernel<false, true><<<grid, 256, 0, st>>>(a);
+  } else {
+    if (vec) place_kernel<true, false><<<grid, 256, 0, st>>>(a); else place_kernel<false, false><<<grid, 256, 0, st>>>(a);
+  }
+  BITS_LAUNCH_CHECK();
+  return BITS_OK;
+}
+
+static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                   const uint32_t* b_end, uint64_t n_b, const uint32_t* off, uint32_t n_chrom, int which, uint64_t seed,
+                   uint32_t round_begin, uint32_t n_rounds, uint32_t flags, void* ws, size_t ws_bytes,
+                   uint64_t* observed_out, uint64_t* round_counts_out, cudaStream_t st) {
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (which != BITS_PERMUTE_A && which != BITS_PERMUTE_B) return BITS_ERR_FLAGS;
+  if (!observed_out || (n_rounds && !round_counts_out)) return BITS_ERR_NULL;
+  if ((uint64_t)round_begin + n_rounds > (1ull << 32)) return BITS_ERR_SIZE;
+  ChromTable chrom;
+  uint32_t l_max = 0;
+  BITS_TRY(check_genome(off, n_chrom, &chrom, &l_max));
+  const Layout L = make_layout(ws, BITS_FN_MC_ROUNDS, n_a, n_b, n_chrom, which);
+  if (!ws_ok(ws, ws_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
+  if (flags & BITS_VALIDATE)
+    BITS_TRY(validate_inputs(a_start, a_end, (uint32_t)n_a, b_start, b_end, (uint32_t)n_b, L.small.bad, st));
+  chrom.off = L.small.chrom;
+  BITS_CUDA_TRY(cudaMemcpyAsync(L.small.chrom, off, sizeof(uint32_t) * ((size_t)n_chrom + 1), cudaMemcpyHostToDevice, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(observed_out, 0, sizeof(uint64_t), st));
+  if (n_rounds) BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out, 0, sizeof(uint64_t) * (size_t)n_rounds, st));
+
+  // spans of the permuted set + the NO_PLACEMENT check (one synchronisation)
+  const uint32_t n_p = (uint32_t)(which == BITS_PERMUTE_A ? n_a : n_b);
+  if (n_p) {
+    BITS_CUDA_TRY(cudaMemsetAsync(L.small.max_span, 0, sizeof(uint32_t), st));
+    spans_kernel<<<grid_for(n_p, 256), 256, 0, st>>>(which == BITS_PERMUTE_A ? a_start : b_start,
+                                                     which == BITS_PERMUTE_A ? a_end : b_end, n_p, L.spans,
+                                                     L.small.max_span);
+    BITS_LAUNCH_CHECK();
+    uint32_t h_max = 0;
+    BITS_CUDA_TRY(cudaMemcpyAsync(&h_max, L.small.max_span, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    BITS_CUDA_TRY(cudaStreamSynchronize(st));
+    if (h_max >= l_max) return BITS_ERR_NO_PLACEMENT;
+  }
+  if (n_a == 0 || n_b == 0) return BITS_OK;   // every count is 0 (already written)
+
+  // observed = total(A, B)
+  uint32_t epoch = 1;
+  BITS_TRY(reset_sort_ctx(L.b, st));
+  BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
+  BITS_TRY(launch_count(a_start, a_end, (uint32_t)n_a, L.b, nullptr, observed_out, st));
+  if (n_rounds == 0) return BITS_OK;
+
+  const PhiloxKeys key = make_philox_keys(seed);
+  if (which == BITS_PERMUTE_A) {
+    McAArgs m;
+    m.spans = L.spans; m.n_a = (uint32_t)n_a; m.key = key; m.chrom = chrom;
+    m.bs = sorted_set(L.b, 0); m.be = sorted_set(L.b, 1);
+    m.round_counts = reinterpret_cast<unsigned long long*>(round_counts_out);
+    const unsigned gx = (unsigned)ceil_div(ceil_div(n_a, 4), 256);
+    for (uint32_t done = 0; done < n_rounds;) {
+      const uint32_t chunk = n_rounds - done < 32768u ? n_rounds - done : 32768u;
+      m.round0 = round_begin + done; m.out0 = done;
+      mc_permute_a_kernel<<<dim3(gx, chunk), 256, 0, st>>>(m);
+      BITS_LAUNCH_CHECK();
+      done += chunk;
+    }
+    return BITS_OK;
+  }
+
+  // PERMUTE_B: A's ends and starts sorted once; every round place -> sort x2 -> search -> reduce.
+  uint32_t q_epoch = 1;
+  BITS_TRY(reset_sort_ctx(L.q, st));
+  BITS_TRY(launch_histogram(a_end, a_start, L.q.hist[0][0], L.q.hist[0][1], L.q.n, 2, st));
+  BITS_TRY(launch_sort_passes(plan_for(L.q, a_end, a_start, 0), &q_epoch, st));
+  const uint32_t* q_end_sorted = L.q.buf[0][0];
+  const uint32_t* q_start_sorted = L.q.buf[1][0];
+  // the observed-count sort used histogram parity 0; clear it so round 0 can accumulate into it
+  BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[0][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[0][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+  const bool fused = g_opt.place_fused_hist != 0;
+  for (uint32_t k = 0; k < n_rounds; ++k) {
+    const int par = (int)(k & 1);
+    // epochs (30 bits) and ticket counters (32 bits, taken modulo n_tiles) must not wrap
+    if (epoch > (1u << 30) - 8u || (uint64_t)epoch * L.b.n_tiles > (1ull << 32) - 8ull * L.b.n_tiles) {
+      BITS_CUDA_TRY(cudaMemsetAsync(L.b.status[0], 0, sizeof(uint64_t) * (uint64_t)L.b.n_tiles * rs::kRadix, st));
+      BITS_CUDA_TRY(cudaMemsetAsync(L.b.status[1], 0, sizeof(uint64_t) * (uint64_t)L.b.n_tiles * rs::kRadix, st));
+      BITS_CUDA_TRY(cudaMemsetAsync(L.b.ticket, 0, sizeof(uint32_t) * 64, st));
+      epoch = 1;
+    }
+    if (fused) {
+      BITS_TRY(launch_place(L.spans, L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, round_begin + k, 1u, key, chrom, true,
+                            L.b.hist[par][0], L.b.hist[par][1], L.b.hist[par ^ 1][0], L.b.hist[par ^ 1][1], st));
+    } else {
+      BITS_TRY(launch_place(L.spans, L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, round_begin + k, 1u, key, chrom, true,
+                            nullptr, nullptr, nullptr, nullptr, st));
+      BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[par][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+      BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[par][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+      BITS_TRY(launch_histogram(L.b.buf[0][0], L.b.buf[1][0], L.b.hist[par][0], L.b.hist[par][1], (uint32_t)n_b, 2, st));
+    }
+    BITS_TRY(launch_sort_passes(plan_for(L.b, L.b.buf[0][0], L.b.buf[1][0], par), &epoch, st));
+    unsigned long long* out = reinterpret_cast<unsigned long long*>(round_counts_out + k);
+    if (g_opt.mc_sorted_queries) {
+      sorted_query_total_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(q_end_sorted, q_start_sorted, (uint32_t)n_a,
+                                                                    L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, out);
+      BITS_LAUNCH_CHECK();
+    } else {
+      BITS_TRY(launch_build_index(L.b, st));
+      BITS_TRY(launch_count(a_start, a_end, (uint32_t)n_a, L.b, nullptr, reinterpret_cast<uint64_t*>(out), st));
+    }
+  }
+  return BITS_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------
+struct HostStage {
+  uint32_t *a_s, *a_e, *b_s, *b_e, *counts;
+  uint64_t *total, *rounds;
+  size_t bytes;
+};
+static HostStage make_stage(void* base, uint64_t n_a, uint64_t n_b, uint32_t n_rounds, bool with_counts) {
+  Carver c(base);
+  HostStage h;
+  h.a_s = c.take<uint32_t>(align_up(n_a, 4) + 4);
+  h.a_e = c.take<uint32_t>(align_up(n_a, 4) + 4);
+  h.b_s = c.take<uint32_t>(align_up(n_b, 4) + 4);
+  h.b_e = c.take<uint32_t>(align_up(n_b, 4) + 4);
+  h.counts = with_counts ? c.take<uint32_t>(align_up(n_a, 4) + 4) : nullptr;
+  h.total = c.take<uint64_t>(32);
+  h.rounds = c.take<uint64_t>((uint64_t)n_rounds + 1);
+  h.bytes = align_up(c.used, 256);
+  return h;
+}
+
+static int stage_in(const HostStage& h, const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                    const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b, cudaStream_t st) {
+  if (n_a) {
+    BITS_CUDA_TRY(cudaMemcpyAsync(h.a_s, a_start, 4 * (size_t)n_a, cudaMemcpyHostToDevice, st));
+    BITS_CUDA_TRY(cudaMemcpyAsync(h.a_e, a_end, 4 * (size_t)n_a, cudaMemcpyHostToDevice, st));
+  }
+  if (n_b) {
+    BITS_CUDA_TRY(cudaMemcpyAsync(h.b_s, b_start, 4 * (size_t)n_b, cudaMemcpyHostToDevice, st));
+    BITS_CUDA_TRY(cudaMemcpyAsync(h.b_e, b_end, 4 * (size_t)n_b, cudaMemcpyHostToDevice, st));
+  }
+  return BITS_OK;
+}
+
+}  // namespace bits
+
+using namespace bits;
+
+extern "C" {
+
+size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which, uint32_t flags) {
+  (void)flags;
+  if (fn < BITS_FN_COUNT || fn > BITS_FN_SORT) return 0;
+  if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return 0;
+  return make_layout(nullptr, fn, n_a, n_b, n_chrom, which).bytes;
+}
+
+size_t bits_host_staging_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_rounds) {
+  if (fn < BITS_FN_COUNT || fn > BITS_FN_MC_ROUNDS) return 0;
+  return make_stage(nullptr, n_a, n_b, n_rounds, fn == BITS_FN_COUNT_PER_INTERVAL).bytes;
+}
+
+int bits_count(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+               const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* workspace, size_t workspace_bytes,
+               uint64_t* total_out, void* stream) {
+  return count_impl(a_start, a_end, n_a, b_start, b_end, n_b, flags, workspace, workspace_bytes, BITS_FN_COUNT,
+                    nullptr, total_out, static_cast<cudaStream_t>(stream));
+}
+
+int bits_count_per_interval(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                            const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* workspace,
+                            size_t workspace_bytes, uint32_t* counts_out, uint64_t* total_out, void* stream) {
+  return count_impl(a_start, a_end, n_a, b_start, b_end, n_b, flags, workspace, workspace_bytes,
+                    BITS_FN_COUNT_PER_INTERVAL, counts_out, total_out, static_cast<cudaStream_t>(stream));
+}
+
+int bits_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                   const uint32_t* b_end, uint64_t n_b, const uint32_t* chrom_offsets, uint32_t n_chrom, int which,
+                   uint64_t seed, uint32_t round_begin, uint32_t n_rounds, uint32_t flags, void* workspace,
+                   size_t workspace_bytes, uint64_t* observed_out, uint64_t* round_counts_out, void* stream) {
+  return mc_impl(a_start, a_end, n_a, b_start, b_end, n_b, chrom_offsets, n_chrom, which, seed, round_begin, n_rounds,
+                 flags, workspace, workspace_bytes, observed_out, round_counts_out, static_cast<cudaStream_t>(stream));
+}
+
+int bits_place(const uint32_t* spans, uint64_t n, const uint32_t* chrom_offsets, uint32_t n_chrom, uint64_t seed,
+               uint32_t round, uint32_t tag, void* workspace, size_t workspace_bytes, uint32_t* start_out,
+               uint32_t* end_out, void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (n >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (n && (!spans || !start_out || !end_out)) return BITS_ERR_NULL;
+  ChromTable chrom;
+  uint32_t l_max = 0;
+  BITS_TRY(check_genome(chrom_offsets, n_chrom, &chrom, &l_max));
+  const Layout L = make_layout(workspace, BITS_FN_PLACE, 0, 0, n_chrom, 0);
+  if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
+  if (n == 0) return BITS_OK;
+  chrom.off = L.small.chrom;
+  BITS_CUDA_TRY(cudaMemcpyAsync(L.small.chrom, chrom_offsets, sizeof(uint32_t) * ((size_t)n_chrom + 1),
+                                cudaMemcpyHostToDevice, st));
+  const bool vec = (n & 3) == 0 && (((uintptr_t)spans | (uintptr_t)start_out | (uintptr_t)end_out) & 15) == 0;
+  return launch_place(spans, start_out, end_out, (uint32_t)n, round, tag, make_philox_keys(seed), chrom, vec, nullptr,
+                      nullptr, nullptr, nullptr, st);
+}
+
+int bits_sort_u32(const uint32_t* keys_in, uint32_t* keys_out, uint64_t n, void* workspace, size_t workspace_bytes,
+                  void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (n >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (n && (!keys_in || !keys_out)) return BITS_ERR_NULL;
+  const Layout L = make_layout(workspace, BITS_FN_SORT, 0, n, 0, 0);
+  if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
+  if (n == 0) return BITS_OK;
+  BITS_TRY(reset_sort_ctx(L.b, st));
+  BITS_TRY(launch_histogram(keys_in, nullptr, L.b.hist[0][0], nullptr, (uint32_t)n, 1, st));
+  SortPlan p = plan_for(L.b, keys_in, keys_in, 0);
+  p.y[0] = keys_out;
+  p.n_arrays = 1;
+  uint32_t epoch = 1;
+  return launch_sort_passes(p, &epoch, st);
+}
+
+int bits_count_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                    const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* workspace, size_t workspace_bytes,
+                    uint64_t* total_out, void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (!total_out) return BITS_ERR_NULL;
+  const size_t main_bytes = bits_workspace_bytes(BITS_FN_COUNT, n_a, n_b, 0, 0, flags);
+  const HostStage h = make_stage(workspace ? static_cast<char*>(workspace) + main_bytes : nullptr, n_a, n_b, 0, false);
+  if (!ws_ok(workspace, workspace_bytes, main_bytes + h.bytes)) return BITS_ERR_WORKSPACE;
+  BITS_TRY(stage_in(h, a_start, a_end, n_a, b_start, b_end, n_b, st));
+  BITS_TRY(count_impl(h.a_s, h.a_e, n_a, h.b_s, h.b_e, n_b, flags, workspace, main_bytes, BITS_FN_COUNT, nullptr,
+                      h.total, st));
+  BITS_CUDA_TRY(cudaMemcpyAsync(total_out, h.total, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+  BITS_CUDA_TRY(cudaStreamSynchronize(st));
+  return BITS_OK;
+}
+
+int bits_count_per_interval_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                                 const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b, uint32_t flags,
+                                 void* workspace, size_t workspace_bytes, uint32_t* counts_out, uint64_t* total_out,
+                                 void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (n_a && !counts_out) return BITS_ERR_NULL;
+  const size_t main_bytes = bits_workspace_bytes(BITS_FN_COUNT_PER_INTERVAL, n_a, n_b, 0, 0, flags);
+  const HostStage h = make_stage(workspace ? static_cast<char*>(workspace) + main_bytes : nullptr, n_a, n_b, 0, true);
+  if (!ws_ok(workspace, workspace_bytes, main_bytes + h.bytes)) return BITS_ERR_WORKSPACE;
+  BITS_TRY(stage_in(h, a_start, a_end, n_a, b_start, b_end, n_b, st));
+  BITS_TRY(count_impl(h.a_s, h.a_e, n_a, h.b_s, h.b_e, n_b, flags, workspace, main_bytes, BITS_FN_COUNT_PER_INTERVAL,
+                      h.counts, h.total, st));
+  if (n_a) BITS_CUDA_TRY(cudaMemcpyAsync(counts_out, h.counts, 4 * (size_t)n_a, cudaMemcpyDeviceToHost, st));
+  if (total_out) BITS_CUDA_TRY(cudaMemcpyAsync(total_out, h.total, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+  BITS_CUDA_TRY(cudaStreamSynchronize(st));
+  return BITS_OK;
+}
+
+int bits_mc_rounds_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                        const uint32_t* b_end, uint64_t n_b, const uint32_t* chrom_offsets, uint32_t n_chrom,
+                        int which, uint64_t seed, uint32_t round_begin, uint32_t n_rounds, uint32_t flags,
+                        void* workspace, size_t workspace_bytes, uint64_t* observed_out, uint64_t* round_counts_out,
+                        void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (!observed_out || (n_rounds && !round_counts_out)) return BITS_ERR_NULL;
+  const size_t main_bytes = bits_workspace_bytes(BITS_FN_MC_ROUNDS, n_a, n_b, n_chrom, which, flags);
+  const HostStage h =
+      make_stage(workspace ? static_cast<char*>(workspace) + main_bytes : nullptr, n_a, n_b, n_rounds, false);
+  if (!ws_ok(workspace, workspace_bytes, main_bytes + h.bytes)) return BITS_ERR_WORKSPACE;
+  BITS_TRY(stage_in(h, a_start, a_end, n_a, b_start, b_end, n_b, st));
+  BITS_TRY(mc_impl(h.a_s, h.a_e, n_a, h.b_s, h.b_e, n_b, chrom_offsets, n_chrom, which, seed, round_begin, n_rounds,
+                   flags, workspace, main_bytes, h.total, h.rounds, st));
+  BITS_CUDA_TRY(cudaMemcpyAsync(observed_out, h.total, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+  if (n_rounds)
+    BITS_CUDA_TRY(cudaMemcpyAsync(round_counts_out, h.rounds, sizeof(uint64_t) * (size_t)n_rounds,
+                                  cudaMemcpyDeviceToHost, st));
+  BITS_CUDA_TRY(cudaStreamSynchronize(st));
+  return BITS_OK;
+}
+
+double bits_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n_rounds, int tail) {
+  if ((tail != 0 && tail != 1) || (n_rounds && !round_counts)) return NAN;
+  uint64_t k = 0;
+  for (uint32_t r = 0; r < n_rounds; ++r)
+    k += tail == 0 ? (round_counts[r] >= observed) : (round_counts[r] <= observed);
+  return (double)(k + 1) / (double)((uint64_t)n_rounds + 1);
+}
+
+uint64_t bits_launch_count(void) { return g_launches; }
+
+int bits_set_option(const char* name, int64_t value) {
+  if (!name) return BITS_ERR_NULL;
+  if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }
+  if (!strcmp(name, "place_fused_hist")) { g_opt.place_fused_hist = value; return BITS_OK; }
+  if (!strcmp(name, "grid_mult")) { if (value < 1 || value > 64) return BITS_ERR_FLAGS; g_opt.grid_mult = value; return BITS_OK; }
+  return BITS_ERR_FLAGS;
+}
+
+const char* bits_strerror(int status) {
+  switch (status) {
+    case BITS_OK: return "ok";
+    case BITS_ERR_NULL: return "a required pointer is NULL";
+    case BITS_ERR_SIZE: return "size out of range (n_a, n_b < 2^32; round_begin + n_rounds <= 2^32)";
+    case BITS_ERR_GENOME: return "bad chromosome offset table";
+    case BITS_ERR_NO_PLACEMENT: return "an interval of the permuted set is as long as every chromosome";
+    case BITS_ERR_WORKSPACE: return "workspace NULL, misaligned or too small";
+    case BITS_ERR_FLAGS: return "unknown flag, option, fn, which or tail";
+    case BITS_ERR_MALFORMED: return "malformed interval (start > end)";
+    case BITS_ERR_CUDA: return "CUDA error (or no CUDA device)";
+    default: return "unknown status";
+  }
+}
+
+const char* bits_version(void) { return "bits_b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,224 @@
+// search.cuh -- the "search" and "reduce" steps.
+//
+// PAPER.md:93-99 (Algorithm 1 ICOUNT): first = BSEARCH(B_S, a.end), last = BSEARCH(B_E, a.start),
+// c = first - last, with the ranks fixed by the set definitions L and R (PAPER.md:83-89,
+// :103-107; reading R1):  first = #{b.start <= a.end}, last = #{b.end < a.start}.
+// Both are "count of keys <= x": last = (a.start == 0) ? 0 : #{b.end <= a.start - 1}.
+// PAPER.md:127-131 (Sec. 2.3): one independent ICOUNT per thread, no communication -- here
+// four queries (eight rank look-ups) per thread for memory-level parallelism.
+//
+// Search structure (not in the paper): a bucket index over each sorted array,
+//   idx[h] = #{keys < h << shift},  h = 0 .. 2^(32-shift),
+// so a look-up is one index read plus one or two 32-byte sectors of keys, instead of ~log2|B|
+// dependent probes.  Sorted arrays are padded with 16 keys of 0xffffffff.
+#pragma once
+#include "common.cuh"
+#include "philox_place.cuh"
+
+namespace bits {
+
+constexpr int kPad = 16;   // sentinel keys after the last real key of a sorted array
+
+struct SortedSet {
+  const uint32_t* keys;   // ascending, 32-byte aligned, padded with kPad x 0xffffffff
+  const uint32_t* idx;    // uint32[(1 << (32 - shift)) + 1]
+  uint32_t n;
+  uint32_t shift;         // 1..31
+};
+
+inline uint32_t index_shift_for(uint64_t n) {
+  // about one bucket per four keys, between 2 and 2^24 buckets
+  uint32_t bits = 1;
+  while (bits < 24 && (1ull << bits) < n / 4) ++bits;
+  return 32 - bits;
+}
+inline uint64_t index_entries(uint32_t shift) { return (1ull << (32 - shift)) + 1; }
+
+__device__ __forceinline__ uint32_t count_le8(const uint4& a, const uint4& b, uint32_t q) {
+  return (a.x <= q) + (a.y <= q) + (a.z <= q) + (a.w <= q) + (b.x <= q) + (b.y <= q) + (b.z <= q) + (b.w <= q);
+}
+
+// #{keys <= q}
+__device__ __forceinline__ uint32_t rank_le(const SortedSet& s, uint32_t q) {
+  const uint32_t h = q >> s.shift;
+  const uint32_t pos = __ldg(s.idx + h);
+  uint32_t base = pos & ~7u;      // every key before `pos` is < h << shift <= q
+  const uint4* p = reinterpret_cast<const uint4*>(s.keys + base);
+  uint32_t c = count_le8(__ldg(p), __ldg(p + 1), q);
+  if (c == 8) {
+    base += 8;
+    c = count_le8(__ldg(p + 2), __ldg(p + 3), q);
+    if (c == 8) {                 // long bucket: finish with a binary search inside it
+      uint32_t lo = base + 8, hi = __ldg(s.idx + h + 1);
+      while (lo < hi) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        if (__ldg(s.keys + mid) <= q) lo = mid + 1; else hi = mid;
+      }
+      return min(lo, s.n);
+    }
+  }
+  return min(base + c, s.n);
+}
+
+// c(a) = #{b.start <= a.end} - #{b.end < a.start}
+__device__ __forceinline__ uint32_t icount(const SortedSet& bs, const SortedSet& be, uint32_t a_start, uint32_t a_end) {
+  const uint32_t first = rank_le(bs, a_end);
+  const uint32_t last = a_start == 0 ? 0u : rank_le(be, a_start - 1u);
+  return first - last;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Index build.  One thread per position i in [0, n]: fills idx[(key[i-1] >> s) + 1 .. key[i] >> s]
+// with i (key[-1] = "-1", key[n] = "2^32").  Long gaps are filled by the whole warp.  Also writes
+// the kPad sentinels.  grid.y = array (0: starts, 1: ends).
+struct IndexArgs {
+  uint32_t* keys[2];      // sorted; sentinels are written at keys[n .. n+kPad)
+  uint32_t* idx[2];
+  uint32_t n;
+  uint32_t shift;
+};
+
+__global__ void __launch_bounds__(256) build_index_kernel(IndexArgs a) {
+  uint32_t* __restrict__ keys = blockIdx.y ? a.keys[1] : a.keys[0];
+  uint32_t* __restrict__ idx = blockIdx.y ? a.idx[1] : a.idx[0];
+  const uint32_t n = a.n, s = a.shift;
+  const uint32_t H = 1u << (32 - s);
+  const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;   // warps are never partly out of range
+  const uint32_t lane = threadIdx.x & 31;
+  if (gid < kPad) keys[(uint64_t)n + gid] = 0xffffffffu;
+  uint32_t lo = 1, hi = 0;   // fill idx[lo..hi] = i  (empty by default)
+  const uint32_t i = (uint32_t)gid;
+  if (gid <= n) {
+    lo = (i == 0) ? 0u : (keys[i - 1] >> s) + 1u;
+    hi = (i == n) ? H : (keys[i] >> s);
+  }
+  const bool some = lo <= hi;
+  const uint32_t len = some ? hi - lo + 1u : 0u;
+  if (some && len <= 4)
+    for (uint32_t h = lo; h <= hi; ++h) idx[h] = i;
+  uint32_t big = __ballot_sync(kFullMask, len > 4);
+  while (big) {
+    const int src = __ffs(big) - 1;
+    big &= big - 1;
+    const uint32_t l = __shfl_sync(kFullMask, lo, src), hh = __shfl_sync(kFullMask, hi, src);
+    const uint32_t v = __shfl_sync(kFullMask, i, src);
+    for (uint64_t h = (uint64_t)l + lane; h <= hh; h += 32) idx[h] = v;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Count kernel: queries in input order, four per thread.  Writes per-interval counts if
+// counts != nullptr; adds the block's sum to *total if total != nullptr.
+template <bool kVec>
+__global__ void __launch_bounds__(256) count_kernel(const uint32_t* __restrict__ a_start,
+                                                    const uint32_t* __restrict__ a_end, uint32_t n_a,
+                                                    SortedSet bs, SortedSet be,
+                                                    uint32_t* __restrict__ counts, unsigned long long* total) {
+  __shared__ uint64_t s_red[8];
+  uint64_t sum = 0;
+  const uint64_t n4 = ((uint64_t)n_a + 3) >> 2;
+  for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n4; t += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t i0 = t << 2;
+    uint32_t qs[4], qe[4], c[4];
+    const bool full = i0 + 3 < n_a;
+    if (kVec && full) {
+      const uint4 s4 = __ldcs(reinterpret_cast<const uint4*>(a_start) + t);
+      const uint4 e4 = __ldcs(reinterpret_cast<const uint4*>(a_end) + t);
+      qs[0] = s4.x; qs[1] = s4.y; qs[2] = s4.z; qs[3] = s4.w;
+      qe[0] = e4.x; qe[1] = e4.y; qe[2] = e4.z; qe[3] = e4.w;
+    } else {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const bool ok = i0 + j < n_a;
+        qs[j] = ok ? a_start[i0 + j] : 0u;
+        qe[j] = ok ? a_end[i0 + j] : 0u;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) c[j] = icount(bs, be, qs[j], qe[j]);
+    if (!full) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) if (i0 + j >= n_a) c[j] = 0;
+    }
+    if (counts) {
+      if (kVec && full) {
+        __stcs(reinterpret_cast<uint4*>(counts) + t, make_uint4(c[0], c[1], c[2], c[3]));
+      } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (i0 + j < n_a) counts[i0 + j] = c[j];
+      }
+    }
+    sum += (uint64_t)c[0] + c[1] + c[2] + c[3];
+  }
+  if (total) block_sum_atomic(sum, s_red, total);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Plain rank look-ups for SORTED queries (the per-round search when B is re-placed: A's ends and
+// A's starts are sorted once per call, so neighbouring threads walk neighbouring keys and the
+// probes coalesce).  sum_first = sum_q #{keys <= q};  sum_last = sum_q #{keys < q}.
+// The round total is sum_first(B_S; A ends) - sum_last(B_E; A starts): integer sums commute, so
+// this equals sum_a (first - last) bit for bit.
+template <bool kStrict>
+__device__ __forceinline__ uint32_t rank_plain(const uint32_t* __restrict__ keys, uint32_t n, uint32_t q) {
+  uint32_t lo = 0, len = n;
+  while (len > 0) {
+    const uint32_t half = len >> 1;
+    const uint32_t k = __ldg(keys + lo + half);
+    const bool right = kStrict ? (k < q) : (k <= q);
+    lo = right ? lo + half + 1 : lo;
+    len = right ? len - half - 1 : half;
+  }
+  return lo;
+}
+
+__global__ void __launch_bounds__(256) sorted_query_total_kernel(const uint32_t* __restrict__ q_end_sorted,
+                                                                 const uint32_t* __restrict__ q_start_sorted, uint32_t n_q,
+                                                                 const uint32_t* __restrict__ b_s, const uint32_t* __restrict__ b_e,
+                                                                 uint32_t n_b, unsigned long long* total) {
+  __shared__ uint64_t s_red[8];
+  // two's-complement accumulation: the final sum is exact modulo 2^64 and non-negative
+  uint64_t sum = 0;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_q; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint32_t first = rank_plain<false>(b_s, n_b, __ldg(q_end_sorted + i));
+    const uint32_t last = rank_plain<true>(b_e, n_b, __ldg(q_start_sorted + i));
+    sum += (uint64_t)first - (uint64_t)last;
+  }
+  block_sum_atomic(sum, s_red, total);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused Monte Carlo kernel for re-placed QUERIES (BITS_PERMUTE_A): place -> search -> reduce with
+// no intermediate arrays.  grid = (tiles of 1024 queries, rounds in this launch).
+struct McAArgs {
+  const uint32_t* spans;     // dev uint32[n_a], padded to a multiple of 4 with zeros
+  uint32_t n_a;
+  uint32_t round0;           // first round of this launch
+  PhiloxKeys key;
+  ChromTable chrom;
+  SortedSet bs, be;
+  unsigned long long* round_counts;   // indexed by blockIdx.y + out0
+  uint32_t out0;
+};
+
+__global__ void __launch_bounds__(256) mc_permute_a_kernel(McAArgs a) {
+  __shared__ uint32_t s_off[kMaxChromSmem];
+  __shared__ uint64_t s_red[8];
+  const uint32_t* off = stage_chrom_table(a.chrom, s_off);
+  const uint32_t round = a.round0 + blockIdx.y;
+  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t i0 = t << 2;
+  uint64_t sum = 0;
+  if (i0 < a.n_a) {
+    const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans) + t);
+    const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
+    uint32_t st[4];
+    place4(i0, round, 0u, a.key, d, off, a.chrom, st);
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (i0 + j < a.n_a) sum += icount(a.bs, a.be, st[j], st[j] + d[j]);
+  }
+  block_sum_atomic(sum, s_red, a.round_counts + a.out0 + blockIdx.y);
+}
+
+}  // namespace bits

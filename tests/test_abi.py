@@ -1,0 +1,100 @@
+"""C-ABI checks that need no GPU: the library builds, loads, exports every symbol include/bits.h
+declares, sizes workspaces, and rejects bad arguments on the host before any CUDA call."""
+import ctypes as C
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1208_3407_b200 import bits
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "bits.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(bits_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported_and_bound():
+    names = declared_symbols()
+    assert len(names) >= 15
+    raw = C.CDLL(bits.lib_path() if os.path.exists(bits.lib_path()) else bits.lib()._name)
+    bits.lib()
+    for n in names:
+        assert hasattr(raw, n), f"{n} declared in bits.h but not exported"
+    assert set(names) == set(bits.EXPORTS)
+
+
+def test_version_and_strerror():
+    assert "sm_100a" in bits.version()
+    assert bits.strerror(0) == "ok"
+    for s in range(1, 9):
+        assert bits.strerror(s) not in ("ok", "unknown status")
+    assert bits.strerror(99) == "unknown status"
+
+
+def test_workspace_sizes():
+    w = bits.workspace_bytes
+    assert w(99, 1, 1) == 0
+    assert w(bits.FN_COUNT, 2**32, 1) == 0
+    small, big = w(bits.FN_COUNT, 10, 1000), w(bits.FN_COUNT, 10, 10_000_000)
+    assert 0 < small < big
+    assert big >= 4 * 4 * 10_000_000                      # two arrays, ping + pong
+    assert big % 256 == 0
+    mc_a = w(bits.FN_MC_ROUNDS, 10_000, 1_000_000, 24, bits.PERMUTE_A)
+    mc_b = w(bits.FN_MC_ROUNDS, 10_000, 1_000_000, 24, bits.PERMUTE_B)
+    assert mc_b > mc_a > w(bits.FN_COUNT, 10_000, 1_000_000)
+    assert w(bits.FN_MC_ROUNDS, 0, 0, 1, 0) > 0
+    assert bits.host_staging_bytes(bits.FN_MC_ROUNDS, 1000, 1000, 100) >= 4 * 4 * 1000 + 8 * 100
+
+
+def test_pvalue():
+    assert bits.pvalue(10, [], 0) == 1.0
+    assert bits.pvalue(10, [1, 2, 3], 0) == 1 / 4
+    assert bits.pvalue(10, [1, 2, 3], 1) == 1.0
+    assert bits.pvalue(2, [1, 2, 3, 2], 0) == 4 / 5
+    assert bits.pvalue(0, [5] * 99, 1) == 1 / 100
+    assert math.isnan(bits.pvalue(1, [1], 2))
+    big = 2**63 + 5                                        # uint64 range, not int64
+    assert bits.pvalue(big, np.array([big - 1, big, big + 1], dtype=np.uint64), 0) == 3 / 4
+
+
+def test_set_option_rejects_unknown():
+    with pytest.raises(bits.BitsError):
+        bits.set_option("no_such_knob", 1)
+    bits.set_option("grid_mult", 8)
+    with pytest.raises(bits.BitsError):
+        bits.set_option("grid_mult", 0)
+
+
+def test_host_side_argument_checks_return_before_cuda():
+    L = bits.lib()
+    fake = 0x1000  # never dereferenced: every call below must fail in the host checks
+    ws = 256 * 4
+    off = np.array([0, 100], dtype=np.uint32)
+    st = L.bits_count(fake, fake, 2**32, fake, fake, 1, 0, ws, 1 << 40, fake, None)
+    assert st == 2                                         # BITS_ERR_SIZE
+    assert L.bits_count(fake, fake, 1, fake, fake, 1, 8, ws, 1 << 40, fake, None) == 6     # flags
+    assert L.bits_count(None, fake, 1, fake, fake, 1, 0, ws, 1 << 40, fake, None) == 1     # null
+    assert L.bits_count(fake, fake, 1, fake, fake, 1, 0, ws, 1 << 40, None, None) == 1     # null out
+    assert L.bits_count(fake, fake, 1, fake, fake, 1, 0, None, 0, fake, None) == 5         # workspace
+    assert L.bits_count(fake, fake, 1, fake, fake, 1, 0, ws + 8, 1 << 40, fake, None) == 5  # misaligned
+    assert L.bits_count(fake, fake, 1, fake, fake, 1, 0, ws, 16, fake, None) == 5          # too small
+    assert L.bits_count_per_interval(fake, fake, 1, fake, fake, 1, 0, ws, 1 << 40, None, fake, None) == 1
+    mc = lambda o, nch, which, rb, nr: L.bits_mc_rounds(fake, fake, 1, fake, fake, 1, o, nch, which, 1, rb, nr, 0,
+                                                        ws, 1 << 40, fake, fake, None)
+    assert mc(off.ctypes.data, 1, 2, 0, 1) == 6                                            # which
+    assert mc(None, 1, 0, 0, 1) == 1
+    assert mc(off.ctypes.data, 0, 0, 0, 1) == 3                                            # n_chrom == 0
+    assert mc(off.ctypes.data, 1, 0, 2**32 - 1, 2) == 2                                    # round overflow
+    bad1 = np.array([1, 100], dtype=np.uint32)
+    bad2 = np.array([0, 100, 100], dtype=np.uint32)
+    assert mc(bad1.ctypes.data, 1, 0, 0, 1) == 3
+    assert mc(bad2.ctypes.data, 2, 0, 0, 1) == 3
+    assert L.bits_place(fake, 4, bad1.ctypes.data, 1, 1, 0, 0, ws, 1 << 40, fake, fake, None) == 3
+    assert L.bits_sort_u32(None, fake, 4, ws, 1 << 40, None) == 1
+    assert L.bits_sort_u32(fake, fake, 2**32, ws, 1 << 40, None) == 2

@@ -1,0 +1,334 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) against the CPU oracle.
+
+All comparisons are BIT-EXACT: the path is integer-only (uint32 coordinates and ranks, uint64
+sums), so there is no tolerance anywhere.  Run on the B200 box with  pytest -m gpu.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1208_3407_b200 import bits
+from paper_1208_3407_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def dev(a):
+    a = np.ascontiguousarray(a, dtype=np.uint32)
+    return torch.from_numpy(a.view(np.int32)).to(DEV)
+
+
+def host_u32(t):
+    return t.cpu().numpy().view(np.uint32)
+
+
+def host_u64(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+def sync():
+    torch.cuda.synchronize()
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    bits.lib()
+
+
+# ------------------------------------------------------------------------------------- sort
+@pytest.mark.parametrize("n", [0, 1, 2, 31, 33, 8191, 8192, 8193, 16384, 100_003, 1_000_000, 3_000_017])
+def test_sort_random_full_range(n):
+    rng = np.random.default_rng(n + 1)
+    k = rng.integers(0, 2**32, n, dtype=np.uint64).astype(np.uint32)
+    got = host_u32(bits.sort_u32(dev(k)))
+    assert np.array_equal(got, oracle.sort_u32(k))
+
+
+@pytest.mark.parametrize("kind", ["equal", "sorted", "reverse", "low_bits", "high_bits", "two_values", "max"])
+def test_sort_structured(kind):
+    n = 70_001
+    rng = np.random.default_rng(5)
+    k = {
+        "equal": np.full(n, 0xDEADBEEF, dtype=np.uint64),
+        "sorted": np.sort(rng.integers(0, 2**32, n, dtype=np.uint64)),
+        "reverse": np.sort(rng.integers(0, 2**32, n, dtype=np.uint64))[::-1],
+        "low_bits": rng.integers(0, 1000, n, dtype=np.uint64),
+        "high_bits": rng.integers(0, 200, n, dtype=np.uint64) << np.uint64(24),
+        "two_values": rng.integers(0, 2, n, dtype=np.uint64) * np.uint64(0xFFFFFFFF),
+        "max": np.full(n, 0xFFFFFFFF, dtype=np.uint64),
+    }[kind].astype(np.uint32)
+    assert np.array_equal(host_u32(bits.sort_u32(dev(k))), oracle.sort_u32(k))
+
+
+def test_sort_repeated_calls_share_workspace():
+    rng = np.random.default_rng(17)
+    n = 50_000
+    ws = torch.empty(bits.workspace_bytes(bits.FN_SORT, 0, n), dtype=torch.uint8, device=DEV)
+    ws.fill_(0xAB)                         # garbage workspace must not matter
+    for _ in range(5):
+        k = rng.integers(0, 2**32, n, dtype=np.uint64).astype(np.uint32)
+        assert np.array_equal(host_u32(bits.sort_u32(dev(k), workspace=ws)), np.sort(k))
+
+
+# ------------------------------------------------------------------------------------- place
+GEN = W.genome_offsets(W.GENOME24_LENGTHS)
+SMALL = np.array([0, 10, 25, 1000, 1003, 5000], dtype=np.uint32)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 1023, 1024, 1025, 250_001])
+def test_place_genome(n):
+    rng = np.random.default_rng(n)
+    spans = np.clip(np.rint(1000 * np.exp(rng.standard_normal(n))), 20, 100_000).astype(np.uint32) - 1
+    for seed, rnd, tag in ((1, 0, 0), (0xFEDCBA9876543210, 4_000_000_000, 1)):
+        s, e = bits.place(dev(spans), GEN, seed, rnd, tag)
+        os_, oe = oracle.place_round(spans, GEN, seed, rnd, tag)
+        assert np.array_equal(host_u32(s), os_) and np.array_equal(host_u32(e), oe)
+
+
+def test_place_general_path_some_chromosomes_too_short():
+    rng = np.random.default_rng(2)
+    spans = rng.integers(0, 900, 10_000).astype(np.uint32)     # many spans exceed chromosomes 0, 1, 3
+    s, e = bits.place(dev(spans), SMALL, 7, 3, 0)
+    os_, oe = oracle.place_round(spans, SMALL, 7, 3, 0)
+    assert np.array_equal(host_u32(s), os_) and np.array_equal(host_u32(e), oe)
+
+
+def test_place_many_chromosomes_and_unaligned_pointers():
+    rng = np.random.default_rng(3)
+    lens = rng.integers(1000, 5000, 1500)                      # table too large for shared memory
+    off = W.genome_offsets(lens)
+    spans = rng.integers(0, 999, 4099).astype(np.uint32)
+    d = dev(np.concatenate([[0], spans]))[1:]                  # 4-byte aligned only
+    s, e = bits.place(d, off, 11, 5, 1)
+    os_, oe = oracle.place_round(spans, off, 11, 5, 1)
+    assert np.array_equal(host_u32(s), os_) and np.array_equal(host_u32(e), oe)
+
+
+# ------------------------------------------------------------------------------------- count
+def check_counts(a_s, a_e, b_s, b_e, flags=0, b_for_gpu=None):
+    want_total, want_counts = oracle.count_per_interval(a_s, a_e, b_s, b_e)
+    gb_s, gb_e = b_for_gpu if b_for_gpu is not None else (b_s, b_e)
+    d = [dev(x) for x in (a_s, a_e, gb_s, gb_e)]
+    counts, total = bits.count_per_interval(*d, flags=flags)
+    total_only = bits.count(*d, flags=flags)
+    sync()
+    assert np.array_equal(host_u32(counts), want_counts)
+    assert int(host_u64(total)[0]) == want_total
+    assert int(host_u64(total_only)[0]) == want_total
+    return want_total
+
+
+def test_count_config1_tiny():
+    w = W.make_config(1)
+    check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
+
+
+@pytest.mark.parametrize("n_a,n_b", [(1, 1), (5, 3), (3, 5), (1000, 7), (7, 1000), (4097, 8193), (10_001, 70_001)])
+def test_count_random_ragged(n_a, n_b):
+    rng = np.random.default_rng(n_a * 31 + n_b)
+    a_s = rng.integers(0, 2**31, n_a, dtype=np.int64)
+    a_e = a_s + rng.integers(0, 2**22, n_a)
+    b_s = rng.integers(0, 2**31, n_b, dtype=np.int64)
+    b_e = b_s + rng.integers(0, 2**22, n_b)
+    check_counts(a_s, a_e, b_s, b_e)
+
+
+def test_count_dense_small_coordinates_with_ties():
+    rng = np.random.default_rng(12)
+    a_s = rng.integers(0, 300, 5000)
+    a_e = a_s + rng.integers(0, 40, 5000)
+    b_s = rng.integers(0, 300, 20_000)                         # thousands of duplicates per key
+    b_e = b_s + rng.integers(0, 40, 20_000)
+    check_counts(a_s, a_e, b_s, b_e)
+
+
+def test_count_edge_cases():
+    top = 2**32 - 2
+    check_counts([0, top - 5, 0, top, 5], [0, top, top, top, 5], [0, top, 7, top - 1], [0, top, 9, top])
+    K = 3000                                                   # nested B: the containment trap
+    k = np.arange(K)
+    check_counts(np.arange(0, K, 7), np.arange(0, K, 7), k, 2 * K - k)
+    check_counts([10, 10, 10, 10], [20, 20, 20, 20], [20, 21, 0, 0], [30, 30, 10, 9])   # shared endpoints
+    check_counts(np.arange(100), np.arange(100) + 3, np.full(5000, 50), np.full(5000, 60))  # one huge bucket
+    # keys equal to 0xffffffff (no genome table on the counting calls, so the full range is legal)
+    check_counts([0, 2**32 - 1], [2**32 - 1, 2**32 - 1], [2**32 - 1, 5, 2**32 - 1], [2**32 - 1, 2**32 - 1, 2**32 - 1])
+
+
+def test_count_empty_sets():
+    a = dev([1, 5]), dev([3, 9])
+    e = dev([]), dev([])
+    counts, total = bits.count_per_interval(*a, *e)
+    sync()
+    assert host_u32(counts).tolist() == [0, 0] and int(host_u64(total)[0]) == 0
+    counts, total = bits.count_per_interval(*e, *a)
+    sync()
+    assert counts.numel() == 0 and int(host_u64(total)[0]) == 0
+    assert int(host_u64(bits.count(*e, *e))[0]) == 0
+
+
+def test_count_flags_sorted_and_validate():
+    w = W.make_config(2, scale=0.02)
+    bs, be = np.sort(w.b_start), np.sort(w.b_end)
+    check_counts(w.a_start, w.a_end, w.b_start, w.b_end, flags=bits.B_SORTED, b_for_gpu=(bs, be))
+    check_counts(w.a_start, w.a_end, w.b_start, w.b_end, flags=bits.VALIDATE)
+    bad_e = w.a_end.copy()
+    bad_e[123] = w.a_start[123] - 1
+    with pytest.raises(bits.BitsError) as ei:
+        bits.count(dev(w.a_start), dev(bad_e), dev(w.b_start), dev(w.b_end), flags=bits.VALIDATE)
+    assert ei.value.status == 7
+
+
+def test_count_unaligned_query_pointers():
+    w = W.make_config(2, scale=0.01)
+    a_s = dev(np.concatenate([[0], w.a_start]))[1:]
+    a_e = dev(np.concatenate([[0], w.a_end]))[1:]
+    want_total, want_counts = oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end)
+    counts, total = bits.count_per_interval(a_s, a_e, dev(w.b_start), dev(w.b_end))
+    sync()
+    assert np.array_equal(host_u32(counts), want_counts) and int(host_u64(total)[0]) == want_total
+
+
+def test_count_config2_full_size():
+    w = W.make_config(2)
+    total = check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
+    assert 0.5e6 < total < 1.5e6
+    # count(A, B) = count(B, A), and self-comparison >= N, at full size on the GPU path
+    t_ba = bits.count(dev(w.b_start), dev(w.b_end), dev(w.a_start), dev(w.a_end))
+    t_aa = bits.count(dev(w.a_start), dev(w.a_end), dev(w.a_start), dev(w.a_end))
+    sync()
+    assert int(host_u64(t_ba)[0]) == total and int(host_u64(t_aa)[0]) >= w.n_a
+
+
+def test_count_config4_full_size():
+    w = W.make_config(4)
+    total = check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
+    assert total > 5e7
+
+
+# ------------------------------------------------------------------------------------- Monte Carlo
+def run_mc(w, which, seed, r0, n, flags=0):
+    obs, rc = bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, which,
+                             seed, r0, n, flags=flags)
+    sync()
+    return int(host_u64(obs)[0]), host_u64(rc)
+
+
+@pytest.mark.parametrize("which", [0, 1])
+def test_mc_config1_all_rounds(which):
+    w = W.make_config(1)
+    obs, rc = run_mc(w, which, w.mc_seed, 0, 100)
+    o_obs, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, which, w.mc_seed, 0, 100)
+    assert obs == o_obs and np.array_equal(rc, o_rc)
+    assert bits.pvalue(obs, rc, 0) == oracle.pvalue(o_obs, o_rc, 0)
+    assert bits.pvalue(obs, rc, 1) == oracle.pvalue(o_obs, o_rc, 1)
+
+
+@pytest.mark.parametrize("which", [0, 1])
+def test_mc_round_slicing_and_big_round_numbers(which):
+    w = W.make_config(1)
+    seed = 0xA5A5_5A5A_1234_5678
+    _, full = run_mc(w, which, seed, 4_294_967_000, 40)
+    _, lo = run_mc(w, which, seed, 4_294_967_000, 13)
+    _, hi = run_mc(w, which, seed, 4_294_967_013, 27)
+    assert np.array_equal(full, np.concatenate([lo, hi]))
+    _, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, which, seed, 4_294_967_000, 40)
+    assert np.array_equal(full, o_rc)
+
+
+@pytest.mark.parametrize("k,which,scale,rounds", [(3, 0, 0.1, 60), (5, 1, 0.01, 12), (3, 1, 0.05, 6), (5, 0, 0.01, 9)])
+def test_mc_scaled_configs(k, which, scale, rounds):
+    w = W.make_config(k, scale=scale)
+    obs, rc = run_mc(w, which, 1, 0, rounds)
+    o_obs, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, which, 1, 0, rounds)
+    assert obs == o_obs and np.array_equal(rc, o_rc)
+
+
+def test_mc_small_genome_general_placement_path():
+    rng = np.random.default_rng(6)
+    off = np.array([0, 40_000, 41_000, 90_000, 100_000], dtype=np.uint32)
+    lo = np.array([0, 41_000, 90_000])
+    a_s = lo[rng.integers(0, 3, 3000)] + rng.integers(0, 3000, 3000)
+    a_e = a_s + rng.integers(0, 2500, 3000)                    # spans above the 1,000 bp chromosome
+    b_s = lo[rng.integers(0, 3, 5000)] + rng.integers(0, 3000, 5000)
+    b_e = b_s + rng.integers(0, 2500, 5000)
+    for which in (0, 1):
+        obs, rc = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, which, 9, 0, 15)
+        sync()
+        o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, which, 9, 0, 15)
+        assert int(host_u64(obs)[0]) == o_obs and np.array_equal(host_u64(rc), o_rc)
+
+
+def test_mc_errors_and_degenerate():
+    off = np.array([0, 1000, 3000], dtype=np.uint32)
+    a = dev([1, 5]), dev([3, 9])
+    e = dev([]), dev([])
+    for which in (0, 1):
+        obs, rc = bits.mc_rounds(*a, *e, off, which, 1, 0, 4)
+        sync()
+        assert int(host_u64(obs)[0]) == 0 and not host_u64(rc).any()
+        obs, rc = bits.mc_rounds(*e, *a, off, which, 1, 0, 4)
+        sync()
+        assert int(host_u64(obs)[0]) == 0 and not host_u64(rc).any()
+        obs, rc = bits.mc_rounds(*a, *a, off, which, 1, 0, 0)
+        sync()
+        assert int(host_u64(obs)[0]) == oracle.count([1, 5], [3, 9], [1, 5], [3, 9]) and rc.numel() == 0
+    long_ = dev([0]), dev([2000])                              # span 2000 >= longest chromosome (2000)
+    with pytest.raises(bits.BitsError) as ei:
+        bits.mc_rounds(*long_, *a, off, 0, 1, 0, 4)
+    assert ei.value.status == 4
+    obs, rc = bits.mc_rounds(*a, *long_, off, 0, 1, 0, 4)       # the long interval is not permuted: fine
+    sync()
+
+
+def test_mc_config3_full_size_sampled_rounds():
+    w = W.make_config(3)
+    obs, rc = run_mc(w, 0, 1, 0, 10_000)
+    o_obs, o_lo = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 0, 1, 0, 150)
+    _, o_hi = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 0, 1, 9_900, 100)
+    assert obs == o_obs
+    assert np.array_equal(rc[:150], o_lo) and np.array_equal(rc[9_900:], o_hi)
+    assert rc.min() > 0 and 0.5 < rc.mean() / 1.3e4 < 2.0       # every round ran; E[count] ~ 1.3e4
+
+
+def test_mc_config5_full_size_sampled_rounds():
+    w = W.make_config(5)
+    obs, rc = run_mc(w, 1, 1, 0, 40)
+    o_obs, o_lo = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 1, 0, 2)
+    _, o_hi = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 1, 39, 1)
+    assert obs == o_obs
+    assert np.array_equal(rc[:2], o_lo) and rc[39] == o_hi[0]
+    assert rc.min() > 0 and np.unique(rc).size > 30
+    # the other search design (bucket index rebuilt per round) must give the same integers
+    bits.set_option("mc_sorted_queries", 0)
+    bits.set_option("place_fused_hist", 0)
+    try:
+        _, rc2 = run_mc(w, 1, 1, 0, 3)
+    finally:
+        bits.set_option("mc_sorted_queries", 1)
+        bits.set_option("place_fused_hist", 1)
+    assert np.array_equal(rc2, rc[:3])
+
+
+# ------------------------------------------------------------------------------------- host-buffer entry points
+def test_host_variants_config1():
+    w = W.make_config(1)
+    o_total, o_counts = oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end)
+    assert bits.count_host(w.a_start, w.a_end, w.b_start, w.b_end) == o_total
+    counts, total = bits.count_per_interval_host(w.a_start, w.a_end, w.b_start, w.b_end)
+    assert total == o_total and np.array_equal(counts, o_counts)
+    for which in (0, 1):
+        r = bits.mc_rounds_host(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, which, 1, 0, 25)
+        o_obs, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, which, 1, 0, 25)
+        assert r.observed == o_obs and np.array_equal(r.round_counts, o_rc)
+        assert r.p_enrich == oracle.pvalue(o_obs, o_rc, 0) and r.p_deplete == oracle.pvalue(o_obs, o_rc, 1)
+
+
+def test_launches_are_counted():
+    before = bits.launch_count()
+    w = W.make_config(1)
+    bits.count(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end))
+    sync()
+    assert bits.launch_count() >= before + 7     # histogram + 4 passes + index + count
