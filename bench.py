@@ -1,0 +1,407 @@
+#!/usr/bin/env python
+"""bench.py -- Monte Carlo rounds/s of the BITS hot path (place -> sort -> search -> reduce) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 5] [--rounds R]
+
+Workload (config.workload): BASELINE.json configs[4], "Monte Carlo at scale with per-round sort":
+24-chromosome genome, A = 1e6 query intervals, B = 1e7 intervals re-placed with Philox and radix-
+sorted (starts and ends) every round, all of A counted and reduced per round.  One STEP is one
+bits_mc_rounds call of R rounds (default R = 1000, the configuration's round count), i.e. R passes
+of the whole hot path, plus the one-off observed count.  value = rounds/s over K timed steps with
+the inputs resident in HBM; e2e = the same through bits_mc_rounds_host with pinned HOST buffers
+(H2D of A and B and D2H of the counts inside the timed region).
+
+Under torchrun (N > 1) every rank runs its own R rounds (round_begin = rank * R): the rounds of a
+Monte Carlo job are independent, so they shard with no data-path collective ("weak" scaling).
+
+--impl reference times the CPU oracle (oracle/, single-threaded C++) on the same workload, each
+step a bounded sample of rounds.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=5)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    p.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    p.add_argument("--scale", type=float, default=1.0, help="scale the set sizes (testing only; 1.0 = the named config)")
+    p.add_argument("--rounds", type=int, default=0, help="rounds per step (0 = the configuration's own count)")
+    p.add_argument("--no-extras", action="store_true", help="skip the secondary workloads, e2e and cpu_baseline legs")
+    p.add_argument("--no-profile-events", action="store_true", help="do not bracket kernels with events in the timed region")
+    return p.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth)"
+    return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        with open(self.path) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) < 7:
+                    continue
+                try:
+                    sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+                except ValueError:
+                    continue
+                for n, v in zip(names, c[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+        os.unlink(self.path)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_name(k: int) -> str:
+    from paper_1208_3407_b200 import workloads as W
+    return W.CONFIG_NAMES[k]
+
+
+def config_block(w, rounds: int, n_gpus: int) -> dict:
+    return {"workload": w.name, "n_a": w.n_a, "n_b": w.n_b, "n_chrom": int(w.chrom_offsets.size - 1),
+            "rounds_per_step": rounds, "which": {0: "permute_A", 1: "permute_B", None: "count"}[w.which],
+            "mc_seed": w.mc_seed, "data_seed": w.spec.get("seed"), "scale": w.spec.get("scale", 1.0),
+            "parallelism": f"rounds sharded over {n_gpus} GPU(s), no collective",
+            "l2": "no flush: every round re-writes and re-sorts 160 MB of keys plus 160 MB of ping-pong buffers (> 126 MB L2)"}
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def oracle_marginal_rounds_per_s(w, which: int, round_begin: int, n_rounds: int):
+    """Oracle rounds/s from the marginal cost of n_rounds rounds: t(R = n_rounds) - t(R = 0).
+    (The R = 0 call is the one-off observed count, which a 1000-round job amortises away.)"""
+    import oracle
+    args = (w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, which, w.mc_seed)
+    t0 = time.perf_counter(); oracle.mc_rounds(*args, round_begin, 0); t_obs = time.perf_counter() - t0
+    t0 = time.perf_counter(); oracle.mc_rounds(*args, round_begin, n_rounds); t_r = time.perf_counter() - t0
+    per_round = max((t_r - t_obs) / n_rounds, 1e-9)
+    return 1.0 / per_round, t_obs, t_r
+
+
+def oracle_sample_text(n_rounds: int, w) -> str:
+    return (f"{n_rounds} of the workload's {w.n_rounds} rounds per step (full-size A and B): time of "
+            f"oracle.mc_rounds(R={n_rounds}) minus time of oracle.mc_rounds(R=0), i.e. the marginal per-round "
+            f"cost (place {w.n_b if w.which == 1 else w.n_a} intervals, std::sort both key arrays, {w.n_a} ICOUNTs, sum)")
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_1208_3407_b200 import workloads as W
+    oracle.build()
+    w = W.make_config(args.config, scale=args.scale)
+    if w.which is None:
+        raise SystemExit("--impl reference times the Monte Carlo configs (1, 3, 5)")
+    r_sample = 1 if args.config == 5 else (args.rounds or 100)
+    for i in range(args.warmup):
+        oracle_marginal_rounds_per_s(w, w.which, i * r_sample, r_sample)
+    t_total, rounds_total, per_step = 0.0, 0, []
+    for i in range(args.steps):
+        rps, _, _ = oracle_marginal_rounds_per_s(w, w.which, (args.warmup + i) * r_sample, r_sample)
+        per_step.append(rps)
+        t_total += r_sample / rps
+        rounds_total += r_sample
+    value = rounds_total / t_total
+    line = {
+        "impl": "reference", "metric": "mc_rounds_per_s", "value": value, "unit": "rounds/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": config_block(w, r_sample, args.gpus),
+        "cpu_baseline": {"value": value, "unit": "rounds/s", "cores": 1, "kind": "oracle",
+                         "sample": oracle_sample_text(r_sample, w)},
+        "e2e": {"value": value, "unit": "rounds/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "intervals_searched_per_s": value * w.n_a,
+        "host_cores": os.cpu_count(),
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ B200 arm
+def to_dev(a, device):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.uint32).view(np.int32)).to(device)
+
+
+def pinned(a):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a, dtype=np.uint32).view(np.int32)).pin_memory()
+    return t, t.numpy().view(np.uint32)
+
+
+def time_device(fn, reps: int, warmup: int = 3):
+    """Median and min device time (ms) of fn() by CUDA events on the current stream."""
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); fn(); b.record(); b.synchronize()
+        ts.append(a.elapsed_time(b))
+    return statistics.median(ts), min(ts)
+
+
+def secondary_workloads(device, peak_gbs):
+    """The other throughputs BASELINE.json's metric names, on their own configs (not the timed headline)."""
+    import torch
+    from paper_1208_3407_b200 import bits
+    from paper_1208_3407_b200 import workloads as W
+    out = {}
+    # config 4: 1e7 queries counted against 1e7 intervals (sort B once + per-interval search + reduce)
+    w = W.make_config(4)
+    d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    ws = torch.empty(bits.workspace_bytes(bits.FN_COUNT_PER_INTERVAL, w.n_a, w.n_b), dtype=torch.uint8, device=device)
+    counts = torch.empty(w.n_a, dtype=torch.int32, device=device)
+    total = torch.empty(1, dtype=torch.int64, device=device)
+    bits.set_option("profile", 2); bits.set_option("profile", 1)
+    med, mn = time_device(lambda: bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total), 10)
+    prof = bits.profile_read(); bits.set_option("profile", 0)
+    ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in prof.items()}
+    sort_ms = ms["histogram"] + 4 * ms["sort_pass"]
+    out["cfg4_large_count_10M"] = {
+        "intervals_searched_per_s": w.n_a / (med * 1e-3), "ms_median": med, "ms_min": mn,
+        "sort_keys_per_s": 2 * w.n_b / (sort_ms * 1e-3) if sort_ms else None,
+        "kernel_ms": {"histogram": ms["histogram"], "sort_pass": ms["sort_pass"], "index_build": ms["index_build"],
+                      "count": ms["count"]},
+        "hbm_bytes_model": 72 * w.n_b + 12 * w.n_a + 8 * w.n_b,
+        "hbm_frac_of_peak": (72 * w.n_b + 12 * w.n_a + 8 * w.n_b) / (med * 1e-3) / 1e9 / peak_gbs,
+    }
+    del d, ws, counts
+    # config 3: 1e4 queries re-placed per round against a fixed 1e6-interval B, 10,000 rounds, fused kernel
+    w = W.make_config(3)
+    d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, w.n_a, w.n_b, 24, 0), dtype=torch.uint8, device=device)
+    obs = torch.empty(1, dtype=torch.int64, device=device)
+    rc = torch.empty(w.n_rounds, dtype=torch.int64, device=device)
+    med, mn = time_device(lambda: bits.mc_rounds(*d, w.chrom_offsets, 0, w.mc_seed, 0, w.n_rounds, workspace=ws,
+                                                 observed_out=obs, round_counts_out=rc), 5)
+    out["cfg3_mc_permuteA_1e4x1M"] = {"mc_rounds_per_s": w.n_rounds / (med * 1e-3),
+                                      "intervals_searched_per_s": w.n_rounds * w.n_a / (med * 1e-3),
+                                      "ms_median": med, "ms_min": mn}
+    # config 2: 1e6 x 1e6 count
+    w = W.make_config(2)
+    d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    ws = torch.empty(bits.workspace_bytes(bits.FN_COUNT_PER_INTERVAL, w.n_a, w.n_b), dtype=torch.uint8, device=device)
+    med, mn = time_device(lambda: bits.count_per_interval(*d, workspace=ws), 10)
+    out["cfg2_genome_count_1M"] = {"intervals_searched_per_s": w.n_a / (med * 1e-3), "ms_median": med, "ms_min": mn}
+    return out
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1208_3407_b200 import bits
+    from paper_1208_3407_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    bits.lib()
+
+    w = W.make_config(args.config, scale=args.scale)
+    if w.which is None:
+        raise SystemExit("the timed headline is a Monte Carlo config (1, 3 or 5); counts are reported as extras")
+    R = args.rounds or w.n_rounds
+    r0 = rank * R                                         # this rank's slice of the round space
+    n_chrom = int(w.chrom_offsets.size - 1)
+    d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, w.which), dtype=torch.uint8, device=device)
+    obs = torch.empty(1, dtype=torch.int64, device=device)
+    rc = torch.empty(R, dtype=torch.int64, device=device)
+
+    def step():
+        bits.mc_rounds(*d, w.chrom_offsets, w.which, w.mc_seed, r0, R, workspace=ws, observed_out=obs, round_counts_out=rc)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    profile_events = not args.no_profile_events
+    bits.set_option("profile", 2)
+    bits.set_option("profile", 1 if profile_events else 0)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = bits.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    barrier()
+    elapsed_ms = ev0.elapsed_time(ev1)
+    launches = bits.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    prof = bits.profile_read()
+    bits.set_option("profile", 0)
+    if world > 1:
+        t = torch.tensor([elapsed_ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(t.item())
+        lt = torch.tensor([launches], dtype=torch.int64, device=device)
+        dist.all_reduce(lt, op=dist.ReduceOp.SUM)
+        launches = int(lt.item())
+    rounds_total = world * R * args.steps
+    value = rounds_total / (elapsed_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (one digit pass of the radix sort over both key arrays) ----
+    peak, peak_src = measured_peaks()
+    n_sorted = w.n_b if w.which == 1 else 0
+    roofline = None
+    if prof["sort_pass"][1] and n_sorted:
+        pass_ms = prof["sort_pass"][0] / prof["sort_pass"][1]
+        alg_bytes = 2 * n_sorted * 8                      # two arrays x (4 B read + 4 B write) per key
+        achieved = alg_bytes / (pass_ms * 1e-3) / 1e9
+        shares = {k: v[0] for k, v in prof.items() if v[1]}
+        tot = sum(shares.values())
+        roofline = {"bound": "hbm", "kernel": "onesweep_pass_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                    "avg_launch_ms": pass_ms, "launches_timed": prof["sort_pass"][1],
+                    "algorithmic_bytes_per_launch": alg_bytes,
+                    "kernel_ms_per_round": {k: v[0] / (R * args.steps) for k, v in prof.items() if v[1]},
+                    "kernel_share_of_step": {k: v / tot for k, v in shares.items()},
+                    "round_hbm_bytes_model": 12 * n_sorted + 72 * n_sorted - 8 * n_sorted + 8 * w.n_a,
+                    }
+        roofline["round_frac_of_peak"] = roofline["round_hbm_bytes_model"] * value / world / 1e9 / peak
+
+    line = {
+        "metric": "mc_rounds_per_s", "value": value, "unit": "rounds/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": elapsed_ms / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": config_block(w, R, world), "gpu_launches": launches,
+        "intervals_searched_per_s": value * w.n_a,
+        "sort_keys_per_s": (2 * n_sorted * value) if n_sorted else None,
+        "profile_events_in_timed_region": profile_events,
+    }
+    if roofline:
+        line["roofline"] = roofline
+        line["sort_keys_per_s_kernel_only"] = 2 * n_sorted / (4 * roofline["avg_launch_ms"] * 1e-3)
+    if clocks is not None:
+        line["clocks"] = clocks
+
+    # ---- end to end through the host-buffer entry point (H2D + run + D2H inside the timed region) ----
+    if not args.no_extras:
+        hp = [pinned(x) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+        hws = bits.host_workspace(bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, w.which, R, device=device)
+        rc_host_t = torch.empty(R, dtype=torch.int64).pin_memory()
+        rc_host = rc_host_t.numpy().view(np.uint64)
+
+        def e2e_step():
+            return bits.mc_rounds_host(hp[0][1], hp[1][1], hp[2][1], hp[3][1], w.chrom_offsets, w.which, w.mc_seed,
+                                       r0, R, workspace=hws, device=device, round_counts_out=rc_host)
+        del ws
+        for _ in range(min(args.warmup, 2)):
+            e2e_step()
+        barrier()
+        e2e_steps = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            res = e2e_step()
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        line["e2e"] = {"value": world * R * e2e_steps / t_e2e, "unit": "rounds/s",
+                       "h2d_bytes_per_step": 4 * 2 * (w.n_a + w.n_b) + 4 * (n_chrom + 1),
+                       "d2h_bytes_per_step": 8 * R + 8, "steps": e2e_steps, "api": "bits_mc_rounds_host (pinned host buffers)",
+                       "observed": res.observed, "p_enrich": res.p_enrich, "p_deplete": res.p_deplete}
+        # the device-resident and host-buffer paths must agree bit for bit
+        same = bool(np.array_equal(rc.cpu().numpy().view(np.uint64), rc_host))
+        line["e2e"]["matches_device_path"] = same
+        del hws, hp
+
+    if rank == 0 and world == 1 and not args.no_extras:
+        line["other_workloads"] = secondary_workloads(device, peak)
+        n_cpu = 2 if args.config == 5 else 50
+        rps, t_obs, t_r = oracle_marginal_rounds_per_s(w, w.which, 0, n_cpu)
+        line["cpu_baseline"] = {"value": rps, "unit": "rounds/s", "cores": 1, "kind": "oracle",
+                                "sample": oracle_sample_text(n_cpu, w), "observed_count_s": t_obs,
+                                "host_cores": os.cpu_count()}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

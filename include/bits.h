@@ -164,6 +164,13 @@ double bits_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n_r
 /* Kernels launched by this library in this process since load (for bench.py's gpu_launches). */
 uint64_t bits_launch_count(void);
 
+/* Per-kernel-class device time, measured with CUDA events on the launching stream while
+ * bits_set_option("profile", 1) is on (2 resets the totals).  cls: 0 place, 1 histogram,
+ * 2 sort pass, 3 index build, 4 count (search + reduce), 5 sorted-query search + reduce,
+ * 6 fused Monte Carlo kernel (place + search + reduce), 7 other.  Synchronises the recorded
+ * events.  ms_out / launches_out: host pointers, may be NULL. */
+int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out);
+
 /* Tuning knobs for design studies (bench.py --study); returns BITS_ERR_FLAGS for an unknown
  * name.  They never change results.  Names are listed in DESIGN.md "Knobs". */
 int bits_set_option(const char* name, int64_t value);

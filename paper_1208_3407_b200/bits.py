@@ -47,6 +47,7 @@ _SIGNATURES = {
                                       _vp]),
     "bits_pvalue": (C.c_double, [C.c_uint64, _u64p, C.c_uint32, C.c_int]),
     "bits_launch_count": (C.c_uint64, []),
+    "bits_profile_read": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p]),
     "bits_set_option": (C.c_int, [C.c_char_p, C.c_int64]),
     "bits_strerror": (C.c_char_p, [C.c_int]),
     "bits_version": (C.c_char_p, []),
@@ -96,6 +97,19 @@ def launch_count() -> int:
 
 def set_option(name: str, value: int) -> None:
     _chk(lib().bits_set_option(name.encode(), int(value)))
+
+
+PROFILE_CLASSES = ("place", "histogram", "sort_pass", "index_build", "count", "sorted_query", "mc_permute_a", "other")
+
+
+def profile_read() -> dict:
+    """{class: (milliseconds, launches)} accumulated while set_option("profile", 1) was on."""
+    out = {}
+    for i, name in enumerate(PROFILE_CLASSES):
+        ms, n = C.c_double(0), C.c_uint64(0)
+        _chk(lib().bits_profile_read(i, C.addressof(ms), C.addressof(n)))
+        out[name] = (ms.value, int(n.value))
+    return out
 
 
 def workspace_bytes(fn: int, n_a: int, n_b: int, n_chrom: int = 0, which: int = 0, flags: int = 0) -> int:

@@ -4,6 +4,8 @@
 #include <math.h>
 #include <string.h>
 
+#include <vector>
+
 #include "common.cuh"
 #include "philox_place.cuh"
 #include "place_kernels.cuh"
@@ -22,6 +24,51 @@ struct Options {
 static Options g_opt;
 
 constexpr int kSMs = 148;
+
+// ---------------------------------------------------------------------------------------------
+// Optional per-kernel-class timing with CUDA events on the launching stream (bits_set_option
+// "profile" = 1; read with bits_profile_read).  Used by bench.py for the roofline figures.
+enum { kClsPlace = 0, kClsHist, kClsSortPass, kClsIndex, kClsCount, kClsSortedQuery, kClsMcA, kClsOther, kNumCls };
+struct Profiler {
+  bool on = false;
+  std::vector<cudaEvent_t> ev;     // pairs: 2k = start, 2k+1 = stop
+  std::vector<int> cls;            // class of pair k
+  size_t used = 0;                 // pairs in flight
+  double ms[kNumCls] = {0};
+  uint64_t launches[kNumCls] = {0};
+  void collect() {
+    for (size_t k = 0; k < used; ++k) {
+      float t = 0.f;
+      if (cudaEventSynchronize(ev[2 * k + 1]) == cudaSuccess &&
+          cudaEventElapsedTime(&t, ev[2 * k], ev[2 * k + 1]) == cudaSuccess) {
+        ms[cls[k]] += t;
+        ++launches[cls[k]];
+      }
+    }
+    (void)cudaGetLastError();
+    used = 0;
+  }
+  void reset() { collect(); for (int i = 0; i < kNumCls; ++i) { ms[i] = 0; launches[i] = 0; } }
+};
+static Profiler g_prof;
+
+struct ProfScope {
+  cudaStream_t st;
+  long k = -1;
+  ProfScope(int c, cudaStream_t s) : st(s) {
+    if (!g_prof.on) return;
+    if (g_prof.used >= (1u << 16)) g_prof.collect();
+    if (g_prof.ev.size() < 2 * (g_prof.used + 1)) {
+      cudaEvent_t a, b;
+      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { (void)cudaGetLastError(); return; }
+      g_prof.ev.push_back(a); g_prof.ev.push_back(b); g_prof.cls.push_back(c);
+    }
+    k = (long)g_prof.used++;
+    g_prof.cls[k] = c;
+    cudaEventRecord(g_prof.ev[2 * k], st);
+  }
+  ~ProfScope() { if (k >= 0) cudaEventRecord(g_prof.ev[2 * k + 1], st); }
+};
 
 // ---------------------------------------------------------------------------------------------
 // Workspace: a bump allocator that is run twice -- once with base == nullptr to size, once to carve.
@@ -148,6 +195,7 @@ static int launch_sort_passes(const SortPlan& p, uint32_t* epoch, cudaStream_t s
       a.arr[k].ticket = p.ticket + k;
     }
     a.n = p.n; a.n_tiles = p.n_tiles; a.shift = 8 * pass; a.epoch = (*epoch)++;
+    ProfScope prof(kClsSortPass, st);
     rs::onesweep_pass_kernel<<<dim3(p.n_tiles, p.n_arrays), rs::kThreads, 0, st>>>(a);
     BITS_LAUNCH_CHECK();
   }
@@ -160,6 +208,7 @@ static int launch_histogram(const uint32_t* k0, const uint32_t* k1, uint32_t* h0
   h.keys[0] = k0; h.keys[1] = n_arrays > 1 ? k1 : k0;
   h.hist[0] = h0; h.hist[1] = n_arrays > 1 ? h1 : h0;
   h.n = n;
+  ProfScope prof(kClsHist, st);
   rs::histogram_kernel<<<dim3(grid_for(ceil_div(n, 4), 512), n_arrays), 512, 0, st>>>(h);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
@@ -196,6 +245,7 @@ static int launch_build_index(const SortCtx& c, cudaStream_t st) {
   ia.idx[0] = c.idx[0]; ia.idx[1] = c.idx[1];
   ia.n = c.n; ia.shift = c.shift;
   const uint64_t threads = (uint64_t)c.n + 1 > (uint64_t)kPad ? (uint64_t)c.n + 1 : (uint64_t)kPad;
+  ProfScope prof(kClsIndex, st);
   build_index_kernel<<<dim3((unsigned)ceil_div(threads, 256), 2), 256, 0, st>>>(ia);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
@@ -225,6 +275,7 @@ static int launch_count(const uint32_t* a_start, const uint32_t* a_end, uint32_t
                         uint32_t* counts, uint64_t* total, cudaStream_t st) {
   const bool vec = (((uintptr_t)a_start | (uintptr_t)a_end | (uintptr_t)counts) & 15) == 0;
   const int grid = grid_for(ceil_div(n_a, 4), 256);
+  ProfScope prof(kClsCount, st);
   if (vec)
     count_kernel<true><<<grid, 256, 0, st>>>(a_start, a_end, n_a, sorted_set(b, 0), sorted_set(b, 1), counts,
                                              reinterpret_cast<unsigned long long*>(total));
@@ -305,6 +356,7 @@ static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* en
   a.spans = spans; a.start_out = start_out; a.end_out = end_out; a.n = n; a.round = round; a.tag = tag;
   a.key = key; a.chrom = chrom; a.hist_start = hist_s; a.hist_end = hist_e; a.zero_a = zero_s; a.zero_b = zero_e;
   const int grid = grid_for(ceil_div(n, 4), 256);
+  ProfScope prof(kClsPlace, st);
   if (hist_s) {
     if (vec) place_kernel<true, true><<<grid, 256, 0, st>>>(a); else place_kernel<false, true><<<grid, 256, 0, st>>>(a);
   } else {
@@ -366,6 +418,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     for (uint32_t done = 0; done < n_rounds;) {
       const uint32_t chunk = n_rounds - done < 32768u ? n_rounds - done : 32768u;
       m.round0 = round_begin + done; m.out0 = done;
+      ProfScope prof(kClsMcA, st);
       mc_permute_a_kernel<<<dim3(gx, chunk), 256, 0, st>>>(m);
       BITS_LAUNCH_CHECK();
       done += chunk;
@@ -406,6 +459,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     BITS_TRY(launch_sort_passes(plan_for(L.b, L.b.buf[0][0], L.b.buf[1][0], par), &epoch, st));
     unsigned long long* out = reinterpret_cast<unsigned long long*>(round_counts_out + k);
     if (g_opt.mc_sorted_queries) {
+      ProfScope prof(kClsSortedQuery, st);
       sorted_query_total_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(q_end_sorted, q_start_sorted, (uint32_t)n_a,
                                                                     L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, out);
       BITS_LAUNCH_CHECK();
@@ -597,10 +651,22 @@ double bits_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n_r
 
 uint64_t bits_launch_count(void) { return g_launches; }
 
+int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
+  if (cls < 0 || cls >= kNumCls) return BITS_ERR_FLAGS;
+  g_prof.collect();
+  if (ms_out) *ms_out = g_prof.ms[cls];
+  if (launches_out) *launches_out = g_prof.launches[cls];
+  return BITS_OK;
+}
+
 int bits_set_option(const char* name, int64_t value) {
   if (!name) return BITS_ERR_NULL;
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }
   if (!strcmp(name, "place_fused_hist")) { g_opt.place_fused_hist = value; return BITS_OK; }
+  if (!strcmp(name, "profile")) {   // 0 = off, 1 = on, 2 = reset the accumulated times
+    if (value == 2) g_prof.reset(); else g_prof.on = value != 0;
+    return BITS_OK;
+  }
   if (!strcmp(name, "grid_mult")) { if (value < 1 || value > 64) return BITS_ERR_FLAGS; g_opt.grid_mult = value; return BITS_OK; }
   return BITS_ERR_FLAGS;
 }
