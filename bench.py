@@ -267,7 +267,8 @@ def run_b200(args):
     if w.which is None:
         raise SystemExit("the timed headline is a Monte Carlo config (1, 3 or 5); counts are reported as extras")
     R = args.rounds or w.n_rounds
-    r0 = rank * R                                         # this rank's slice of the round space
+    from paper_1208_3407_b200 import shard
+    r0, _ = shard.weak_slice(rank, R)                     # this rank's slice of the round space
     n_chrom = int(w.chrom_offsets.size - 1)
     d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
     ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, w.which), dtype=torch.uint8, device=device)
