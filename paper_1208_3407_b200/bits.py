@@ -99,7 +99,8 @@ def set_option(name: str, value: int) -> None:
     _chk(lib().bits_set_option(name.encode(), int(value)))
 
 
-PROFILE_CLASSES = ("place", "histogram", "sort_pass", "index_build", "count", "sorted_query", "mc_permute_a", "other")
+PROFILE_CLASSES = ("place", "histogram", "sort_pass", "index_build", "count", "sorted_query", "mc_permute_a", "other",
+                   "plan", "scatter", "bucket_sort", "place_scatter", "bucket_sort_search")
 
 
 def profile_read() -> dict:

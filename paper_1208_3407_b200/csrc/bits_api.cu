@@ -10,6 +10,8 @@
 #include "philox_place.cuh"
 #include "place_kernels.cuh"
 #include "radix_sort.cuh"
+#include "msd_sort.cuh"
+#include "mc_fused.cuh"
 #include "search.cuh"
 
 namespace bits {
@@ -17,6 +19,8 @@ namespace bits {
 unsigned long long g_launches = 0;
 
 struct Options {
+  int64_t sort_msd = 1;            // 1 = MSD bucket sort with the LSD sort as device-side fallback, 0 = LSD sort only
+  int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+scatter / slab plan / bucket sort+search (mc_fused.cuh)
   int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
   int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
@@ -28,7 +32,8 @@ constexpr int kSMs = 148;
 // ---------------------------------------------------------------------------------------------
 // Optional per-kernel-class timing with CUDA events on the launching stream (bits_set_option
 // "profile" = 1; read with bits_profile_read).  Used by bench.py for the roofline figures.
-enum { kClsPlace = 0, kClsHist, kClsSortPass, kClsIndex, kClsCount, kClsSortedQuery, kClsMcA, kClsOther, kNumCls };
+enum { kClsPlace = 0, kClsHist, kClsSortPass, kClsIndex, kClsCount, kClsSortedQuery, kClsMcA, kClsOther,
+       kClsPlan, kClsScatter, kClsBucketSort, kClsPlaceScatter, kClsBucketSortSearch, kNumCls };
 struct Profiler {
   bool on = false;
   std::vector<cudaEvent_t> ev;     // pairs: 2k = start, 2k+1 = stop
@@ -94,6 +99,12 @@ struct SortCtx {
   uint32_t* ticket = nullptr;                                       // uint32[2]
   uint32_t* idx[2] = {nullptr, nullptr};
   uint32_t shift = 31;
+  // MSD bucket sort (msd_sort.cuh)
+  uint32_t* bin_hist[2] = {nullptr, nullptr};       // uint32[kBins]
+  uint32_t* bin_cursor[2] = {nullptr, nullptr};     // uint32[kBins]
+  uint32_t* bucket_start[2] = {nullptr, nullptr};   // uint32[kBins + 1]
+  uint32_t* n_buckets = nullptr;                    // uint32[2]
+  uint32_t* msd_flag = nullptr;                     // uint32[2]
   void carve(Carver& c, uint64_t n_keys, bool with_index) {
     n = (uint32_t)n_keys;
     n_tiles = rs::num_tiles(n_keys);
@@ -104,6 +115,13 @@ struct SortCtx {
       for (int a = 0; a < 2; ++a) hist[p][a] = c.take<uint32_t>(rs::kPasses * rs::kRadix);
     for (int a = 0; a < 2; ++a) status[a] = c.take<uint64_t>((uint64_t)n_tiles * rs::kRadix);
     ticket = c.take<uint32_t>(64);
+    for (int a = 0; a < 2; ++a) {
+      bin_hist[a] = c.take<uint32_t>(msd::kBins);
+      bin_cursor[a] = c.take<uint32_t>(msd::kBins);
+      bucket_start[a] = c.take<uint32_t>(msd::kBins + 4);
+    }
+    n_buckets = c.take<uint32_t>(64);
+    msd_flag = n_buckets ? n_buckets + 8 : nullptr;
     shift = index_shift_for(n_keys);
     if (with_index)
       for (int a = 0; a < 2; ++a) idx[a] = c.take<uint32_t>(index_entries(shift));
@@ -126,8 +144,16 @@ struct Layout {
   SortCtx b;              // the searched set
   SortCtx q;              // PERMUTE_B: A's ends (array 0) and starts (array 1), sorted once
   uint32_t* spans = nullptr;
+  // PERMUTE_B fused rounds (mc_fused.cuh)
+  uint32_t* slabs[2] = {nullptr, nullptr};
+  uint64_t slab_words = 0;               // capacity of each slab array
+  uint32_t* slab_cursor[2] = {nullptr, nullptr};
+  uint32_t* qb[2] = {nullptr, nullptr};
+  uint32_t* round_flags = nullptr;       // uint32[kFlagChunk]
   size_t bytes = 0;
 };
+constexpr uint32_t kFlagChunk = 4096;    // fused rounds are checked for raised flags in chunks of this many
+static inline uint64_t slab_capacity_words(uint64_t n) { return align_up(n + n / 4 + (4u << 20), 64); }
 
 static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which) {
   Layout L;
@@ -145,6 +171,13 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
       } else {
         L.spans = c.take<uint32_t>(align_up(n_b, 4) + 4);
         L.q.carve(c, n_a, false);
+        L.slab_words = slab_capacity_words(n_b);
+        for (int a = 0; a < 2; ++a) {
+          L.slabs[a] = c.take<uint32_t>(L.slab_words);
+          L.slab_cursor[a] = c.take<uint32_t>(mcf::kMaxBins);
+          L.qb[a] = c.take<uint32_t>(mcf::kMaxBins + 4);
+        }
+        L.round_flags = c.take<uint32_t>(kFlagChunk);
       }
       break;
     case BITS_FN_PLACE:
@@ -181,6 +214,7 @@ struct SortPlan {
   uint32_t* ticket;
   uint32_t n, n_tiles;
   int n_arrays;
+  const uint32_t* run_if = nullptr;   // device uint32[2]: passes run only if one of them is non-zero (null: always)
 };
 
 static int launch_sort_passes(const SortPlan& p, uint32_t* epoch, cudaStream_t st) {
@@ -195,6 +229,7 @@ static int launch_sort_passes(const SortPlan& p, uint32_t* epoch, cudaStream_t s
       a.arr[k].ticket = p.ticket + k;
     }
     a.n = p.n; a.n_tiles = p.n_tiles; a.shift = 8 * pass; a.epoch = (*epoch)++;
+    a.run_if[0] = p.run_if; a.run_if[1] = p.run_if ? p.run_if + (p.n_arrays > 1 ? 1 : 0) : nullptr;
     ProfScope prof(kClsSortPass, st);
     rs::onesweep_pass_kernel<<<dim3(p.n_tiles, p.n_arrays), rs::kThreads, 0, st>>>(a);
     BITS_LAUNCH_CHECK();
@@ -203,11 +238,12 @@ static int launch_sort_passes(const SortPlan& p, uint32_t* epoch, cudaStream_t s
 }
 
 static int launch_histogram(const uint32_t* k0, const uint32_t* k1, uint32_t* h0, uint32_t* h1, uint32_t n,
-                            int n_arrays, cudaStream_t st) {
+                            int n_arrays, cudaStream_t st, const uint32_t* run_if = nullptr) {
   rs::HistArgs h;
   h.keys[0] = k0; h.keys[1] = n_arrays > 1 ? k1 : k0;
   h.hist[0] = h0; h.hist[1] = n_arrays > 1 ? h1 : h0;
   h.n = n;
+  h.run_if[0] = run_if; h.run_if[1] = run_if ? run_if + (n_arrays > 1 ? 1 : 0) : nullptr;
   ProfScope prof(kClsHist, st);
   rs::histogram_kernel<<<dim3(grid_for(ceil_div(n, 4), 512), n_arrays), 512, 0, st>>>(h);
   BITS_LAUNCH_CHECK();
@@ -223,6 +259,9 @@ static int reset_sort_ctx(const SortCtx& c, cudaStream_t st) {
   BITS_CUDA_TRY(cudaMemsetAsync(c.status[0], 0, sizeof(uint64_t) * (uint64_t)c.n_tiles * rs::kRadix, st));
   BITS_CUDA_TRY(cudaMemsetAsync(c.status[1], 0, sizeof(uint64_t) * (uint64_t)c.n_tiles * rs::kRadix, st));
   BITS_CUDA_TRY(cudaMemsetAsync(c.ticket, 0, sizeof(uint32_t) * 64, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.bin_hist[0], 0, sizeof(uint32_t) * msd::kBins, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.bin_hist[1], 0, sizeof(uint32_t) * msd::kBins, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.n_buckets, 0, sizeof(uint32_t) * 64, st));
   return BITS_OK;
 }
 
@@ -237,6 +276,88 @@ static SortPlan plan_for(const SortCtx& c, const uint32_t* src0, const uint32_t*
   p.ticket = c.ticket;
   p.n = c.n; p.n_tiles = c.n_tiles; p.n_arrays = 2;
   return p;
+}
+
+// One-time attribute setup for the kernels that use more than 48 KB of shared memory.
+static int msd_configure() {
+  static int done = -1;
+  if (done < 0) {
+    const cudaError_t e1 = cudaFuncSetAttribute(msd::scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kScSmem);
+    const cudaError_t e2 = cudaFuncSetAttribute(msd::bucket_sort_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
+    const cudaError_t e3 = cudaFuncSetAttribute(msd::bucket_sort_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
+    const cudaError_t e4 = cudaFuncSetAttribute(mcf::place_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mcf::kPsSmem);
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { (void)cudaGetLastError(); return BITS_ERR_CUDA; }
+    done = 1;
+  }
+  return BITS_OK;
+}
+
+// Sort n_arrays (1 or 2) arrays of c.n keys: src -> ... -> y (c.buf[a][0] unless y_override).
+// MSD bucket sort (plan -> scatter -> bucket sort) with the LSD sort as device-side fallback.
+// bin_hist_ready: c.bin_hist already holds the top-bits histogram of the sources (made by the
+// placement kernel).  The stage is complete once the stream reaches the end of what is enqueued.
+static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* src1, int n_arrays, uint32_t* y_override,
+                       bool bin_hist_ready, uint32_t* epoch, cudaStream_t st) {
+  SortPlan p = plan_for(c, src0, n_arrays > 1 ? src1 : src0, 0);
+  p.n_arrays = n_arrays;
+  if (y_override) p.y[0] = y_override;
+  if (!g_opt.sort_msd) {
+    BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+    if (n_arrays > 1) BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+    BITS_TRY(launch_histogram(src0, src1, c.hist[0][0], c.hist[0][1], c.n, n_arrays, st));
+    return launch_sort_passes(p, epoch, st);
+  }
+  BITS_TRY(msd_configure());
+  if (!bin_hist_ready) {
+    msd::BinHistArgs h;
+    h.keys[0] = src0; h.keys[1] = n_arrays > 1 ? src1 : src0;
+    h.hist[0] = c.bin_hist[0]; h.hist[1] = c.bin_hist[1];
+    h.n = c.n;
+    ProfScope prof(kClsHist, st);
+    msd::bin_hist_kernel<<<dim3(grid_for(ceil_div(c.n, 4), 512), n_arrays), 512, 0, st>>>(h);
+    BITS_LAUNCH_CHECK();
+  }
+  {
+    msd::PlanArgs pa;
+    for (int a = 0; a < 2; ++a) {
+      pa.p[a].hist = c.bin_hist[a]; pa.p[a].bin_cursor = c.bin_cursor[a]; pa.p[a].bucket_start = c.bucket_start[a];
+      pa.p[a].n_buckets = c.n_buckets + a; pa.p[a].flag = c.msd_flag + a; pa.p[a].lsd_hist = c.hist[0][a];
+    }
+    ProfScope prof(kClsPlan, st);
+    msd::plan_kernel<<<n_arrays, 1024, 0, st>>>(pa);
+    BITS_LAUNCH_CHECK();
+  }
+  {
+    msd::ScatterArgs sa;
+    for (int a = 0; a < 2; ++a) {
+      const int aa = a < n_arrays ? a : 0;
+      sa.arr[a].src = p.src[aa]; sa.arr[a].dst = p.x[aa]; sa.arr[a].bin_cursor = c.bin_cursor[aa]; sa.arr[a].flag = c.msd_flag + aa;
+    }
+    sa.n = c.n; sa.n_tiles = (uint32_t)ceil_div(c.n, msd::kScTile);
+    const uint32_t per = (uint32_t)kSMs / (uint32_t)n_arrays;
+    ProfScope prof(kClsScatter, st);
+    msd::scatter_kernel<<<dim3(sa.n_tiles < per ? sa.n_tiles : per, n_arrays), msd::kScThreads, msd::kScSmem, st>>>(sa);
+    BITS_LAUNCH_CHECK();
+  }
+  {
+    msd::BucketArgs ba;
+    for (int a = 0; a < 2; ++a) {
+      const int aa = a < n_arrays ? a : 0;
+      ba.arr[a].src = p.x[aa]; ba.arr[a].dst = p.y[aa]; ba.arr[a].bucket_start = c.bucket_start[aa];
+      ba.arr[a].n_buckets = c.n_buckets + aa; ba.arr[a].flag = c.msd_flag + aa;
+    }
+    const uint32_t want = (uint32_t)ceil_div((uint64_t)c.n * 2, msd::kBucketCap) + 1;   // about the number of buckets
+    const uint32_t per = 2u * (uint32_t)kSMs / (uint32_t)n_arrays;
+    ProfScope prof(kClsBucketSort, st);
+    ba.slab = 0; ba.round_flag = nullptr; ba.round_total = nullptr;
+    for (int a = 0; a < 2; ++a) { ba.arr[a].q_sorted = nullptr; ba.arr[a].qb = nullptr; }
+    msd::bucket_sort_kernel<false, false><<<dim3(want < per ? want : per, n_arrays), msd::kBkThreads, msd::kBkSmem, st>>>(ba);
+    BITS_LAUNCH_CHECK();
+  }
+  // fallback: the stable LSD sort redoes everything if a flag was raised, else these launches exit at once
+  p.run_if = c.msd_flag;
+  BITS_TRY(launch_histogram(src0, src1, c.hist[0][0], c.hist[0][1], c.n, n_arrays, st, c.msd_flag));
+  return launch_sort_passes(p, epoch, st);
 }
 
 static int launch_build_index(const SortCtx& c, cudaStream_t st) {
@@ -258,9 +379,7 @@ static int setup_searched_set(const SortCtx& c, const uint32_t* b_start, const u
     BITS_CUDA_TRY(cudaMemcpyAsync(c.buf[0][0], b_start, sizeof(uint32_t) * (size_t)c.n, cudaMemcpyDeviceToDevice, st));
     BITS_CUDA_TRY(cudaMemcpyAsync(c.buf[1][0], b_end, sizeof(uint32_t) * (size_t)c.n, cudaMemcpyDeviceToDevice, st));
   } else {
-    BITS_TRY(launch_histogram(b_start, b_end, c.hist[0][0], c.hist[0][1], c.n, 2, st));
-    const SortPlan p = plan_for(c, b_start, b_end, 0);
-    BITS_TRY(launch_sort_passes(p, epoch, st));
+    BITS_TRY(sort_arrays(c, b_start, b_end, 2, nullptr, false, epoch, st));
   }
   return launch_build_index(c, st);
 }
@@ -350,17 +469,19 @@ static int check_genome(const uint32_t* off, uint32_t n_chrom, ChromTable* t, ui
 }
 
 static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* end_out, uint32_t n, uint32_t round,
-                        uint32_t tag, const PhiloxKeys& key, const ChromTable& chrom, bool vec, uint32_t* hist_s,
-                        uint32_t* hist_e, uint32_t* zero_s, uint32_t* zero_e, cudaStream_t st) {
+                        uint32_t tag, const PhiloxKeys& key, const ChromTable& chrom, bool vec, int hist_mode,
+                        uint32_t* hist_s, uint32_t* hist_e, uint32_t* zero_s, uint32_t* zero_e, cudaStream_t st) {
   PlaceArgs a;
   a.spans = spans; a.start_out = start_out; a.end_out = end_out; a.n = n; a.round = round; a.tag = tag;
   a.key = key; a.chrom = chrom; a.hist_start = hist_s; a.hist_end = hist_e; a.zero_a = zero_s; a.zero_b = zero_e;
   const int grid = grid_for(ceil_div(n, 4), 256);
   ProfScope prof(kClsPlace, st);
-  if (hist_s) {
-    if (vec) place_kernel<true, true><<<grid, 256, 0, st>>>(a); else place_kernel<false, true><<<grid, 256, 0, st>>>(a);
+  if (hist_mode == kHistBins) {
+    if (vec) place_kernel<true, kHistBins><<<grid, 256, 0, st>>>(a); else place_kernel<false, kHistBins><<<grid, 256, 0, st>>>(a);
+  } else if (hist_mode == kHistDigits) {
+    if (vec) place_kernel<true, kHistDigits><<<grid, 256, 0, st>>>(a); else place_kernel<false, kHistDigits><<<grid, 256, 0, st>>>(a);
   } else {
-    if (vec) place_kernel<true, false><<<grid, 256, 0, st>>>(a); else place_kernel<false, false><<<grid, 256, 0, st>>>(a);
+    if (vec) place_kernel<true, kHistNone><<<grid, 256, 0, st>>>(a); else place_kernel<false, kHistNone><<<grid, 256, 0, st>>>(a);
   }
   BITS_LAUNCH_CHECK();
   return BITS_OK;
@@ -388,16 +509,16 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
 
   // spans of the permuted set + the NO_PLACEMENT check (one synchronisation)
   const uint32_t n_p = (uint32_t)(which == BITS_PERMUTE_A ? n_a : n_b);
+  uint32_t h_max_span = 0;
   if (n_p) {
     BITS_CUDA_TRY(cudaMemsetAsync(L.small.max_span, 0, sizeof(uint32_t), st));
     spans_kernel<<<grid_for(n_p, 256), 256, 0, st>>>(which == BITS_PERMUTE_A ? a_start : b_start,
                                                      which == BITS_PERMUTE_A ? a_end : b_end, n_p, L.spans,
                                                      L.small.max_span);
     BITS_LAUNCH_CHECK();
-    uint32_t h_max = 0;
-    BITS_CUDA_TRY(cudaMemcpyAsync(&h_max, L.small.max_span, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    BITS_CUDA_TRY(cudaMemcpyAsync(&h_max_span, L.small.max_span, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
     BITS_CUDA_TRY(cudaStreamSynchronize(st));
-    if (h_max >= l_max) return BITS_ERR_NO_PLACEMENT;
+    if (h_max_span >= l_max) return BITS_ERR_NO_PLACEMENT;
   }
   if (n_a == 0 || n_b == 0) return BITS_OK;   // every count is 0 (already written)
 
@@ -429,34 +550,50 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   // PERMUTE_B: A's ends and starts sorted once; every round place -> sort x2 -> search -> reduce.
   uint32_t q_epoch = 1;
   BITS_TRY(reset_sort_ctx(L.q, st));
-  BITS_TRY(launch_histogram(a_end, a_start, L.q.hist[0][0], L.q.hist[0][1], L.q.n, 2, st));
-  BITS_TRY(launch_sort_passes(plan_for(L.q, a_end, a_start, 0), &q_epoch, st));
+  BITS_TRY(sort_arrays(L.q, a_end, a_start, 2, nullptr, false, &q_epoch, st));
   const uint32_t* q_end_sorted = L.q.buf[0][0];
   const uint32_t* q_start_sorted = L.q.buf[1][0];
-  // the observed-count sort used histogram parity 0; clear it so round 0 can accumulate into it
-  BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[0][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[0][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-  const bool fused = g_opt.place_fused_hist != 0;
-  for (uint32_t k = 0; k < n_rounds; ++k) {
-    const int par = (int)(k & 1);
-    // epochs (30 bits) and ticket counters (32 bits, taken modulo n_tiles) must not wrap
-    if (epoch > (1u << 30) - 8u || (uint64_t)epoch * L.b.n_tiles > (1ull << 32) - 8ull * L.b.n_tiles) {
+  const bool msd_on = g_opt.sort_msd != 0;
+  const bool hist_in_place = g_opt.place_fused_hist != 0;
+  // histograms the placement kernel accumulates into: the MSD sort's bins (left zero by plan_kernel)
+  // or, with the LSD sort only, the four digit histograms (parity double-buffered, cleared by the
+  // placement kernel of the previous round)
+  if (!msd_on) {
+    BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[0][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+    BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[0][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+    BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[1][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+    BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[1][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+  }
+  uint32_t n_general = 0;   // rounds done by the general path so far (parity of the LSD histograms)
+  // One round by the general path: place -> sort both arrays -> search with the sorted queries.
+  auto general_round = [&](uint32_t k) -> int {
+    const int par = (int)(n_general++ & 1);
+    // epochs (30 bits) must not wrap
+    if (epoch > (1u << 30) - 16u) {
       BITS_CUDA_TRY(cudaMemsetAsync(L.b.status[0], 0, sizeof(uint64_t) * (uint64_t)L.b.n_tiles * rs::kRadix, st));
       BITS_CUDA_TRY(cudaMemsetAsync(L.b.status[1], 0, sizeof(uint64_t) * (uint64_t)L.b.n_tiles * rs::kRadix, st));
-      BITS_CUDA_TRY(cudaMemsetAsync(L.b.ticket, 0, sizeof(uint32_t) * 64, st));
       epoch = 1;
     }
-    if (fused) {
+    // placed keys go to the "result" buffers; the sort reads them, works through the temp buffers
+    // and lands back in the result buffers
+    if (msd_on) {
       BITS_TRY(launch_place(L.spans, L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, round_begin + k, 1u, key, chrom, true,
-                            L.b.hist[par][0], L.b.hist[par][1], L.b.hist[par ^ 1][0], L.b.hist[par ^ 1][1], st));
+                            hist_in_place ? kHistBins : kHistNone, hist_in_place ? L.b.bin_hist[0] : nullptr,
+                            hist_in_place ? L.b.bin_hist[1] : nullptr, nullptr, nullptr, st));
+      BITS_TRY(sort_arrays(L.b, L.b.buf[0][0], L.b.buf[1][0], 2, nullptr, hist_in_place, &epoch, st));
     } else {
-      BITS_TRY(launch_place(L.spans, L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, round_begin + k, 1u, key, chrom, true,
-                            nullptr, nullptr, nullptr, nullptr, st));
-      BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[par][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-      BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[par][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-      BITS_TRY(launch_histogram(L.b.buf[0][0], L.b.buf[1][0], L.b.hist[par][0], L.b.hist[par][1], (uint32_t)n_b, 2, st));
+      if (hist_in_place) {
+        BITS_TRY(launch_place(L.spans, L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, round_begin + k, 1u, key, chrom, true,
+                              kHistDigits, L.b.hist[par][0], L.b.hist[par][1], L.b.hist[par ^ 1][0], L.b.hist[par ^ 1][1], st));
+      } else {
+        BITS_TRY(launch_place(L.spans, L.b.buf[0][0], L.b.buf[1][0], (uint32_t)n_b, round_begin + k, 1u, key, chrom, true,
+                              kHistNone, nullptr, nullptr, nullptr, nullptr, st));
+        BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[par][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+        BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[par][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+        BITS_TRY(launch_histogram(L.b.buf[0][0], L.b.buf[1][0], L.b.hist[par][0], L.b.hist[par][1], (uint32_t)n_b, 2, st));
+      }
+      BITS_TRY(launch_sort_passes(plan_for(L.b, L.b.buf[0][0], L.b.buf[1][0], par), &epoch, st));
     }
-    BITS_TRY(launch_sort_passes(plan_for(L.b, L.b.buf[0][0], L.b.buf[1][0], par), &epoch, st));
     unsigned long long* out = reinterpret_cast<unsigned long long*>(round_counts_out + k);
     if (g_opt.mc_sorted_queries) {
       ProfScope prof(kClsSortedQuery, st);
@@ -467,6 +604,104 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       BITS_TRY(launch_build_index(L.b, st));
       BITS_TRY(launch_count(a_start, a_end, (uint32_t)n_a, L.b, nullptr, reinterpret_cast<uint64_t*>(out), st));
     }
+    return BITS_OK;
+  };
+
+  // Fused rounds: possible when fixed bins (key >> shift) can hold the re-placed keys in slabs of at
+  // most kBucketCap keys with a wide margin.  Expected keys per bin <= n_b * 2^shift / V(d_max),
+  // V(d) = number of valid starts for span d.
+  mcf::PlaceScatterArgs ps;
+  bool fused_ok = msd_on && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0;
+  if (fused_ok) {
+    uint64_t v_min = 0;
+    for (uint32_t c = 0; c < n_chrom; ++c) { const uint32_t Lc = off[c + 1] - off[c]; v_min += Lc > h_max_span ? Lc - h_max_span : 0; }
+    const uint64_t G = off[n_chrom];
+    int best = -1; uint32_t best_slab = 0;
+    for (int sh = 31; sh >= 0 && v_min > 0; --sh) {
+      const uint64_t nbins = (G + (1ull << sh) - 1) >> sh;
+      if (nbins > (uint64_t)mcf::kMaxBins) break;
+      const double avg = (double)n_b * (double)(1ull << sh) / (double)v_min;
+      const double need = avg * 1.125 + 8.0 * sqrt(avg) + 32.0;
+      if (need > (double)msd::kBucketCap) continue;
+      const uint32_t slab = (uint32_t)align_up((uint64_t)need + 1, 4);
+      if (nbins * slab > L.slab_words) continue;
+      best = sh; best_slab = slab;
+      break;
+    }
+    fused_ok = best >= 0;
+    if (fused_ok) {
+      ps.spans = L.spans; ps.n = (uint32_t)n_b; ps.tag = 1u; ps.key = key; ps.chrom = chrom;
+      ps.shift = (uint32_t)best; ps.n_bins = (uint32_t)((G + (1ull << best) - 1) >> best); ps.slab = best_slab;
+      // balanced tiles: every block gets the same number of equally sized tiles
+      const uint32_t blocks = 2u * (uint32_t)kSMs;
+      const uint32_t tiles_per_block = (uint32_t)ceil_div(n_b, (uint64_t)blocks * mcf::kPsTile);
+      uint32_t tile = (uint32_t)align_up(ceil_div(n_b, (uint64_t)blocks * tiles_per_block), 4);
+      if (tile > (uint32_t)mcf::kPsTile) tile = mcf::kPsTile;
+      ps.tile = tile; ps.n_tiles = (uint32_t)ceil_div(n_b, tile);
+      for (int a = 0; a < 2; ++a) { ps.slab_keys[a] = L.slabs[a]; ps.cursor[a] = L.slab_cursor[a]; }
+    }
+  }
+  if (!fused_ok) {
+    for (uint32_t k = 0; k < n_rounds; ++k) BITS_TRY(general_round(k));
+    return BITS_OK;
+  }
+  BITS_TRY(msd_configure());
+  BITS_CUDA_TRY(cudaMemsetAsync(L.slab_cursor[0], 0, sizeof(uint32_t) * mcf::kMaxBins, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(L.slab_cursor[1], 0, sizeof(uint32_t) * mcf::kMaxBins, st));
+  {
+    mcf::QueryBinsArgs qa;
+    qa.q_sorted[0] = q_end_sorted; qa.q_sorted[1] = q_start_sorted; qa.qb[0] = L.qb[0]; qa.qb[1] = L.qb[1];
+    qa.n_q = (uint32_t)n_a; qa.n_bins = ps.n_bins; qa.shift = ps.shift;
+    mcf::query_bins_kernel<<<dim3((unsigned)ceil_div(ps.n_bins + 1, 256), 2), 256, 0, st>>>(qa);
+    BITS_LAUNCH_CHECK();
+  }
+  std::vector<uint32_t> h_flags;
+  for (uint32_t done = 0; done < n_rounds;) {
+    const uint32_t chunk = n_rounds - done < kFlagChunk ? n_rounds - done : kFlagChunk;
+    BITS_CUDA_TRY(cudaMemsetAsync(L.round_flags, 0, sizeof(uint32_t) * chunk, st));
+    for (uint32_t j = 0; j < chunk; ++j) {
+      const uint32_t k = done + j;
+      unsigned long long* out = reinterpret_cast<unsigned long long*>(round_counts_out + k);
+      ps.round = round_begin + k; ps.flag = L.round_flags + j;
+      {
+        ProfScope prof(kClsPlaceScatter, st);
+        const uint32_t blocks = 2u * (uint32_t)kSMs;
+        mcf::place_scatter_kernel<<<ps.n_tiles < blocks ? ps.n_tiles : blocks, mcf::kPsThreads, mcf::kPsSmem, st>>>(ps);
+        BITS_LAUNCH_CHECK();
+      }
+      {
+        mcf::SlabPlanArgs sp;
+        for (int a = 0; a < 2; ++a) { sp.cursor[a] = L.slab_cursor[a]; sp.bucket_start[a] = L.b.bucket_start[a]; sp.qb[a] = L.qb[a]; }
+        sp.n_buckets = L.b.n_buckets; sp.n_bins = ps.n_bins; sp.slab = ps.slab; sp.n_keys = (uint32_t)n_b;
+        sp.flag = ps.flag; sp.msd_flag = L.b.msd_flag; sp.n_q = (uint32_t)n_a; sp.round_total = out;
+        ProfScope prof(kClsPlan, st);
+        mcf::slab_plan_kernel<<<2, 1024, 0, st>>>(sp);
+        BITS_LAUNCH_CHECK();
+      }
+      {
+        msd::BucketArgs ba;
+        for (int a = 0; a < 2; ++a) {
+          ba.arr[a].src = L.slabs[a]; ba.arr[a].dst = L.b.buf[a][0]; ba.arr[a].bucket_start = L.b.bucket_start[a];
+          ba.arr[a].n_buckets = L.b.n_buckets + a; ba.arr[a].flag = L.b.msd_flag + a;
+          ba.arr[a].q_sorted = a ? q_start_sorted : q_end_sorted; ba.arr[a].qb = L.qb[a];
+        }
+        ba.slab = ps.slab; ba.round_flag = ps.flag; ba.round_total = out;
+        const uint32_t per = (uint32_t)kSMs;
+        ProfScope prof(kClsBucketSortSearch, st);
+        msd::bucket_sort_kernel<true, true><<<dim3(ps.n_bins < per ? ps.n_bins : per, 2), msd::kBkThreads, msd::kBkSmem, st>>>(ba);
+        BITS_LAUNCH_CHECK();
+      }
+    }
+    // rounds whose flag was raised are redone by the general path (one synchronisation per chunk)
+    h_flags.assign(chunk, 0);
+    BITS_CUDA_TRY(cudaMemcpyAsync(h_flags.data(), L.round_flags, sizeof(uint32_t) * chunk, cudaMemcpyDeviceToHost, st));
+    BITS_CUDA_TRY(cudaStreamSynchronize(st));
+    for (uint32_t j = 0; j < chunk; ++j) {
+      if (!h_flags[j]) continue;
+      BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out + done + j, 0, sizeof(uint64_t), st));
+      BITS_TRY(general_round(done + j));
+    }
+    done += chunk;
   }
   return BITS_OK;
 }
@@ -561,8 +796,8 @@ int bits_place(const uint32_t* spans, uint64_t n, const uint32_t* chrom_offsets,
   BITS_CUDA_TRY(cudaMemcpyAsync(L.small.chrom, chrom_offsets, sizeof(uint32_t) * ((size_t)n_chrom + 1),
                                 cudaMemcpyHostToDevice, st));
   const bool vec = (n & 3) == 0 && (((uintptr_t)spans | (uintptr_t)start_out | (uintptr_t)end_out) & 15) == 0;
-  return launch_place(spans, start_out, end_out, (uint32_t)n, round, tag, make_philox_keys(seed), chrom, vec, nullptr,
-                      nullptr, nullptr, nullptr, st);
+  return launch_place(spans, start_out, end_out, (uint32_t)n, round, tag, make_philox_keys(seed), chrom, vec, kHistNone,
+                      nullptr, nullptr, nullptr, nullptr, st);
 }
 
 int bits_sort_u32(const uint32_t* keys_in, uint32_t* keys_out, uint64_t n, void* workspace, size_t workspace_bytes,
@@ -574,12 +809,8 @@ int bits_sort_u32(const uint32_t* keys_in, uint32_t* keys_out, uint64_t n, void*
   if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
   if (n == 0) return BITS_OK;
   BITS_TRY(reset_sort_ctx(L.b, st));
-  BITS_TRY(launch_histogram(keys_in, nullptr, L.b.hist[0][0], nullptr, (uint32_t)n, 1, st));
-  SortPlan p = plan_for(L.b, keys_in, keys_in, 0);
-  p.y[0] = keys_out;
-  p.n_arrays = 1;
   uint32_t epoch = 1;
-  return launch_sort_passes(p, &epoch, st);
+  return sort_arrays(L.b, keys_in, keys_in, 1, keys_out, false, &epoch, st);
 }
 
 int bits_count_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
@@ -661,6 +892,8 @@ int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
 
 int bits_set_option(const char* name, int64_t value) {
   if (!name) return BITS_ERR_NULL;
+  if (!strcmp(name, "mc_fused")) { g_opt.mc_fused = value; return BITS_OK; }
+  if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }
   if (!strcmp(name, "place_fused_hist")) { g_opt.place_fused_hist = value; return BITS_OK; }
   if (!strcmp(name, "profile")) {   // 0 = off, 1 = on, 2 = reset the accumulated times

@@ -5,6 +5,7 @@
 #pragma once
 #include "philox_place.cuh"
 #include "radix_sort.cuh"
+#include "msd_sort.cuh"
 
 namespace bits {
 
@@ -41,22 +42,28 @@ struct PlaceArgs {
   uint32_t tag;
   PhiloxKeys key;
   ChromTable chrom;
-  uint32_t* hist_start;    // kHist: uint32[4][256] global histograms to add into
+  uint32_t* hist_start;    // kHistDigits: uint32[4][256], kHistBins: uint32[msd::kBins] -- global histograms to add into
   uint32_t* hist_end;
-  uint32_t* zero_a;        // kHist: 2 x uint32[4][256] to clear for the NEXT round (block 0), or null
+  uint32_t* zero_a;        // kHistDigits: 2 x uint32[4][256] to clear for the NEXT round (block 0), or null
   uint32_t* zero_b;
 };
 
+// which histogram of the freshly made keys the placement kernel accumulates
+enum { kHistNone = 0, kHistDigits = 1, kHistBins = 2 };
+
 // Four intervals per thread.  kVec: all three arrays 16-byte aligned and padded to a multiple
 // of four elements (the library's own workspace buffers); otherwise scalar accesses.
-template <bool kVec, bool kHist>
+// kHist: kHistDigits = the LSD sort's four 8-bit digit histograms, kHistBins = the MSD sort's
+// histogram of the top msd::kBinBits bits (one shared-memory atomic per key).
+template <bool kVec, int kHist>
 __global__ void __launch_bounds__(256) place_kernel(PlaceArgs a) {
+  constexpr int kHalf = kHist == kHistDigits ? rs::kPasses * rs::kRadix : (kHist == kHistBins ? msd::kBins : 1);
   __shared__ uint32_t s_off[kMaxChromSmem];
-  __shared__ uint32_t s_h[kHist ? 2 * rs::kPasses * rs::kRadix : 1];
-  if (kHist) {
-    for (int i = threadIdx.x; i < 2 * rs::kPasses * rs::kRadix; i += blockDim.x) s_h[i] = 0;
-    if (blockIdx.x == 0 && a.zero_a)
-      for (int i = threadIdx.x; i < rs::kPasses * rs::kRadix; i += blockDim.x) { a.zero_a[i] = 0; a.zero_b[i] = 0; }
+  __shared__ uint32_t s_h[kHist != kHistNone ? 2 * kHalf : 1];
+  if (kHist != kHistNone) {
+    for (int i = threadIdx.x; i < 2 * kHalf; i += blockDim.x) s_h[i] = 0;
+    if (kHist == kHistDigits && blockIdx.x == 0 && a.zero_a)
+      for (int i = threadIdx.x; i < kHalf; i += blockDim.x) { a.zero_a[i] = 0; a.zero_b[i] = 0; }
   }
   const uint32_t* off = stage_chrom_table(a.chrom, s_off);   // barrier inside
   const uint32_t n = a.n;
@@ -83,24 +90,29 @@ __global__ void __launch_bounds__(256) place_kernel(PlaceArgs a) {
       for (int j = 0; j < 4; ++j)
         if (i0 + j < n) { a.start_out[i0 + j] = st[j]; a.end_out[i0 + j] = en[j]; }
     }
-    if (kHist) {
+    if (kHist != kHistNone) {
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         if (i0 + j < n) {
+          if (kHist == kHistDigits) {
 #pragma unroll
-          for (int p = 0; p < rs::kPasses; ++p) {
-            atomicAdd(&s_h[p * rs::kRadix + ((st[j] >> (8 * p)) & 255u)], 1u);
-            atomicAdd(&s_h[(rs::kPasses + p) * rs::kRadix + ((en[j] >> (8 * p)) & 255u)], 1u);
+            for (int p = 0; p < rs::kPasses; ++p) {
+              atomicAdd(&s_h[p * rs::kRadix + ((st[j] >> (8 * p)) & 255u)], 1u);
+              atomicAdd(&s_h[kHalf + p * rs::kRadix + ((en[j] >> (8 * p)) & 255u)], 1u);
+            }
+          } else {
+            atomicAdd(&s_h[st[j] >> msd::kBinShift], 1u);
+            atomicAdd(&s_h[kHalf + (en[j] >> msd::kBinShift)], 1u);
           }
         }
       }
     }
   }
-  if (kHist) {
+  if (kHist != kHistNone) {
     __syncthreads();
-    for (int i = threadIdx.x; i < rs::kPasses * rs::kRadix; i += blockDim.x) {
+    for (int i = threadIdx.x; i < kHalf; i += blockDim.x) {
       if (s_h[i]) atomicAdd(&a.hist_start[i], s_h[i]);
-      if (s_h[rs::kPasses * rs::kRadix + i]) atomicAdd(&a.hist_end[i], s_h[rs::kPasses * rs::kRadix + i]);
+      if (s_h[kHalf + i]) atomicAdd(&a.hist_end[i], s_h[kHalf + i]);
     }
   }
 }

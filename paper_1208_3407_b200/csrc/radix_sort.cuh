@@ -41,7 +41,14 @@ struct SortPassArgs {
   uint32_t n_tiles;
   uint32_t shift;
   uint32_t epoch;         // 1 .. 2^30-1, unique per pass since the status array was cleared
+  const uint32_t* run_if[2];   // both null: always run; else run only if *run_if[0] | *run_if[1] (fallback of msd_sort.cuh)
 };
+
+
+
+__device__ __forceinline__ bool skip_launch(const uint32_t* const run_if[2]) {
+  return run_if[0] != nullptr && ((*run_if[0]) | (*run_if[1])) == 0u;
+}
 
 inline uint32_t num_tiles(uint64_t n) { return (uint32_t)ceil_div(n, kTile); }
 
@@ -80,10 +87,12 @@ struct HistArgs {
   const uint32_t* keys[2];
   uint32_t* hist[2];
   uint32_t n;
+  const uint32_t* run_if[2];
 };
 
 __global__ void __launch_bounds__(512) histogram_kernel(HistArgs a) {
   __shared__ uint32_t s_h[kPasses * kRadix];
+  if (skip_launch(a.run_if)) return;
   for (int i = threadIdx.x; i < kPasses * kRadix; i += blockDim.x) s_h[i] = 0;
   __syncthreads();
   const uint32_t* __restrict__ keys = blockIdx.y ? a.keys[1] : a.keys[0];
@@ -129,6 +138,7 @@ __global__ void __launch_bounds__(kThreads, 2) onesweep_pass_kernel(SortPassArgs
   __shared__ uint32_t s_wsum[8];
   __shared__ uint32_t s_tile;
 
+  if (skip_launch(a.run_if)) return;
   const SortArray A = blockIdx.y ? a.arr[1] : a.arr[0];   // (no dynamic indexing of the parameter block)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid == 0) s_tile = atomicAdd(A.ticket, 1u) % a.n_tiles;
