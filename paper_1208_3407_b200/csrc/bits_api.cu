@@ -11,7 +11,7 @@
 #include "place_kernels.cuh"
 #include "radix_sort.cuh"
 #include "msd_sort.cuh"
-#include "mc_fused.cuh"
+#include "mc_tile.cuh"
 #include "search.cuh"
 
 namespace bits {
@@ -20,7 +20,7 @@ unsigned long long g_launches = 0;
 
 struct Options {
   int64_t sort_msd = 1;            // 1 = MSD bucket sort with the LSD sort as device-side fallback, 0 = LSD sort only
-  int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+scatter / slab plan / bucket sort+search (mc_fused.cuh)
+  int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+tile sort / bin sort+search (mc_tile.cuh)
   int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
   int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
@@ -131,10 +131,12 @@ struct SortCtx {
 struct Small {            // small device scalars
   uint32_t* max_span;     // [1]
   uint32_t* bad;          // [1]
+  unsigned long long* span_sum;   // [1]
   uint32_t* chrom;        // [n_chrom + 1]
   void carve(Carver& c, uint32_t n_chrom) {
     max_span = c.take<uint32_t>(64);
     bad = max_span ? max_span + 1 : nullptr;
+    span_sum = max_span ? reinterpret_cast<unsigned long long*>(max_span + 2) : nullptr;
     chrom = c.take<uint32_t>((uint64_t)n_chrom + 1);
   }
 };
@@ -144,16 +146,27 @@ struct Layout {
   SortCtx b;              // the searched set
   SortCtx q;              // PERMUTE_B: A's ends (array 0) and starts (array 1), sorted once
   uint32_t* spans = nullptr;
-  // PERMUTE_B fused rounds (mc_fused.cuh)
-  uint32_t* slabs[2] = {nullptr, nullptr};
-  uint64_t slab_words = 0;               // capacity of each slab array
-  uint32_t* slab_cursor[2] = {nullptr, nullptr};
+  // PERMUTE_B fused rounds (mc_tile.cuh); null when the set is too large for that path
+  uint2* pairs = nullptr;                // [n_b] tile-sorted (start, end) pairs
+  uint16_t* tile_off = nullptr;          // [(kMaxBins + 1) * tile_stride] transposed per-tile bin prefixes
+  uint32_t tile_stride = 0;
+  uint32_t* cross_cnt[2] = {nullptr, nullptr};   // [kMaxBins + 1] by round parity
+  uint32_t* cross_keys = nullptr;        // [kMaxBins * kCrossCap]
   uint32_t* qb[2] = {nullptr, nullptr};
   uint32_t* round_flags = nullptr;       // uint32[kFlagChunk]
   size_t bytes = 0;
 };
 constexpr uint32_t kFlagChunk = 4096;    // fused rounds are checked for raised flags in chunks of this many
-static inline uint64_t slab_capacity_words(uint64_t n) { return align_up(n + n / 4 + (4u << 20), 64); }
+constexpr uint64_t kFusedMaxKeys = 24u << 20;   // beyond this the bins of the fused path cannot hold the set
+constexpr uint32_t kTileBlocks = 2u * 148u;     // place_tile_kernel: two resident blocks per SM
+// Tiles are balanced: every block gets the same number of equally sized tiles.
+static inline uint32_t tile_size_for(uint64_t n) {
+  const uint64_t per_block = ceil_div(n, (uint64_t)kTileBlocks * mct::kTile);
+  uint64_t tile = align_up(ceil_div(n, (uint64_t)kTileBlocks * (per_block ? per_block : 1)), 4);
+  if (tile > (uint64_t)mct::kTile) tile = mct::kTile;
+  if (tile < 4) tile = 4;
+  return (uint32_t)tile;
+}
 
 static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which) {
   Layout L;
@@ -171,13 +184,18 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
       } else {
         L.spans = c.take<uint32_t>(align_up(n_b, 4) + 4);
         L.q.carve(c, n_a, false);
-        L.slab_words = slab_capacity_words(n_b);
-        for (int a = 0; a < 2; ++a) {
-          L.slabs[a] = c.take<uint32_t>(L.slab_words);
-          L.slab_cursor[a] = c.take<uint32_t>(mcf::kMaxBins);
-          L.qb[a] = c.take<uint32_t>(mcf::kMaxBins + 4);
+        if (n_b <= kFusedMaxKeys) {
+          const uint32_t n_tiles = (uint32_t)ceil_div(n_b, tile_size_for(n_b));
+          L.tile_stride = (uint32_t)align_up((uint64_t)n_tiles + 1, 8);
+          L.pairs = c.take<uint2>(align_up(n_b, 4) + 4);
+          L.tile_off = c.take<uint16_t>((uint64_t)(mct::kMaxBins + 1) * L.tile_stride);
+          for (int a = 0; a < 2; ++a) {
+            L.cross_cnt[a] = c.take<uint32_t>(mct::kMaxBins + 4);
+            L.qb[a] = c.take<uint32_t>(mct::kMaxBins + 4);
+          }
+          L.cross_keys = c.take<uint32_t>((uint64_t)mct::kMaxBins * mct::kCrossCap);
+          L.round_flags = c.take<uint32_t>(kFlagChunk);
         }
-        L.round_flags = c.take<uint32_t>(kFlagChunk);
       }
       break;
     case BITS_FN_PLACE:
@@ -284,8 +302,8 @@ static int msd_configure() {
   if (done < 0) {
     const cudaError_t e1 = cudaFuncSetAttribute(msd::scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kScSmem);
     const cudaError_t e2 = cudaFuncSetAttribute(msd::bucket_sort_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
-    const cudaError_t e3 = cudaFuncSetAttribute(msd::bucket_sort_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
-    const cudaError_t e4 = cudaFuncSetAttribute(mcf::place_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mcf::kPsSmem);
+    const cudaError_t e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::kBsSmem);
+    const cudaError_t e4 = cudaFuncSetAttribute(mct::place_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::kPtSmem);
     if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { (void)cudaGetLastError(); return BITS_ERR_CUDA; }
     done = 1;
   }
@@ -510,14 +528,18 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   // spans of the permuted set + the NO_PLACEMENT check (one synchronisation)
   const uint32_t n_p = (uint32_t)(which == BITS_PERMUTE_A ? n_a : n_b);
   uint32_t h_max_span = 0;
+  double h_mean_span = 0.0;
   if (n_p) {
-    BITS_CUDA_TRY(cudaMemsetAsync(L.small.max_span, 0, sizeof(uint32_t), st));
+    BITS_CUDA_TRY(cudaMemsetAsync(L.small.max_span, 0, 4 * sizeof(uint32_t), st));
     spans_kernel<<<grid_for(n_p, 256), 256, 0, st>>>(which == BITS_PERMUTE_A ? a_start : b_start,
                                                      which == BITS_PERMUTE_A ? a_end : b_end, n_p, L.spans,
-                                                     L.small.max_span);
+                                                     L.small.max_span, L.small.span_sum);
     BITS_LAUNCH_CHECK();
-    BITS_CUDA_TRY(cudaMemcpyAsync(&h_max_span, L.small.max_span, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    uint32_t h_small[4] = {0, 0, 0, 0};
+    BITS_CUDA_TRY(cudaMemcpyAsync(h_small, L.small.max_span, sizeof(h_small), cudaMemcpyDeviceToHost, st));
     BITS_CUDA_TRY(cudaStreamSynchronize(st));
+    h_max_span = h_small[0];
+    h_mean_span = (double)(((uint64_t)h_small[3] << 32) | h_small[2]) / (double)n_p;
     if (h_max_span >= l_max) return BITS_ERR_NO_PLACEMENT;
   }
   if (n_a == 0 || n_b == 0) return BITS_OK;   // every count is 0 (already written)
@@ -607,38 +629,41 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     return BITS_OK;
   };
 
-  // Fused rounds: possible when fixed bins (key >> shift) can hold the re-placed keys in slabs of at
-  // most kBucketCap keys with a wide margin.  Expected keys per bin <= n_b * 2^shift / V(d_max),
-  // V(d) = number of valid starts for span d.
-  mcf::PlaceScatterArgs ps;
-  bool fused_ok = msd_on && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0;
+  // Fused rounds (mc_tile.cuh): possible when fixed bins (key >> shift) hold the re-placed keys with a
+  // wide margin (expected keys per bin <= n_b * 2^shift / V(d_max), V(d) = number of valid starts for
+  // span d), every span is shorter than a bin, and few ends fall into the bin after their start's.
+  mct::PlaceTileArgs pt;
+  mct::BinSortArgs bs;
+  bool fused_ok = msd_on && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0 && L.pairs != nullptr;
   if (fused_ok) {
     uint64_t v_min = 0;
     for (uint32_t c = 0; c < n_chrom; ++c) { const uint32_t Lc = off[c + 1] - off[c]; v_min += Lc > h_max_span ? Lc - h_max_span : 0; }
     const uint64_t G = off[n_chrom];
-    int best = -1; uint32_t best_slab = 0;
-    for (int sh = 31; sh >= 0 && v_min > 0; --sh) {
+    int best = -1;
+    for (int sh = 31; sh >= 1 && v_min > 0; --sh) {
       const uint64_t nbins = (G + (1ull << sh) - 1) >> sh;
-      if (nbins > (uint64_t)mcf::kMaxBins) break;
+      if (nbins >= (uint64_t)mct::kMaxBins) break;
+      if ((uint64_t)h_max_span >= (1ull << sh)) break;     // an end may lie at most one bin after its start
       const double avg = (double)n_b * (double)(1ull << sh) / (double)v_min;
       const double need = avg * 1.125 + 8.0 * sqrt(avg) + 32.0;
-      if (need > (double)msd::kBucketCap) continue;
-      const uint32_t slab = (uint32_t)align_up((uint64_t)need + 1, 4);
-      if (nbins * slab > L.slab_words) continue;
-      best = sh; best_slab = slab;
+      if (need > (double)mct::kCap) continue;
+      // ends handed over per bin: about avg * mean span / bin width
+      const double cross = avg * h_mean_span / (double)(1ull << sh);
+      if (cross * 2.0 + 8.0 * sqrt(cross) + 32.0 > (double)mct::kCrossCap) continue;
+      best = sh;
       break;
     }
     fused_ok = best >= 0;
     if (fused_ok) {
-      ps.spans = L.spans; ps.n = (uint32_t)n_b; ps.tag = 1u; ps.key = key; ps.chrom = chrom;
-      ps.shift = (uint32_t)best; ps.n_bins = (uint32_t)((G + (1ull << best) - 1) >> best); ps.slab = best_slab;
-      // balanced tiles: every block gets the same number of equally sized tiles
-      const uint32_t blocks = 2u * (uint32_t)kSMs;
-      const uint32_t tiles_per_block = (uint32_t)ceil_div(n_b, (uint64_t)blocks * mcf::kPsTile);
-      uint32_t tile = (uint32_t)align_up(ceil_div(n_b, (uint64_t)blocks * tiles_per_block), 4);
-      if (tile > (uint32_t)mcf::kPsTile) tile = mcf::kPsTile;
-      ps.tile = tile; ps.n_tiles = (uint32_t)ceil_div(n_b, tile);
-      for (int a = 0; a < 2; ++a) { ps.slab_keys[a] = L.slabs[a]; ps.cursor[a] = L.slab_cursor[a]; }
+      pt.spans = L.spans; pt.n = (uint32_t)n_b; pt.tag = 1u; pt.key = key; pt.chrom = chrom;
+      pt.shift = (uint32_t)best; pt.n_bins = (uint32_t)((G + (1ull << best) - 1) >> best);
+      pt.tile = tile_size_for(n_b); pt.n_tiles = (uint32_t)ceil_div(n_b, pt.tile);
+      pt.pairs = L.pairs; pt.off = L.tile_off; pt.stride = L.tile_stride; pt.cross_keys = L.cross_keys;
+      bs.pairs = L.pairs; bs.off = L.tile_off; bs.stride = L.tile_stride; bs.n_tiles = pt.n_tiles; bs.tile = pt.tile;
+      bs.n = (uint32_t)n_b; bs.shift = pt.shift; bs.n_bins = pt.n_bins; bs.cross_keys = L.cross_keys;
+      bs.dst[0] = L.b.buf[0][0]; bs.dst[1] = L.b.buf[1][0];
+      bs.q_sorted[0] = q_end_sorted; bs.q_sorted[1] = q_start_sorted; bs.qb[0] = L.qb[0]; bs.qb[1] = L.qb[1];
+      bs.n_q = (uint32_t)n_a;
     }
   }
   if (!fused_ok) {
@@ -646,49 +671,35 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     return BITS_OK;
   }
   BITS_TRY(msd_configure());
-  BITS_CUDA_TRY(cudaMemsetAsync(L.slab_cursor[0], 0, sizeof(uint32_t) * mcf::kMaxBins, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(L.slab_cursor[1], 0, sizeof(uint32_t) * mcf::kMaxBins, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(L.cross_cnt[0], 0, sizeof(uint32_t) * (mct::kMaxBins + 4), st));
+  BITS_CUDA_TRY(cudaMemsetAsync(L.cross_cnt[1], 0, sizeof(uint32_t) * (mct::kMaxBins + 4), st));
   {
-    mcf::QueryBinsArgs qa;
+    mct::QueryBinsArgs qa;
     qa.q_sorted[0] = q_end_sorted; qa.q_sorted[1] = q_start_sorted; qa.qb[0] = L.qb[0]; qa.qb[1] = L.qb[1];
-    qa.n_q = (uint32_t)n_a; qa.n_bins = ps.n_bins; qa.shift = ps.shift;
-    mcf::query_bins_kernel<<<dim3((unsigned)ceil_div(ps.n_bins + 1, 256), 2), 256, 0, st>>>(qa);
+    qa.n_q = (uint32_t)n_a; qa.n_bins = pt.n_bins; qa.shift = pt.shift;
+    mct::query_bins_kernel<<<dim3((unsigned)ceil_div(pt.n_bins + 1, 256), 2), 256, 0, st>>>(qa);
     BITS_LAUNCH_CHECK();
   }
   std::vector<uint32_t> h_flags;
+  uint32_t n_fused = 0;     // fused rounds launched so far (parity of the hand-over counters)
   for (uint32_t done = 0; done < n_rounds;) {
     const uint32_t chunk = n_rounds - done < kFlagChunk ? n_rounds - done : kFlagChunk;
     BITS_CUDA_TRY(cudaMemsetAsync(L.round_flags, 0, sizeof(uint32_t) * chunk, st));
-    for (uint32_t j = 0; j < chunk; ++j) {
+    for (uint32_t j = 0; j < chunk; ++j, ++n_fused) {
       const uint32_t k = done + j;
-      unsigned long long* out = reinterpret_cast<unsigned long long*>(round_counts_out + k);
-      ps.round = round_begin + k; ps.flag = L.round_flags + j;
+      const int par = (int)(n_fused & 1u);
+      pt.round = round_begin + k; pt.flag = L.round_flags + j; pt.cross_cnt = L.cross_cnt[par];
       {
         ProfScope prof(kClsPlaceScatter, st);
+        mct::place_tile_kernel<<<pt.n_tiles < kTileBlocks ? pt.n_tiles : kTileBlocks, mct::kPtThreads, mct::kPtSmem, st>>>(pt);
+        BITS_LAUNCH_CHECK();
+      }
+      bs.cross_cnt = L.cross_cnt[par]; bs.cross_cnt_next = L.cross_cnt[par ^ 1]; bs.flag = pt.flag;
+      bs.round_total = reinterpret_cast<unsigned long long*>(round_counts_out + k);
+      {
         const uint32_t blocks = 2u * (uint32_t)kSMs;
-        mcf::place_scatter_kernel<<<ps.n_tiles < blocks ? ps.n_tiles : blocks, mcf::kPsThreads, mcf::kPsSmem, st>>>(ps);
-        BITS_LAUNCH_CHECK();
-      }
-      {
-        mcf::SlabPlanArgs sp;
-        for (int a = 0; a < 2; ++a) { sp.cursor[a] = L.slab_cursor[a]; sp.bucket_start[a] = L.b.bucket_start[a]; sp.qb[a] = L.qb[a]; }
-        sp.n_buckets = L.b.n_buckets; sp.n_bins = ps.n_bins; sp.slab = ps.slab; sp.n_keys = (uint32_t)n_b;
-        sp.flag = ps.flag; sp.msd_flag = L.b.msd_flag; sp.n_q = (uint32_t)n_a; sp.round_total = out;
-        ProfScope prof(kClsPlan, st);
-        mcf::slab_plan_kernel<<<2, 1024, 0, st>>>(sp);
-        BITS_LAUNCH_CHECK();
-      }
-      {
-        msd::BucketArgs ba;
-        for (int a = 0; a < 2; ++a) {
-          ba.arr[a].src = L.slabs[a]; ba.arr[a].dst = L.b.buf[a][0]; ba.arr[a].bucket_start = L.b.bucket_start[a];
-          ba.arr[a].n_buckets = L.b.n_buckets + a; ba.arr[a].flag = L.b.msd_flag + a;
-          ba.arr[a].q_sorted = a ? q_start_sorted : q_end_sorted; ba.arr[a].qb = L.qb[a];
-        }
-        ba.slab = ps.slab; ba.round_flag = ps.flag; ba.round_total = out;
-        const uint32_t per = (uint32_t)kSMs;
         ProfScope prof(kClsBucketSortSearch, st);
-        msd::bucket_sort_kernel<true, true><<<dim3(ps.n_bins < per ? ps.n_bins : per, 2), msd::kBkThreads, msd::kBkSmem, st>>>(ba);
+        mct::bin_sort_search_kernel<<<pt.n_bins < blocks ? pt.n_bins : blocks, mct::kBsThreads, mct::kBsSmem, st>>>(bs);
         BITS_LAUNCH_CHECK();
       }
     }

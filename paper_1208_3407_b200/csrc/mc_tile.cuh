@@ -1,0 +1,365 @@
+// mc_tile.cuh -- the Monte Carlo round when the SEARCHED set is re-placed (BITS_PERMUTE_B;
+// "a random interval set is generated and placed into the associated data
+// structure" every round), as TWO launches with no global atomics on the data path:
+//
+//   place_tile_kernel   place (Philox4x32-10 -> start', end') fused with the
+//                       first half of the sort: every tile of <= 8192 fresh intervals is ordered
+//                       by bin (bin = start' >> shift, fixed per call) in shared memory and
+//                       written out as (start', end') pairs, coalesced; next to it goes the
+//                       tile's exclusive bin prefix, transposed:  off[b][tile] = #{pairs of the
+//                       tile in bins < b}.  Fresh keys never go to HBM unsorted.
+//   bin_sort_search_kernel  one bin at a time per block.  Row b of the prefix table gives, per
+//                       tile, where the bin's pairs sit; its row sum is the number of keys in
+//                       all earlier bins, i.e. where the bin starts in the sorted arrays -- no
+//                       histogram pass, no scan over bins, no reservation.  The pairs are
+//                       gathered (cp.async) into shared memory; starts and ends are each sorted
+//                       there (Algorithm 2's Sort(B_S), Sort(B_E): counting
+//                       sort on the next 12 bits, ties inside a sub-bucket ordered by comparison
+//                       counting on the way out), written to B_S / B_E, and -- while the bin is
+//                       still in shared memory -- the queries that fall into its key range are
+//                       ranked against it (Algorithm 1's two BSEARCHes) and
+//                       their ranks summed.
+//
+// An end that lies in the bin after its start's bin (span < bin width is a precondition of this
+// path, checked on the host) is handed over through a small per-bin list.  A bin with more than
+// kCap keys or an over-full hand-over list raises the round's flag; the host redoes flagged
+// rounds with the general path (place_kernel -> sort_arrays -> sorted_query_total_kernel).
+#pragma once
+#include "msd_sort.cuh"
+#include "philox_place.cuh"
+
+namespace bits {
+namespace mct {
+
+constexpr int kMaxBins = 4096;
+constexpr int kPtThreads = 512;
+constexpr int kPtIpt = 16;                       // intervals per thread and tile (four groups of four consecutive ones)
+constexpr int kTile = kPtThreads * kPtIpt;       // 8192 intervals
+constexpr size_t kPtSmem = (size_t)kTile * sizeof(uint2) + (size_t)(kMaxBins + kMaxChromSmem) * sizeof(uint32_t);
+
+constexpr int kBsThreads = 512;
+constexpr int kBsKpt = 16;
+constexpr int kCap = kBsThreads * kBsKpt;        // 8192 keys per bin and array
+constexpr int kSubBits = 12;
+constexpr int kSub = 1 << kSubBits;
+constexpr int kCrossCap = 512;                   // hand-over list entries per bin
+constexpr size_t kBsSmem = (size_t)(2 * kCap + 2 * (kSub + 32)) * sizeof(uint32_t);
+
+constexpr uint32_t kFlagBinTooBig = 1u, kFlagCrossFull = 4u;
+
+struct PlaceTileArgs {
+  const uint32_t* spans;     // dev uint32[n], padded to a multiple of 4 with zeros, 16-byte aligned
+  uint32_t n;
+  uint32_t tile;             // intervals per tile: a multiple of 4, <= kTile (balanced over the grid by the host)
+  uint32_t n_tiles;
+  uint32_t round;
+  uint32_t tag;
+  PhiloxKeys key;
+  ChromTable chrom;
+  uint32_t shift;            // bin = key >> shift, 1..31
+  uint32_t n_bins;           // <= kMaxBins
+  uint2* pairs;              // [n]: tile t holds its intervals [t * tile, ...) ordered by bin
+  uint16_t* off;             // [(n_bins + 1) * stride]: off[b * stride + t] = #{pairs of tile t in bins < b}
+  uint32_t stride;
+  uint32_t* cross_cnt;       // [n_bins + 1] ends handed over to each bin this round (zero on entry)
+  uint32_t* cross_keys;      // [n_bins * kCrossCap]
+  uint32_t* flag;            // round flag
+};
+
+__global__ void __launch_bounds__(kPtThreads, 2) place_tile_kernel(PlaceTileArgs a) {
+  constexpr int kPer = kMaxBins / kPtThreads;   // 8 bin counters per thread
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  uint2* s_stage = reinterpret_cast<uint2*>(smem_raw);                   // [kTile]
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_stage + kTile);        // [kMaxBins] counts, then bases
+  uint32_t* s_off = s_cnt + kMaxBins;                                    // [kMaxChromSmem]
+  __shared__ uint32_t s_w[32];
+  const int tid = threadIdx.x;
+  for (int i = tid; i < kMaxBins; i += kPtThreads) s_cnt[i] = 0;
+  const uint32_t* off = stage_chrom_table(a.chrom, s_off);               // barrier inside
+  const uint32_t shift = a.shift;
+  for (uint32_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
+    const uint32_t base = tile * a.tile;
+    const uint32_t count = min(a.tile, a.n - base);
+    uint32_t st[kPtIpt], rp[kPtIpt / 2];
+#pragma unroll
+    for (int g = 0; g < kPtIpt / 4; ++g) {
+      const uint32_t l0 = 4u * (tid + g * kPtThreads);                   // four consecutive intervals of the tile
+      rp[2 * g] = 0; rp[2 * g + 1] = 0;
+      if (l0 < count) {
+        const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l0));
+        const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
+        uint32_t ss[4];
+        place4(base + l0, a.round, a.tag, a.key, dd, off, a.chrom, ss);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          st[4 * g + j] = ss[j];
+          if (l0 + j < count) {
+            const uint32_t bin = ss[j] >> shift;
+            const uint32_t r = atomicAdd(&s_cnt[bin], 1u);
+            rp[2 * g + (j >> 1)] |= r << (16 * (j & 1));
+            const uint32_t e = ss[j] + dd[j], ebin = e >> shift;
+            if (ebin != bin) {                                           // rare: the end lies in the next bin
+              const uint32_t slot = atomicAdd(&a.cross_cnt[ebin], 1u);
+              if (slot < (uint32_t)kCrossCap) a.cross_keys[(size_t)ebin * kCrossCap + slot] = e;
+              else atomicOr(a.flag, kFlagCrossFull);
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();
+    // exclusive scan of the bin counts -> bases (kept in s_cnt) and the transposed prefix row entries
+    {
+      const uint4 v0 = reinterpret_cast<const uint4*>(s_cnt)[2 * tid], v1 = reinterpret_cast<const uint4*>(s_cnt)[2 * tid + 1];
+      const uint32_t c[kPer] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+      uint32_t sum = 0;
+#pragma unroll
+      for (int j = 0; j < kPer; ++j) sum += c[j];
+      uint32_t run = msd::block_excl_scan<kPtThreads>(sum, s_w);
+      uint32_t lb[kPer];
+#pragma unroll
+      for (int j = 0; j < kPer; ++j) { lb[j] = run; run += c[j]; }
+      reinterpret_cast<uint4*>(s_cnt)[2 * tid] = make_uint4(lb[0], lb[1], lb[2], lb[3]);
+      reinterpret_cast<uint4*>(s_cnt)[2 * tid + 1] = make_uint4(lb[4], lb[5], lb[6], lb[7]);
+      const uint32_t b0 = (uint32_t)tid * kPer;
+      if (b0 <= a.n_bins) {
+        uint16_t* o = a.off + (size_t)b0 * a.stride + tile;
+#pragma unroll
+        for (int j = 0; j < kPer; ++j)
+          if (b0 + j <= a.n_bins) o[(size_t)j * a.stride] = (uint16_t)lb[j];
+      }
+    }
+    __syncthreads();
+    // stage the pairs in bin order (spans re-read: L1 hits)
+#pragma unroll
+    for (int g = 0; g < kPtIpt / 4; ++g) {
+      const uint32_t l0 = 4u * (tid + g * kPtThreads);
+      if (l0 < count) {
+        const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l0));
+        const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (l0 + j < count) {
+            const uint32_t s = st[4 * g + j];
+            const uint32_t r = (rp[2 * g + (j >> 1)] >> (16 * (j & 1))) & 0xffffu;
+            s_stage[s_cnt[s >> shift] + r] = make_uint2(s, s + dd[j]);
+          }
+      }
+    }
+    __syncthreads();
+    reinterpret_cast<uint4*>(s_cnt)[2 * tid] = make_uint4(0, 0, 0, 0);
+    reinterpret_cast<uint4*>(s_cnt)[2 * tid + 1] = make_uint4(0, 0, 0, 0);
+    {
+      uint2* __restrict__ dst = a.pairs + base;                          // base % 4 == 0: 32-byte aligned
+      const uint32_t c2 = count >> 1;
+#pragma unroll
+      for (int j = 0; j < kPtIpt / 2; ++j) {
+        const uint32_t i = tid + j * kPtThreads;
+        if (i < c2) reinterpret_cast<uint4*>(dst)[i] = reinterpret_cast<const uint4*>(s_stage)[i];
+      }
+      if ((count & 1u) && tid == 0) dst[count - 1] = s_stage[count - 1];
+    }
+    __syncthreads();   // s_stage and s_cnt are free again
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+struct BinSortArgs {
+  const uint2* pairs;
+  const uint16_t* off;
+  uint32_t stride;
+  uint32_t n_tiles;
+  uint32_t tile;
+  uint32_t n;                           // keys per array
+  uint32_t shift;
+  uint32_t n_bins;
+  const uint32_t* cross_cnt;            // this round's hand-over counts
+  const uint32_t* cross_keys;
+  uint32_t* cross_cnt_next;             // the other parity: cleared here for the next round
+  uint32_t* dst[2];                     // B_S, B_E: the sorted arrays of this round
+  const uint32_t* q_sorted[2];          // ascending: A's ends (ranked in B_S, "<="), A's starts (ranked in B_E, "<")
+  const uint32_t* qb[2];                // [n_bins + 1]: queries qb[d] .. qb[d+1]-1 fall into bin d's key range
+  uint32_t n_q;
+  unsigned long long* round_total;      // += sum of ranks in B_S - sum of ranks in B_E
+  uint32_t* flag;
+};
+
+// Sort buf[0..m) (keys of bin d; entries whose bin is not d are dropped), write them to
+// dst[gbase ..], rank the queries q_sorted[qlo..qhi) and return this thread's sum of ranks.
+// s_sub: kSub + 1 counters, zero on entry; s_clear: the other counter array, cleared here.
+template <bool kStrict>
+__device__ __forceinline__ uint64_t sort_bin(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint32_t* s_sub,
+                                             uint32_t* s_clear, uint32_t* s_w, uint32_t gbase, uint32_t* __restrict__ dst,
+                                             const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi) {
+  constexpr int kPer = kSub / kBsThreads;   // 8
+  const int tid = threadIdx.x;
+  const uint32_t mask = (1u << shift) - 1u;
+  const uint32_t sshift = shift > (uint32_t)kSubBits ? shift - kSubBits : 0u;
+  uint32_t key[kBsKpt], rp[kBsKpt / 2];
+#pragma unroll
+  for (int j = 0; j < kBsKpt; ++j) {
+    if ((j & 1) == 0) rp[j >> 1] = 0xffffffffu;
+    if ((uint32_t)(j * kBsThreads) >= m) continue;
+    const uint32_t i = tid + j * kBsThreads;
+    if (i < m) {
+      const uint32_t k = buf[i];
+      key[j] = k;
+      if ((k >> shift) == d) {
+        const uint32_t r = atomicAdd(&s_sub[(k & mask) >> sshift], 1u);
+        rp[j >> 1] = (j & 1) ? ((rp[j >> 1] & 0xffffu) | (r << 16)) : ((rp[j >> 1] & 0xffff0000u) | r);
+      }
+    }
+  }
+  __syncthreads();
+  uint32_t mv;   // valid keys
+  {
+    uint32_t c[kPer];
+    const uint4 v0 = reinterpret_cast<const uint4*>(s_sub)[2 * tid], v1 = reinterpret_cast<const uint4*>(s_sub)[2 * tid + 1];
+    c[0] = v0.x; c[1] = v0.y; c[2] = v0.z; c[3] = v0.w; c[4] = v1.x; c[5] = v1.y; c[6] = v1.z; c[7] = v1.w;
+    uint32_t sum = 0;
+#pragma unroll
+    for (int j = 0; j < kPer; ++j) sum += c[j];
+    uint32_t run = msd::block_excl_scan<kBsThreads>(sum, s_w, &mv);
+    uint32_t lb[kPer];
+#pragma unroll
+    for (int j = 0; j < kPer; ++j) { lb[j] = run; run += c[j]; }
+    reinterpret_cast<uint4*>(s_sub)[2 * tid] = make_uint4(lb[0], lb[1], lb[2], lb[3]);
+    reinterpret_cast<uint4*>(s_sub)[2 * tid + 1] = make_uint4(lb[4], lb[5], lb[6], lb[7]);
+    if (tid == 0) s_sub[kSub] = mv;
+    reinterpret_cast<uint4*>(s_clear)[2 * tid] = make_uint4(0, 0, 0, 0);
+    reinterpret_cast<uint4*>(s_clear)[2 * tid + 1] = make_uint4(0, 0, 0, 0);
+  }
+  __syncthreads();
+  // in place: every key of the bin is in a register by now
+#pragma unroll
+  for (int j = 0; j < kBsKpt; ++j) {
+    if ((uint32_t)(j * kBsThreads) >= m) continue;
+    const uint32_t r = (rp[j >> 1] >> (16 * (j & 1))) & 0xffffu;
+    if (r != 0xffffu) buf[s_sub[(key[j] & mask) >> sshift] + r] = key[j];
+  }
+  __syncthreads();
+  // write out; keys that share a sub-bucket are ordered by comparison counting
+#pragma unroll
+  for (int j = 0; j < kBsKpt; ++j) {
+    if ((uint32_t)(j * kBsThreads) >= mv) continue;
+    const uint32_t p = tid + j * kBsThreads;
+    if (p < mv) {
+      const uint32_t k = buf[p];
+      const uint32_t sb = (k & mask) >> sshift;
+      const uint32_t lo = s_sub[sb], hi = s_sub[sb + 1];
+      uint32_t rank = 0;
+      for (uint32_t t = lo; t < hi; ++t) { const uint32_t kk = buf[t]; rank += (kk < k) | ((kk == k) & (t < p)); }
+      dst[gbase + lo + rank] = k;
+    }
+  }
+  // the queries of this bin: every key of an earlier sub-bucket is smaller, finish inside q's own
+  uint64_t qsum = 0;
+  for (uint32_t qi = qlo + tid; qi < qhi; qi += kBsThreads) {
+    const uint32_t q = __ldg(q_sorted + qi);
+    const uint32_t sb = (q & mask) >> sshift;
+    const uint32_t lo = s_sub[sb], hi = s_sub[sb + 1];
+    uint32_t c = 0;
+    for (uint32_t t = lo; t < hi; ++t) c += kStrict ? (buf[t] < q) : (buf[t] <= q);
+    qsum += (uint64_t)gbase + lo + c;
+  }
+  return qsum;
+}
+
+__global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortArgs a) {
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  uint32_t* s_ks = reinterpret_cast<uint32_t*>(smem_raw);    // [kCap] starts
+  uint32_t* s_ke = s_ks + kCap;                              // [kCap] ends (own + handed over)
+  uint32_t* s_sub0 = s_ke + kCap;                            // [kSub + 32]
+  uint32_t* s_sub1 = s_sub0 + kSub + 32;                     // [kSub + 32]
+  __shared__ uint32_t s_w[32], s_w2[32];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  for (int i = tid; i < kSub + 32; i += kBsThreads) { s_sub0[i] = 0; s_sub1[i] = 0; }
+  const uint32_t runs = (a.n_tiles + kBsThreads - 1) / kBsThreads;    // tiles per thread (contiguous)
+  const uint32_t t0 = min(a.n_tiles, (uint32_t)tid * runs), t1 = min(a.n_tiles, t0 + runs);
+  uint64_t qsum = 0;    // two's-complement: + ranks in B_S, - ranks in B_E
+  for (uint32_t d = blockIdx.x; d < a.n_bins; d += gridDim.x) {
+    a.cross_cnt_next[d] = 0;   // (every thread writes the same zero: harmless, and no divergence)
+    const uint16_t* __restrict__ row0 = a.off + (size_t)d * a.stride;
+    const uint16_t* __restrict__ row1 = row0 + a.stride;
+    uint32_t len_sum = 0, lo_sum = 0;
+    for (uint32_t t = t0; t < t1; ++t) { const uint32_t lo = __ldg(row0 + t), hi = __ldg(row1 + t); len_sum += hi - lo; lo_sum += lo; }
+    // exclusive scan of len_sum (where this thread's pairs go) and block sum of lo_sum (keys in earlier bins)
+    uint32_t incl = len_sum, ls = lo_sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, incl, o); if (lane >= o) incl += t; }
+    ls = __reduce_add_sync(kFullMask, ls);
+    __syncthreads();           // everyone is done with the previous bin's buffers and with s_w / s_w2
+    if (lane == 31) { s_w[w] = incl; s_w2[w] = ls; }
+    __syncthreads();
+    uint32_t x = lane < kBsThreads / 32 ? s_w[lane] : 0u;
+    const uint32_t gbase = __reduce_add_sync(kFullMask, lane < kBsThreads / 32 ? s_w2[lane] : 0u);
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, x, o); if (lane >= o) x += t; }
+    const uint32_t np = __shfl_sync(kFullMask, x, 31);                  // pairs in this bin
+    uint32_t pos = incl - len_sum + (w ? __shfl_sync(kFullMask, x, (w + 31) & 31) : 0u);
+    const uint32_t n_in = min(__ldg(a.cross_cnt + d), (uint32_t)kCrossCap);
+    const uint32_t qlo0 = __ldg(a.qb[0] + d), qhi0 = __ldg(a.qb[0] + d + 1);
+    const uint32_t qlo1 = __ldg(a.qb[1] + d), qhi1 = __ldg(a.qb[1] + d + 1);
+    if (np + n_in > (uint32_t)kCap) {                                   // block-uniform
+      if (tid == 0) atomicOr(a.flag, kFlagBinTooBig);
+      continue;
+    }
+    // gather the bin's pairs from every tile; starts and ends go to separate arrays
+    for (uint32_t t = t0; t < t1; ++t) {
+      const uint32_t lo = __ldg(row0 + t), hi = __ldg(row1 + t);
+      const uint2* src = a.pairs + (size_t)t * a.tile + lo;
+      for (uint32_t j = 0; j < hi - lo; ++j, ++pos) {
+        msd::cp_async4(s_ks + pos, &src[j].x);
+        msd::cp_async4(s_ke + pos, &src[j].y);
+      }
+    }
+    if ((uint32_t)tid < n_in) msd::cp_async4(s_ke + np + tid, a.cross_keys + (size_t)d * kCrossCap + tid);
+    msd::cp_async_wait_all();
+    __syncthreads();
+    // starts: all np keys belong to bin d; B_S position of the bin = gbase
+    qsum += sort_bin<false>(s_ks, np, d, a.shift, s_sub0, s_sub1, s_w, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0);
+    // ends: own ends that stay in the bin + the handed-over ones; n_in ends of earlier pairs lie in this bin
+    qsum -= sort_bin<true>(s_ke, np + n_in, d, a.shift, s_sub1, s_sub0, s_w, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
+  }
+  if (blockIdx.x == 0 && tid == 0) {
+    // queries beyond the last bin count every key
+    qsum += (uint64_t)(a.n_q - __ldg(a.qb[0] + a.n_bins)) * a.n;
+    qsum -= (uint64_t)(a.n_q - __ldg(a.qb[1] + a.n_bins)) * a.n;
+  }
+  __shared__ uint64_t s_red[kBsThreads / 32];
+  __syncthreads();
+  qsum = warp_sum_u64(qsum);
+  if (lane == 0) s_red[w] = qsum;
+  __syncthreads();
+  if (w == 0) {
+    uint64_t t = lane < kBsThreads / 32 ? s_red[lane] : 0;
+    t = warp_sum_u64(t);
+    if (lane == 0 && t != 0) atomicAdd(a.round_total, (unsigned long long)t);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Query ranges per bin, once per call: qb[b] = #{sorted queries < b << shift}, b = 0 .. n_bins.
+struct QueryBinsArgs {
+  const uint32_t* q_sorted[2];   // [n_q] each (A's ends for the start array, A's starts for the end array)
+  uint32_t* qb[2];               // [kMaxBins + 1]
+  uint32_t n_q;
+  uint32_t n_bins;
+  uint32_t shift;
+};
+
+__global__ void __launch_bounds__(256) query_bins_kernel(QueryBinsArgs a) {
+  const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b > a.n_bins) return;
+  const uint32_t* __restrict__ q = blockIdx.y ? a.q_sorted[1] : a.q_sorted[0];
+  const uint64_t bound = (uint64_t)b << a.shift;
+  uint32_t lo = 0, hi = a.n_q;
+  while (lo < hi) {
+    const uint32_t mid = lo + ((hi - lo) >> 1);
+    if ((uint64_t)q[mid] < bound) lo = mid + 1; else hi = mid;
+  }
+  (blockIdx.y ? a.qb[1] : a.qb[0])[b] = lo;
+}
+
+}  // namespace mct
+}  // namespace bits

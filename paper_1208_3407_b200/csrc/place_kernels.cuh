@@ -9,19 +9,23 @@
 
 namespace bits {
 
-// spans[i] = end[i] - start[i]; also the maximum span (for the NO_PLACEMENT check) and,
-// optionally, a malformed-interval flag.  Output padded to a multiple of 4 with zeros.
+// spans[i] = end[i] - start[i]; also the maximum span (for the NO_PLACEMENT check) and the sum of
+// the spans (their mean sizes the fused Monte Carlo path).  Output padded to a multiple of 4 with zeros.
 __global__ void __launch_bounds__(256) spans_kernel(const uint32_t* __restrict__ start, const uint32_t* __restrict__ end,
-                                                    uint32_t n, uint32_t* __restrict__ spans, uint32_t* max_span) {
+                                                    uint32_t n, uint32_t* __restrict__ spans, uint32_t* max_span,
+                                                    unsigned long long* span_sum) {
   uint32_t m = 0;
+  uint64_t sum = 0;
   const uint64_t n_pad = align_up(n, 4);
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pad; i += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t d = i < n ? end[i] - start[i] : 0u;
     spans[i] = d;
     m = max(m, d);
+    sum += d;
   }
   m = __reduce_max_sync(kFullMask, m);
-  if ((threadIdx.x & 31) == 0 && m) atomicMax(max_span, m);
+  sum = warp_sum_u64(sum);
+  if ((threadIdx.x & 31) == 0 && m) { atomicMax(max_span, m); atomicAdd(span_sum, (unsigned long long)sum); }
 }
 
 // flag |= 1 if any start > end
