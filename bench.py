@@ -34,6 +34,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
+NCU_TRAFFIC_BYTES: dict = {}
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
@@ -315,25 +317,43 @@ def run_b200(args):
     rounds_total = world * R * args.steps
     value = rounds_total / (elapsed_ms * 1e-3)
 
-    # ---- roofline of the dominant kernel (one digit pass of the radix sort over both key arrays) ----
+    # ---- roofline of the dominant kernel (the class with the largest share of the timed region) ----
     peak, peak_src = measured_peaks()
     n_sorted = w.n_b if w.which == 1 else 0
+    n_p = w.n_b if w.which == 1 else w.n_a
+    # algorithmic HBM bytes per launch of each kernel class: what the step must move
+    alg = {
+        "place": ("place_kernel", 12 * n_p),                                   # span in, two keys out
+        "sort_pass": ("onesweep_pass_kernel", 2 * n_sorted * 8),               # two arrays x (read + write)
+        "place_scatter": ("place_tile_kernel", 12 * n_p),                      # span in, (start, end) pair out
+        "bucket_sort_search": ("bin_sort_search_kernel", 16 * n_sorted + 8 * w.n_a),   # pairs in, B_S and B_E out, sorted queries in
+        "sorted_query": ("sorted_query_total_kernel", 8 * w.n_a),
+        "mc_permute_a": ("mc_permute_a_kernel", 4 * w.n_a * min(R, 32768)),
+    }
     roofline = None
-    if prof["sort_pass"][1] and n_sorted:
-        pass_ms = prof["sort_pass"][0] / prof["sort_pass"][1]
-        alg_bytes = 2 * n_sorted * 8                      # two arrays x (4 B read + 4 B write) per key
-        achieved = alg_bytes / (pass_ms * 1e-3) / 1e9
-        shares = {k: v[0] for k, v in prof.items() if v[1]}
-        tot = sum(shares.values())
-        roofline = {"bound": "hbm", "kernel": "onesweep_pass_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                    "avg_launch_ms": pass_ms, "launches_timed": prof["sort_pass"][1],
-                    "algorithmic_bytes_per_launch": alg_bytes,
-                    "kernel_ms_per_round": {k: v[0] / (R * args.steps) for k, v in prof.items() if v[1]},
-                    "kernel_share_of_step": {k: v / tot for k, v in shares.items()},
-                    "round_hbm_bytes_model": 12 * n_sorted + 72 * n_sorted - 8 * n_sorted + 8 * w.n_a,
-                    }
-        roofline["round_frac_of_peak"] = roofline["round_hbm_bytes_model"] * value / world / 1e9 / peak
+    timed = {k: v for k, v in prof.items() if v[1] and v[0] > 0}
+    if timed:
+        tot = sum(v[0] for v in timed.values())
+        dom = max((k for k in timed if k in alg), key=lambda k: timed[k][0], default=None)
+        if dom is not None:
+            kname, alg_bytes = alg[dom]
+            launch_ms = timed[dom][0] / timed[dom][1]
+            achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+            roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                        "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(kname), "peak_source": peak_src,
+                        "avg_launch_ms": launch_ms, "launches_timed": timed[dom][1],
+                        "algorithmic_bytes_per_launch": alg_bytes,
+                        "kernel_ms_per_round": {k: v[0] / (R * args.steps) for k, v in timed.items()},
+                        "kernel_share_of_step": {k: v[0] / tot for k, v in timed.items()}}
+            if n_sorted:
+                # SURVEY 8(d) per-round model: place 12 M + sort 72 M (histogram fused: - 8 M) + search 8 N_q
+                model = 12 * n_sorted + 72 * n_sorted - 8 * n_sorted + 8 * w.n_a
+                roofline["round_hbm_bytes_model"] = model
+                roofline["round_frac_of_peak"] = model * value / world / 1e9 / peak
+                # what the two-launch design itself must move per round
+                own = 12 * n_sorted + 16 * n_sorted + 8 * w.n_a
+                roofline["round_hbm_bytes_this_design"] = own
+                roofline["round_frac_of_peak_this_design"] = own * value / world / 1e9 / peak
 
     line = {
         "metric": "mc_rounds_per_s", "value": value, "unit": "rounds/s", "n_gpus": world, "steps": args.steps,
@@ -346,7 +366,6 @@ def run_b200(args):
     }
     if roofline:
         line["roofline"] = roofline
-        line["sort_keys_per_s_kernel_only"] = 2 * n_sorted / (4 * roofline["avg_launch_ms"] * 1e-3)
     if clocks is not None:
         line["clocks"] = clocks
 

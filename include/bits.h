@@ -82,6 +82,15 @@ enum {
 size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which,
                             uint32_t flags);
 
+/* Where, inside a workspace of bits_workspace_bytes(fn, ...) bytes, the call leaves the sorted
+ * arrays it searched (Algorithm 2's B_S and B_E): array 0 = B_S (ascending
+ * starts), 1 = B_E (ascending ends), n_b keys each, valid once the stream has drained.  After
+ * bits_mc_rounds with BITS_PERMUTE_B they are those of the LAST round.  For inspection and for
+ * the parity tests of the sort step inside the Monte Carlo loop.  *offset_out: host, bytes.
+ * Returns BITS_ERR_FLAGS for an fn that sorts no interval set or a bad array. */
+int bits_workspace_sorted_offset(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which,
+                                 int array, size_t* offset_out);
+
 /* Extra device bytes the *_host variant of `fn` needs to stage its inputs and outputs. */
 size_t bits_host_staging_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_rounds);
 

@@ -28,6 +28,7 @@ _lib = None
 
 _SIGNATURES = {
     "bits_workspace_bytes": (C.c_size_t, [C.c_int, C.c_uint64, C.c_uint64, C.c_uint32, C.c_int, C.c_uint32]),
+    "bits_workspace_sorted_offset": (C.c_int, [C.c_int, C.c_uint64, C.c_uint64, C.c_uint32, C.c_int, C.c_int, C.c_void_p]),
     "bits_host_staging_bytes": (C.c_size_t, [C.c_int, C.c_uint64, C.c_uint64, C.c_uint32]),
     "bits_count": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t,
                              _u64p, _vp]),
@@ -115,6 +116,16 @@ def profile_read() -> dict:
 
 def workspace_bytes(fn: int, n_a: int, n_b: int, n_chrom: int = 0, which: int = 0, flags: int = 0) -> int:
     return int(lib().bits_workspace_bytes(fn, n_a, n_b, n_chrom, which, flags))
+
+
+def sorted_arrays_in_workspace(ws: torch.Tensor, fn: int, n_a: int, n_b: int, n_chrom: int = 0, which: int = 0):
+    """(B_S, B_E) views into a workspace the call `fn` ran with (bits_workspace_sorted_offset)."""
+    out = []
+    for array in (0, 1):
+        off = C.c_size_t(0)
+        _chk(lib().bits_workspace_sorted_offset(fn, n_a, n_b, n_chrom, which, array, C.addressof(off)))
+        out.append(ws[off.value: off.value + 4 * n_b].view(torch.int32))
+    return tuple(out)
 
 
 def host_staging_bytes(fn: int, n_a: int, n_b: int, n_rounds: int = 0) -> int:

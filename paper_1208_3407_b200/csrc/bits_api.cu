@@ -133,11 +133,13 @@ struct Small {            // small device scalars
   uint32_t* bad;          // [1]
   unsigned long long* span_sum;   // [1]
   uint32_t* chrom;        // [n_chrom + 1]
+  uint16_t* lut;          // [kLutSize] position -> chromosome look-up table
   void carve(Carver& c, uint32_t n_chrom) {
     max_span = c.take<uint32_t>(64);
     bad = max_span ? max_span + 1 : nullptr;
     span_sum = max_span ? reinterpret_cast<unsigned long long*>(max_span + 2) : nullptr;
     chrom = c.take<uint32_t>((uint64_t)n_chrom + 1);
+    lut = c.take<uint16_t>(kLutSize);
   }
 };
 
@@ -486,6 +488,21 @@ static int check_genome(const uint32_t* off, uint32_t n_chrom, ChromTable* t, ui
   return BITS_OK;
 }
 
+// Copy the offset table and its look-up table into the workspace and point `t` at them.
+static int upload_genome(const uint32_t* off, uint32_t n_chrom, const Small& sm, ChromTable* t, cudaStream_t st) {
+  t->off = sm.chrom;
+  t->lut = nullptr;
+  t->lut_shift = 0;
+  BITS_CUDA_TRY(cudaMemcpyAsync(sm.chrom, off, sizeof(uint32_t) * ((size_t)n_chrom + 1), cudaMemcpyHostToDevice, st));
+  if (n_chrom + 1 <= (uint32_t)kMaxChromSmem && n_chrom < 65536u) {
+    uint16_t lut[kLutSize];
+    t->lut_shift = make_chrom_lut(off, n_chrom, lut);
+    BITS_CUDA_TRY(cudaMemcpyAsync(sm.lut, lut, sizeof(lut), cudaMemcpyHostToDevice, st));   // pageable: staged before return
+    t->lut = sm.lut;
+  }
+  return BITS_OK;
+}
+
 static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* end_out, uint32_t n, uint32_t round,
                         uint32_t tag, const PhiloxKeys& key, const ChromTable& chrom, bool vec, int hist_mode,
                         uint32_t* hist_s, uint32_t* hist_e, uint32_t* zero_s, uint32_t* zero_e, cudaStream_t st) {
@@ -520,8 +537,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   if (!ws_ok(ws, ws_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
   if (flags & BITS_VALIDATE)
     BITS_TRY(validate_inputs(a_start, a_end, (uint32_t)n_a, b_start, b_end, (uint32_t)n_b, L.small.bad, st));
-  chrom.off = L.small.chrom;
-  BITS_CUDA_TRY(cudaMemcpyAsync(L.small.chrom, off, sizeof(uint32_t) * ((size_t)n_chrom + 1), cudaMemcpyHostToDevice, st));
+  BITS_TRY(upload_genome(off, n_chrom, L.small, &chrom, st));
   BITS_CUDA_TRY(cudaMemsetAsync(observed_out, 0, sizeof(uint64_t), st));
   if (n_rounds) BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out, 0, sizeof(uint64_t) * (size_t)n_rounds, st));
 
@@ -640,7 +656,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     for (uint32_t c = 0; c < n_chrom; ++c) { const uint32_t Lc = off[c + 1] - off[c]; v_min += Lc > h_max_span ? Lc - h_max_span : 0; }
     const uint64_t G = off[n_chrom];
     int best = -1;
-    for (int sh = 31; sh >= 1 && v_min > 0; --sh) {
+    for (int sh = mct::kMaxShift; sh >= 1 && v_min > 0; --sh) {
       const uint64_t nbins = (G + (1ull << sh) - 1) >> sh;
       if (nbins >= (uint64_t)mct::kMaxBins) break;
       if ((uint64_t)h_max_span >= (1ull << sh)) break;     // an end may lie at most one bin after its start
@@ -764,6 +780,17 @@ size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom
   return make_layout(nullptr, fn, n_a, n_b, n_chrom, which).bytes;
 }
 
+int bits_workspace_sorted_offset(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which, int array,
+                                 size_t* offset_out) {
+  if (!offset_out) return BITS_ERR_NULL;
+  if (fn < BITS_FN_COUNT || fn > BITS_FN_MC_ROUNDS || (array != 0 && array != 1)) return BITS_ERR_FLAGS;
+  if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return BITS_ERR_SIZE;
+  char* const base = reinterpret_cast<char*>(uintptr_t(1) << 20);   // any non-null base: only differences are used
+  const Layout L = make_layout(base, fn, n_a, n_b, n_chrom, which);
+  *offset_out = (size_t)(reinterpret_cast<char*>(L.b.buf[array][0]) - base);
+  return BITS_OK;
+}
+
 size_t bits_host_staging_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_rounds) {
   if (fn < BITS_FN_COUNT || fn > BITS_FN_MC_ROUNDS) return 0;
   return make_stage(nullptr, n_a, n_b, n_rounds, fn == BITS_FN_COUNT_PER_INTERVAL).bytes;
@@ -803,9 +830,7 @@ int bits_place(const uint32_t* spans, uint64_t n, const uint32_t* chrom_offsets,
   const Layout L = make_layout(workspace, BITS_FN_PLACE, 0, 0, n_chrom, 0);
   if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
   if (n == 0) return BITS_OK;
-  chrom.off = L.small.chrom;
-  BITS_CUDA_TRY(cudaMemcpyAsync(L.small.chrom, chrom_offsets, sizeof(uint32_t) * ((size_t)n_chrom + 1),
-                                cudaMemcpyHostToDevice, st));
+  BITS_TRY(upload_genome(chrom_offsets, n_chrom, L.small, &chrom, st));
   const bool vec = (n & 3) == 0 && (((uintptr_t)spans | (uintptr_t)start_out | (uintptr_t)end_out) & 15) == 0;
   return launch_place(spans, start_out, end_out, (uint32_t)n, round, tag, make_philox_keys(seed), chrom, vec, kHistNone,
                       nullptr, nullptr, nullptr, nullptr, st);

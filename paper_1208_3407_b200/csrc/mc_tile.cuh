@@ -35,15 +35,18 @@ constexpr int kMaxBins = 4096;
 constexpr int kPtThreads = 512;
 constexpr int kPtIpt = 16;                       // intervals per thread and tile (four groups of four consecutive ones)
 constexpr int kTile = kPtThreads * kPtIpt;       // 8192 intervals
-constexpr size_t kPtSmem = (size_t)kTile * sizeof(uint2) + (size_t)(kMaxBins + kMaxChromSmem) * sizeof(uint32_t);
+constexpr size_t kPtSmem = (size_t)kTile * sizeof(uint2) + (size_t)(kMaxBins + kMaxChromSmem) * sizeof(uint32_t) +
+                           (size_t)kLutSize * sizeof(uint16_t);
 
 constexpr int kBsThreads = 512;
 constexpr int kBsKpt = 16;
 constexpr int kCap = kBsThreads * kBsKpt;        // 8192 keys per bin and array
-constexpr int kSubBits = 12;
-constexpr int kSub = 1 << kSubBits;
+constexpr int kSubBits = 13;
+constexpr int kSub = 1 << kSubBits;              // sub-buckets per bin: 16-bit counters, two per word
+constexpr int kSubPad = kSub + 64;               // + the end sentinel, padded to whole uint4s
 constexpr int kCrossCap = 512;                   // hand-over list entries per bin
-constexpr size_t kBsSmem = (size_t)(2 * kCap + 2 * (kSub + 32)) * sizeof(uint32_t);
+constexpr int kMaxShift = 21;                    // key bits below the bin index: a rank of >= 11 bits fits beside them
+constexpr size_t kBsSmem = (size_t)(2 * kCap) * sizeof(uint32_t) + (size_t)(2 * kSubPad) * sizeof(uint16_t);
 
 constexpr uint32_t kFlagBinTooBig = 1u, kFlagCrossFull = 4u;
 
@@ -72,10 +75,11 @@ __global__ void __launch_bounds__(kPtThreads, 2) place_tile_kernel(PlaceTileArgs
   uint2* s_stage = reinterpret_cast<uint2*>(smem_raw);                   // [kTile]
   uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_stage + kTile);        // [kMaxBins] counts, then bases
   uint32_t* s_off = s_cnt + kMaxBins;                                    // [kMaxChromSmem]
+  uint16_t* s_lut = reinterpret_cast<uint16_t*>(s_off + kMaxChromSmem);  // [kLutSize]
   __shared__ uint32_t s_w[32];
   const int tid = threadIdx.x;
   for (int i = tid; i < kMaxBins; i += kPtThreads) s_cnt[i] = 0;
-  const uint32_t* off = stage_chrom_table(a.chrom, s_off);               // barrier inside
+  const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);        // barrier inside
   const uint32_t shift = a.shift;
   for (uint32_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
     const uint32_t base = tile * a.tile;
@@ -184,81 +188,103 @@ struct BinSortArgs {
   uint32_t* flag;
 };
 
-// Sort buf[0..m) (keys of bin d; entries whose bin is not d are dropped), write them to
-// dst[gbase ..], rank the queries q_sorted[qlo..qhi) and return this thread's sum of ranks.
-// s_sub: kSub + 1 counters, zero on entry; s_clear: the other counter array, cleared here.
-template <bool kStrict>
-__device__ __forceinline__ uint64_t sort_bin(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint32_t* s_sub,
-                                             uint32_t* s_clear, uint32_t* s_w, uint32_t gbase, uint32_t* __restrict__ dst,
-                                             const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi) {
-  constexpr int kPer = kSub / kBsThreads;   // 8
+// Sort buf[0..m) (keys of bin d; with kCheckBin, entries whose bin is not d are dropped), write
+// them to dst[gbase ..], rank the queries q_sorted[qlo..qhi) and return this thread's sum of ranks.
+// s_cnt: kSub + 2 uint16 counters (zero on entry) = sub-bucket counts, then exclusive prefixes;
+// s_clear: the other counter array, cleared here for the next call.
+// Counting sort on the kSubBits bits below `shift` with shared-memory atomics (two 16-bit counters
+// per word); a key travels through the phases as  low | rank-in-sub-bucket << shift  in a register.
+// Keys that share a sub-bucket (about every third one) are ordered by comparison counting on the
+// way out.  Returns through *overflow whether a rank did not fit beside the key (block-uniform
+// after the barrier is the caller's job: it is OR-ed into the round flag).
+template <bool kStrict, bool kCheckBin>
+__device__ __forceinline__ uint64_t sort_bin(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint16_t* s_cnt,
+                                             uint16_t* s_clear, uint32_t* s_w, uint32_t gbase, uint32_t* __restrict__ dst,
+                                             const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi,
+                                             uint32_t* flag) {
+  constexpr int kWords = kSub / 2 / kBsThreads;   // counter words per thread in the scan
+  static_assert(kWords % 4 == 0, "uint4 accesses");
   const int tid = threadIdx.x;
   const uint32_t mask = (1u << shift) - 1u;
   const uint32_t sshift = shift > (uint32_t)kSubBits ? shift - kSubBits : 0u;
-  uint32_t key[kBsKpt], rp[kBsKpt / 2];
+  const uint32_t rlimit = (1u << (32u - shift)) - 1u;   // ranks below this fit beside the key (and never give ~0)
+  const uint32_t hibits = d << shift;
+  uint32_t* cnt32 = reinterpret_cast<uint32_t*>(s_cnt);
+  uint32_t kr[kBsKpt];
+  bool over = false;
 #pragma unroll
   for (int j = 0; j < kBsKpt; ++j) {
-    if ((j & 1) == 0) rp[j >> 1] = 0xffffffffu;
+    kr[j] = 0xffffffffu;
     if ((uint32_t)(j * kBsThreads) >= m) continue;
     const uint32_t i = tid + j * kBsThreads;
     if (i < m) {
       const uint32_t k = buf[i];
-      key[j] = k;
-      if ((k >> shift) == d) {
-        const uint32_t r = atomicAdd(&s_sub[(k & mask) >> sshift], 1u);
-        rp[j >> 1] = (j & 1) ? ((rp[j >> 1] & 0xffffu) | (r << 16)) : ((rp[j >> 1] & 0xffff0000u) | r);
+      if (!kCheckBin || (k >> shift) == d) {
+        const uint32_t low = k & mask, sb = low >> sshift, sh16 = (sb & 1u) << 4;
+        const uint32_t r = (atomicAdd(&cnt32[sb >> 1], 1u << sh16) >> sh16) & 0xffffu;
+        over |= r >= rlimit;
+        kr[j] = low | (r << shift);
       }
     }
   }
+  if (over) atomicOr(flag, kFlagBinTooBig);   // the round is redone by the general path; what follows stays in bounds
   __syncthreads();
   uint32_t mv;   // valid keys
   {
-    uint32_t c[kPer];
-    const uint4 v0 = reinterpret_cast<const uint4*>(s_sub)[2 * tid], v1 = reinterpret_cast<const uint4*>(s_sub)[2 * tid + 1];
-    c[0] = v0.x; c[1] = v0.y; c[2] = v0.z; c[3] = v0.w; c[4] = v1.x; c[5] = v1.y; c[6] = v1.z; c[7] = v1.w;
+    uint32_t c[kWords];
+#pragma unroll
+    for (int j = 0; j < kWords / 4; ++j) {
+      const uint4 v = reinterpret_cast<const uint4*>(cnt32)[(kWords / 4) * tid + j];
+      c[4 * j] = v.x; c[4 * j + 1] = v.y; c[4 * j + 2] = v.z; c[4 * j + 3] = v.w;
+    }
     uint32_t sum = 0;
 #pragma unroll
-    for (int j = 0; j < kPer; ++j) sum += c[j];
+    for (int j = 0; j < kWords; ++j) sum += (c[j] & 0xffffu) + (c[j] >> 16);
     uint32_t run = msd::block_excl_scan<kBsThreads>(sum, s_w, &mv);
-    uint32_t lb[kPer];
 #pragma unroll
-    for (int j = 0; j < kPer; ++j) { lb[j] = run; run += c[j]; }
-    reinterpret_cast<uint4*>(s_sub)[2 * tid] = make_uint4(lb[0], lb[1], lb[2], lb[3]);
-    reinterpret_cast<uint4*>(s_sub)[2 * tid + 1] = make_uint4(lb[4], lb[5], lb[6], lb[7]);
-    if (tid == 0) s_sub[kSub] = mv;
-    reinterpret_cast<uint4*>(s_clear)[2 * tid] = make_uint4(0, 0, 0, 0);
-    reinterpret_cast<uint4*>(s_clear)[2 * tid + 1] = make_uint4(0, 0, 0, 0);
+    for (int j = 0; j < kWords; ++j) {
+      const uint32_t lo = c[j] & 0xffffu, hi = c[j] >> 16;
+      c[j] = run | ((run + lo) << 16);
+      run += lo + hi;
+    }
+#pragma unroll
+    for (int j = 0; j < kWords / 4; ++j) {
+      reinterpret_cast<uint4*>(cnt32)[(kWords / 4) * tid + j] = make_uint4(c[4 * j], c[4 * j + 1], c[4 * j + 2], c[4 * j + 3]);
+      reinterpret_cast<uint4*>(s_clear)[(kWords / 4) * tid + j] = make_uint4(0, 0, 0, 0);
+    }
+    if (tid == 0) s_cnt[kSub] = (uint16_t)mv;
   }
   __syncthreads();
   // in place: every key of the bin is in a register by now
 #pragma unroll
   for (int j = 0; j < kBsKpt; ++j) {
     if ((uint32_t)(j * kBsThreads) >= m) continue;
-    const uint32_t r = (rp[j >> 1] >> (16 * (j & 1))) & 0xffffu;
-    if (r != 0xffffu) buf[s_sub[(key[j] & mask) >> sshift] + r] = key[j];
+    if (kr[j] != 0xffffffffu) {
+      const uint32_t low = kr[j] & mask;
+      uint32_t pos = (uint32_t)s_cnt[low >> sshift] + (kr[j] >> shift);
+      pos = pos < (uint32_t)kCap ? pos : 0u;            // only after an overflow (flag raised)
+      buf[pos] = hibits | low;
+    }
   }
   __syncthreads();
-  // write out; keys that share a sub-bucket are ordered by comparison counting
-#pragma unroll
-  for (int j = 0; j < kBsKpt; ++j) {
-    if ((uint32_t)(j * kBsThreads) >= mv) continue;
-    const uint32_t p = tid + j * kBsThreads;
-    if (p < mv) {
-      const uint32_t k = buf[p];
-      const uint32_t sb = (k & mask) >> sshift;
-      const uint32_t lo = s_sub[sb], hi = s_sub[sb + 1];
-      uint32_t rank = 0;
-      for (uint32_t t = lo; t < hi; ++t) { const uint32_t kk = buf[t]; rank += (kk < k) | ((kk == k) & (t < p)); }
-      dst[gbase + lo + rank] = k;
-    }
+  // write out; keys that share a sub-bucket are ordered by comparison counting (ties by position)
+  for (uint32_t p = tid; p < mv; p += kBsThreads) {
+    const uint32_t k = buf[p];
+    const uint32_t sb = (k & mask) >> sshift;
+    const uint32_t lo = s_cnt[sb], hi = s_cnt[sb + 1];
+    uint32_t rank = 0;
+#pragma unroll 1
+    for (uint32_t t = lo; t < hi; ++t) { const uint32_t kk = buf[t]; rank += (kk < k) | ((kk == k) & (t < p)); }
+    dst[gbase + lo + rank] = k;
   }
   // the queries of this bin: every key of an earlier sub-bucket is smaller, finish inside q's own
   uint64_t qsum = 0;
   for (uint32_t qi = qlo + tid; qi < qhi; qi += kBsThreads) {
     const uint32_t q = __ldg(q_sorted + qi);
     const uint32_t sb = (q & mask) >> sshift;
-    const uint32_t lo = s_sub[sb], hi = s_sub[sb + 1];
+    const uint32_t lo = s_cnt[sb], hi = s_cnt[sb + 1];
     uint32_t c = 0;
+#pragma unroll 1
     for (uint32_t t = lo; t < hi; ++t) c += kStrict ? (buf[t] < q) : (buf[t] <= q);
     qsum += (uint64_t)gbase + lo + c;
   }
@@ -269,11 +295,11 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
   extern __shared__ __align__(16) uint8_t smem_raw[];
   uint32_t* s_ks = reinterpret_cast<uint32_t*>(smem_raw);    // [kCap] starts
   uint32_t* s_ke = s_ks + kCap;                              // [kCap] ends (own + handed over)
-  uint32_t* s_sub0 = s_ke + kCap;                            // [kSub + 32]
-  uint32_t* s_sub1 = s_sub0 + kSub + 32;                     // [kSub + 32]
+  uint16_t* s_sub0 = reinterpret_cast<uint16_t*>(s_ke + kCap);   // [kSubPad]
+  uint16_t* s_sub1 = s_sub0 + kSubPad;                           // [kSubPad]
   __shared__ uint32_t s_w[32], s_w2[32];
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  for (int i = tid; i < kSub + 32; i += kBsThreads) { s_sub0[i] = 0; s_sub1[i] = 0; }
+  for (int i = tid; i < kSubPad; i += kBsThreads) { reinterpret_cast<uint32_t*>(s_sub0)[i] = 0; }   // both arrays
   const uint32_t runs = (a.n_tiles + kBsThreads - 1) / kBsThreads;    // tiles per thread (contiguous)
   const uint32_t t0 = min(a.n_tiles, (uint32_t)tid * runs), t1 = min(a.n_tiles, t0 + runs);
   uint64_t qsum = 0;    // two's-complement: + ranks in B_S, - ranks in B_E
@@ -317,9 +343,9 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
     msd::cp_async_wait_all();
     __syncthreads();
     // starts: all np keys belong to bin d; B_S position of the bin = gbase
-    qsum += sort_bin<false>(s_ks, np, d, a.shift, s_sub0, s_sub1, s_w, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0);
+    qsum += sort_bin<false, false>(s_ks, np, d, a.shift, s_sub0, s_sub1, s_w, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0, a.flag);
     // ends: own ends that stay in the bin + the handed-over ones; n_in ends of earlier pairs lie in this bin
-    qsum -= sort_bin<true>(s_ke, np + n_in, d, a.shift, s_sub1, s_sub0, s_w, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
+    qsum -= sort_bin<true, true>(s_ke, np + n_in, d, a.shift, s_sub1, s_sub0, s_w, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1, a.flag);
   }
   if (blockIdx.x == 0 && tid == 0) {
     // queries beyond the last bin count every key

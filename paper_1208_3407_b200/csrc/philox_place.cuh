@@ -11,14 +11,37 @@
 namespace bits {
 
 constexpr int kMaxChromSmem = 1024;   // offset tables up to this many entries are staged in shared memory
+constexpr int kLutSize = 1024;        // entries of the position -> chromosome look-up table
 
 struct ChromTable {
   const uint32_t* off;   // dev uint32[n_chrom + 1]
+  const uint16_t* lut;   // dev uint16[kLutSize]: lut[e] = chromosome that holds position e << lut_shift
   uint32_t n_chrom;
   uint32_t l_min;        // shortest chromosome: spans below it fit every chromosome (fast path)
   uint32_t genome;       // G = off[n_chrom]
   uint32_t step0;        // largest power of two <= max(n_chrom - 1, 1); 0 if n_chrom == 1
+  uint32_t lut_shift;    // (G >> lut_shift) < kLutSize
 };
+
+// The offset table as a kernel searches it: in shared memory (with the look-up table) when it fits.
+struct ChromView {
+  const uint32_t* off;
+  const uint16_t* lut;   // null: binary search
+};
+
+// lut[e] = #{c >= 1 : off[c] <= e << shift}, e = 0 .. G >> shift (host side, once per call).
+inline uint32_t make_chrom_lut(const uint32_t* off, uint32_t n_chrom, uint16_t* lut) {
+  const uint64_t G = off[n_chrom];
+  uint32_t shift = 0;
+  while ((G >> shift) >= (uint64_t)kLutSize) ++shift;
+  uint32_t c = 0;
+  for (uint32_t e = 0; e < (uint32_t)kLutSize; ++e) {
+    const uint64_t pos = (uint64_t)e << shift;
+    while (c + 1 < n_chrom && (uint64_t)off[c + 1] <= pos) ++c;
+    lut[e] = (uint16_t)c;
+  }
+  return shift;
+}
 
 // The ten round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), computed once on the host.
 struct PhiloxKeys {
@@ -53,17 +76,25 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 // Fast path (d < l_min, every chromosome can hold the span): V = G - C*d < 2^32, the running
 // count of valid starts before chromosome c is off[c] - c*d, so the chromosome is found by a
 // fixed-trip binary search and start' = u + c*d.  General path: the literal walk in 64 bits.
-__device__ __forceinline__ uint32_t place_start(uint32_t xl, uint32_t xh, uint32_t d,
-                                                const uint32_t* __restrict__ off, const ChromTable& t) {
+__device__ __forceinline__ uint32_t place_start(uint32_t xl, uint32_t xh, uint32_t d, const ChromView& cv,
+                                                const ChromTable& t) {
+  const uint32_t* __restrict__ off = cv.off;
   if (d < t.l_min) {
     const uint32_t V = t.genome - t.n_chrom * d;
     // u = (x * V) >> 64 with x = xh:xl (64 bits) and V < 2^32
     const uint32_t carry = __umulhi(xl, V);
     const uint32_t u = (uint32_t)(((uint64_t)xh * V + carry) >> 32);
     uint32_t c = 0;
-    for (uint32_t s = t.step0; s > 0; s >>= 1) {
-      const uint32_t m = c + s;
-      if (m < t.n_chrom && off[m] - m * d <= u) c = m;
+    if (cv.lut) {
+      // the thresholds off[c] - c*d only move down as d grows, so the chromosome of u for d = 0
+      // (read from the table at the start of u's block) is a lower bound: step up from there
+      c = cv.lut[u >> t.lut_shift];
+      while (c + 1 < t.n_chrom && off[c + 1] - (c + 1) * d <= u) ++c;
+    } else {
+      for (uint32_t s = t.step0; s > 0; s >>= 1) {
+        const uint32_t m = c + s;
+        if (m < t.n_chrom && off[m] - m * d <= u) c = m;
+      }
     }
     return u + c * d;
   }
@@ -84,20 +115,27 @@ __device__ __forceinline__ uint32_t place_start(uint32_t xl, uint32_t xh, uint32
   return start;
 }
 
-// Stage the offset table in shared memory when it fits; returns the pointer to search through.
-// Ends with __syncthreads().
-__device__ __forceinline__ const uint32_t* stage_chrom_table(const ChromTable& t, uint32_t* s_off) {
+// Stage the offset table (and the look-up table, s_lut = kLutSize entries) in shared memory when
+// it fits; returns the view to search through.  Ends with __syncthreads().
+__device__ __forceinline__ ChromView stage_chrom_table(const ChromTable& t, uint32_t* s_off, uint16_t* s_lut) {
   const bool fits = t.n_chrom + 1 <= (uint32_t)kMaxChromSmem;
+  const bool with_lut = fits && t.lut != nullptr && s_lut != nullptr;
   if (fits)
     for (uint32_t i = threadIdx.x; i <= t.n_chrom; i += blockDim.x) s_off[i] = t.off[i];
+  if (with_lut)
+    for (uint32_t i = threadIdx.x; i < (uint32_t)kLutSize / 2; i += blockDim.x)
+      reinterpret_cast<uint32_t*>(s_lut)[i] = reinterpret_cast<const uint32_t*>(t.lut)[i];
   __syncthreads();
-  return fits ? s_off : t.off;
+  ChromView v;
+  v.off = fits ? s_off : t.off;
+  v.lut = with_lut ? s_lut : nullptr;
+  return v;
 }
 
 // Four consecutive intervals i0..i0+3 (i0 % 4 == 0) of round `round`: two Philox calls.
 // Interval i uses counter (i >> 1, round, tag, 0) and output words 2h, 2h+1 with h = i & 1.
 __device__ __forceinline__ void place4(uint32_t i0, uint32_t round, uint32_t tag, const PhiloxKeys& key,
-                                       const uint32_t d[4], const uint32_t* off, const ChromTable& t,
+                                       const uint32_t d[4], const ChromView& off, const ChromTable& t,
                                        uint32_t start[4]) {
   const uint4 r0 = philox4x32_10(i0 >> 1, round, tag, 0u, key);
   const uint4 r1 = philox4x32_10((i0 >> 1) + 1u, round, tag, 0u, key);

@@ -63,13 +63,14 @@ template <bool kVec, int kHist>
 __global__ void __launch_bounds__(256) place_kernel(PlaceArgs a) {
   constexpr int kHalf = kHist == kHistDigits ? rs::kPasses * rs::kRadix : (kHist == kHistBins ? msd::kBins : 1);
   __shared__ uint32_t s_off[kMaxChromSmem];
+  __shared__ __align__(16) uint16_t s_lut[kLutSize];
   __shared__ uint32_t s_h[kHist != kHistNone ? 2 * kHalf : 1];
   if (kHist != kHistNone) {
     for (int i = threadIdx.x; i < 2 * kHalf; i += blockDim.x) s_h[i] = 0;
     if (kHist == kHistDigits && blockIdx.x == 0 && a.zero_a)
       for (int i = threadIdx.x; i < kHalf; i += blockDim.x) { a.zero_a[i] = 0; a.zero_b[i] = 0; }
   }
-  const uint32_t* off = stage_chrom_table(a.chrom, s_off);   // barrier inside
+  const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);   // barrier inside
   const uint32_t n = a.n;
   const uint32_t n4 = (uint32_t)(((uint64_t)n + 3) >> 2);
   for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n4; t += (uint64_t)gridDim.x * blockDim.x) {

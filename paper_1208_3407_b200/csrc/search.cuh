@@ -203,8 +203,9 @@ struct McAArgs {
 
 __global__ void __launch_bounds__(256) mc_permute_a_kernel(McAArgs a) {
   __shared__ uint32_t s_off[kMaxChromSmem];
+  __shared__ __align__(16) uint16_t s_lut[kLutSize];
   __shared__ uint64_t s_red[8];
-  const uint32_t* off = stage_chrom_table(a.chrom, s_off);
+  const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);
   const uint32_t round = a.round0 + blockIdx.y;
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t i0 = t << 2;

@@ -312,6 +312,23 @@ def test_mc_config5_full_size_sampled_rounds():
     assert np.array_equal(rc2, rc[:3])
 
 
+@pytest.mark.parametrize("k,scale,rounds", [(1, 1.0, 3), (5, 0.02, 2), (5, 1.0, 2)])
+def test_mc_permute_b_leaves_sorted_arrays_of_last_round(k, scale, rounds):
+    """The sort step inside the Monte Carlo loop: after R rounds the workspace holds B_S and B_E of round
+    R-1, which must equal std::sort of the oracle's placement of that round, element for element."""
+    w = W.make_config(k, scale=scale)
+    n_chrom = int(w.chrom_offsets.size - 1)
+    ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, 1), dtype=torch.uint8, device=DEV)
+    bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, 1, w.mc_seed, 5, rounds,
+                   workspace=ws)
+    sync()
+    b_s, b_e = bits.sorted_arrays_in_workspace(ws, bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, 1)
+    spans = (w.b_end - w.b_start).astype(np.uint32)
+    o_s, o_e = oracle.place_round(spans, w.chrom_offsets, w.mc_seed, 5 + rounds - 1, 1)
+    assert np.array_equal(host_u32(b_s), oracle.sort_u32(o_s))
+    assert np.array_equal(host_u32(b_e), oracle.sort_u32(o_e))
+
+
 # ------------------------------------------------------------------------------------- host-buffer entry points
 def test_host_variants_config1():
     w = W.make_config(1)
