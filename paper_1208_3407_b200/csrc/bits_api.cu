@@ -655,20 +655,21 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     uint64_t v_min = 0;
     for (uint32_t c = 0; c < n_chrom; ++c) { const uint32_t Lc = off[c + 1] - off[c]; v_min += Lc > h_max_span ? Lc - h_max_span : 0; }
     const uint64_t G = off[n_chrom];
-    int best = -1;
-    for (int sh = mct::kMaxShift; sh >= 1 && v_min > 0; --sh) {
+    // does a bin of 2^sh coordinates hold its keys, its hand-over list and every span with a wide margin?
+    auto fits = [&](int sh) -> bool {
       const uint64_t nbins = (G + (1ull << sh) - 1) >> sh;
-      if (nbins >= (uint64_t)mct::kMaxBins) break;
-      if ((uint64_t)h_max_span >= (1ull << sh)) break;     // an end may lie at most one bin after its start
+      if (nbins >= (uint64_t)mct::kMaxBins) return false;
+      if ((uint64_t)h_max_span >= (1ull << sh)) return false;   // an end may lie at most one bin after its start
       const double avg = (double)n_b * (double)(1ull << sh) / (double)v_min;
-      const double need = avg * 1.125 + 8.0 * sqrt(avg) + 32.0;
-      if (need > (double)mct::kCap) continue;
-      // ends handed over per bin: about avg * mean span / bin width
-      const double cross = avg * h_mean_span / (double)(1ull << sh);
-      if (cross * 2.0 + 8.0 * sqrt(cross) + 32.0 > (double)mct::kCrossCap) continue;
-      best = sh;
-      break;
-    }
+      if (avg * 1.125 + 8.0 * sqrt(avg) + 32.0 > (double)mct::kCap) return false;
+      const double cross = avg * h_mean_span / (double)(1ull << sh);   // ends handed over per bin
+      return cross * 2.0 + 8.0 * sqrt(cross) + 32.0 <= (double)mct::kCrossCap;
+    };
+    int best = -1;
+    for (int sh = mct::kMaxShift; sh >= 1 && v_min > 0; --sh)
+      if (fits(sh)) { best = sh; break; }
+    // a small set: narrower bins (finer sub-buckets, more blocks) as long as there are no more bins than blocks
+    while (best > 1 && fits(best - 1) && ((G + (1ull << (best - 1)) - 1) >> (best - 1)) <= 2ull * kSMs) --best;
     fused_ok = best >= 0;
     if (fused_ok) {
       pt.spans = L.spans; pt.n = (uint32_t)n_b; pt.tag = 1u; pt.key = key; pt.chrom = chrom;

@@ -43,10 +43,9 @@ constexpr int kBsKpt = 16;
 constexpr int kCap = kBsThreads * kBsKpt;        // 8192 keys per bin and array
 constexpr int kSubBits = 13;
 constexpr int kSub = 1 << kSubBits;              // sub-buckets per bin: 16-bit counters, two per word
-constexpr int kSubPad = kSub + 64;               // + the end sentinel, padded to whole uint4s
 constexpr int kCrossCap = 512;                   // hand-over list entries per bin
-constexpr int kMaxShift = 21;                    // key bits below the bin index: a rank of >= 11 bits fits beside them
-constexpr size_t kBsSmem = (size_t)(2 * kCap) * sizeof(uint32_t) + (size_t)(2 * kSubPad) * sizeof(uint16_t);
+constexpr int kMaxShift = 21;                    // widest bin: 2^21 coordinates, i.e. sub-buckets of 2^8
+constexpr size_t kBsSmem = (size_t)(2 * kCap) * sizeof(uint32_t) + (size_t)(2 * (8 + kSub + 8)) * sizeof(uint16_t);
 
 constexpr uint32_t kFlagBinTooBig = 1u, kFlagCrossFull = 4u;
 
@@ -188,101 +187,130 @@ struct BinSortArgs {
   uint32_t* flag;
 };
 
-// Sort buf[0..m) (keys of bin d; with kCheckBin, entries whose bin is not d are dropped), write
-// them to dst[gbase ..], rank the queries q_sorted[qlo..qhi) and return this thread's sum of ranks.
-// s_cnt: kSub + 2 uint16 counters (zero on entry) = sub-bucket counts, then exclusive prefixes;
-// s_clear: the other counter array, cleared here for the next call.
-// Counting sort on the kSubBits bits below `shift` with shared-memory atomics (two 16-bit counters
-// per word); a key travels through the phases as  low | rank-in-sub-bucket << shift  in a register.
-// Keys that share a sub-bucket (about every third one) are ordered by comparison counting on the
-// way out.  Returns through *overflow whether a rank did not fit beside the key (block-uniform
-// after the barrier is the caller's job: it is OR-ed into the round flag).
-template <bool kStrict, bool kCheckBin>
-__device__ __forceinline__ uint64_t sort_bin(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint16_t* s_cnt,
-                                             uint16_t* s_clear, uint32_t* s_w, uint32_t gbase, uint32_t* __restrict__ dst,
-                                             const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi,
-                                             uint32_t* flag) {
-  constexpr int kWords = kSub / 2 / kBsThreads;   // counter words per thread in the scan
+// Counter arrays of one bin: uint16 cursors, two per word.  Entry kFront + sb belongs to
+// sub-bucket sb; entry kFront - 1 stays 0, so after the scatter (which leaves every cursor at
+// the END of its sub-bucket) the keys of sub-bucket sb sit at [cur[kFront + sb - 1], cur[kFront + sb]).
+constexpr int kFront = 8;                        // halfwords in front of the cursors (one uint4)
+constexpr int kCurLen = kFront + kSub + 8;       // halfwords per cursor array, a whole number of uint4s
+
+__device__ __forceinline__ uint32_t sub_of(uint32_t key, uint32_t mask, uint32_t sshift) { return (key & mask) >> sshift; }
+
+// ++count of the key's sub-bucket (no result needed: a reduction, not an atomic with return)
+__device__ __forceinline__ void count_key(uint32_t* cur32, uint32_t sb) {
+  const uint32_t e = sb + kFront;
+  atomicAdd(&cur32[e >> 1], 1u << ((e & 1u) << 4));
+}
+// position of the next key of sub-bucket sb; bumps the cursor
+__device__ __forceinline__ uint32_t take_slot(uint32_t* cur32, uint32_t sb) {
+  const uint32_t e = sb + kFront, sh = (e & 1u) << 4;
+  return (atomicAdd(&cur32[e >> 1], 1u << sh) >> sh) & 0xffffu;
+}
+
+// Counts -> exclusive prefixes, in place, for both cursor arrays (starts, ends) with one pair of
+// barriers.  total[0], total[1] = keys counted per array.  s_w: 64 words of scratch.
+__device__ __forceinline__ void scan_cursors(uint16_t* cur_s, uint16_t* cur_e, uint32_t* s_w, uint32_t total[2]) {
+  constexpr int kWords = kSub / 2 / kBsThreads;   // cursor words per thread and array
   static_assert(kWords % 4 == 0, "uint4 accesses");
-  const int tid = threadIdx.x;
-  const uint32_t mask = (1u << shift) - 1u;
-  const uint32_t sshift = shift > (uint32_t)kSubBits ? shift - kSubBits : 0u;
-  const uint32_t rlimit = (1u << (32u - shift)) - 1u;   // ranks below this fit beside the key (and never give ~0)
-  const uint32_t hibits = d << shift;
-  uint32_t* cnt32 = reinterpret_cast<uint32_t*>(s_cnt);
-  uint32_t kr[kBsKpt];
-  bool over = false;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  uint32_t c[2][kWords], sum[2] = {0, 0};
 #pragma unroll
-  for (int j = 0; j < kBsKpt; ++j) {
-    kr[j] = 0xffffffffu;
-    if ((uint32_t)(j * kBsThreads) >= m) continue;
-    const uint32_t i = tid + j * kBsThreads;
-    if (i < m) {
-      const uint32_t k = buf[i];
-      if (!kCheckBin || (k >> shift) == d) {
-        const uint32_t low = k & mask, sb = low >> sshift, sh16 = (sb & 1u) << 4;
-        const uint32_t r = (atomicAdd(&cnt32[sb >> 1], 1u << sh16) >> sh16) & 0xffffu;
-        over |= r >= rlimit;
-        kr[j] = low | (r << shift);
-      }
-    }
-  }
-  if (over) atomicOr(flag, kFlagBinTooBig);   // the round is redone by the general path; what follows stays in bounds
-  __syncthreads();
-  uint32_t mv;   // valid keys
-  {
-    uint32_t c[kWords];
+  for (int a = 0; a < 2; ++a) {
+    const uint4* src = reinterpret_cast<const uint4*>((a ? cur_e : cur_s) + kFront) + (kWords / 4) * tid;
 #pragma unroll
     for (int j = 0; j < kWords / 4; ++j) {
-      const uint4 v = reinterpret_cast<const uint4*>(cnt32)[(kWords / 4) * tid + j];
-      c[4 * j] = v.x; c[4 * j + 1] = v.y; c[4 * j + 2] = v.z; c[4 * j + 3] = v.w;
+      const uint4 v = src[j];
+      c[a][4 * j] = v.x; c[a][4 * j + 1] = v.y; c[a][4 * j + 2] = v.z; c[a][4 * j + 3] = v.w;
     }
-    uint32_t sum = 0;
 #pragma unroll
-    for (int j = 0; j < kWords; ++j) sum += (c[j] & 0xffffu) + (c[j] >> 16);
-    uint32_t run = msd::block_excl_scan<kBsThreads>(sum, s_w, &mv);
+    for (int j = 0; j < kWords; ++j) sum[a] += (c[a][j] & 0xffffu) + (c[a][j] >> 16);
+  }
+  // both sums travel through one scan: starts in the low half, ends in the high half (each <= kCap)
+  uint32_t incl = sum[0] | (sum[1] << 16);
+  const uint32_t own = incl;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, incl, o); if (lane >= o) incl += t; }
+  if (lane == 31) s_w[w] = incl;
+  __syncthreads();
+  uint32_t x = lane < kBsThreads / 32 ? s_w[lane] : 0u;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, x, o); if (lane >= o) x += t; }
+  const uint32_t before = w ? __shfl_sync(kFullMask, x, (w + 31) & 31) : 0u;
+  const uint32_t tot = __shfl_sync(kFullMask, x, 31);
+  total[0] = tot & 0xffffu; total[1] = tot >> 16;
+  const uint32_t excl = incl - own + before;
+#pragma unroll
+  for (int a = 0; a < 2; ++a) {
+    uint32_t run = a ? (excl >> 16) : (excl & 0xffffu);
 #pragma unroll
     for (int j = 0; j < kWords; ++j) {
-      const uint32_t lo = c[j] & 0xffffu, hi = c[j] >> 16;
-      c[j] = run | ((run + lo) << 16);
+      const uint32_t lo = c[a][j] & 0xffffu, hi = c[a][j] >> 16;
+      c[a][j] = run | ((run + lo) << 16);
       run += lo + hi;
     }
+    uint4* dst = reinterpret_cast<uint4*>((a ? cur_e : cur_s) + kFront) + (kWords / 4) * tid;
 #pragma unroll
-    for (int j = 0; j < kWords / 4; ++j) {
-      reinterpret_cast<uint4*>(cnt32)[(kWords / 4) * tid + j] = make_uint4(c[4 * j], c[4 * j + 1], c[4 * j + 2], c[4 * j + 3]);
-      reinterpret_cast<uint4*>(s_clear)[(kWords / 4) * tid + j] = make_uint4(0, 0, 0, 0);
-    }
-    if (tid == 0) s_cnt[kSub] = (uint16_t)mv;
+    for (int j = 0; j < kWords / 4; ++j) dst[j] = make_uint4(c[a][4 * j], c[a][4 * j + 1], c[a][4 * j + 2], c[a][4 * j + 3]);
   }
   __syncthreads();
-  // in place: every key of the bin is in a register by now
+}
+
+// Counting-sort scatter of buf[0..m) in place: every key is read into a register, then (after a
+// barrier) stored at the slot its sub-bucket's cursor hands out.  With kCheckBin, entries whose
+// bin is not d are dropped.  Ends with a barrier; afterwards buf[0..valid) is ordered by
+// sub-bucket and cur[kFront + sb] is the END of sub-bucket sb.
+template <bool kCheckBin>
+__device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint32_t mask,
+                                                 uint32_t sshift, uint16_t* cur) {
+  const int tid = threadIdx.x;
+  uint32_t* cur32 = reinterpret_cast<uint32_t*>(cur);
+  uint32_t key[kBsKpt];
 #pragma unroll
   for (int j = 0; j < kBsKpt; ++j) {
-    if ((uint32_t)(j * kBsThreads) >= m) continue;
-    if (kr[j] != 0xffffffffu) {
-      const uint32_t low = kr[j] & mask;
-      uint32_t pos = (uint32_t)s_cnt[low >> sshift] + (kr[j] >> shift);
-      pos = pos < (uint32_t)kCap ? pos : 0u;            // only after an overflow (flag raised)
-      buf[pos] = hibits | low;
-    }
+    const uint32_t i = tid + j * kBsThreads;
+    key[j] = i < m ? buf[i] : 0u;
   }
   __syncthreads();
-  // write out; keys that share a sub-bucket are ordered by comparison counting (ties by position)
+#pragma unroll
+  for (int j = 0; j < kBsKpt; ++j) {
+    if ((uint32_t)(j * kBsThreads) >= m) break;
+    const uint32_t k = key[j];
+    if (tid + j * kBsThreads < m && (!kCheckBin || (k >> shift) == d)) buf[take_slot(cur32, sub_of(k, mask, sshift))] = k;
+  }
+  __syncthreads();
+}
+
+// Write buf[0..mv) (ordered by sub-bucket) to dst[gbase ..] in ascending order: the keys that
+// share a sub-bucket are ordered by comparison counting (ties by position), the first four
+// candidates without a loop.  Then rank the sorted queries q_sorted[qlo..qhi), all of which fall
+// into this bin's key range: every key of an earlier sub-bucket is smaller, the count is finished
+// inside the query's own sub-bucket.  Returns this thread's sum of query ranks.
+template <bool kStrict>
+__device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t mv, uint32_t mask, uint32_t sshift,
+                                                   const uint16_t* cur, uint32_t gbase, uint32_t* __restrict__ dst,
+                                                   const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi) {
+  const int tid = threadIdx.x;
   for (uint32_t p = tid; p < mv; p += kBsThreads) {
     const uint32_t k = buf[p];
-    const uint32_t sb = (k & mask) >> sshift;
-    const uint32_t lo = s_cnt[sb], hi = s_cnt[sb + 1];
+    const uint32_t sb = sub_of(k, mask, sshift);
+    const uint32_t lo = cur[kFront - 1 + sb], hi = cur[kFront + sb];
     uint32_t rank = 0;
+#pragma unroll
+    for (uint32_t i = 0; i < 4; ++i) {
+      const uint32_t t = lo + i;
+      const uint32_t kk = buf[t];                    // buf is padded: t < kCap + 4
+      rank += (t < hi) & (kk < k + (t < p ? 1u : 0u));
+    }
+    if (hi - lo > 4) {
 #pragma unroll 1
-    for (uint32_t t = lo; t < hi; ++t) { const uint32_t kk = buf[t]; rank += (kk < k) | ((kk == k) & (t < p)); }
+      for (uint32_t t = lo + 4; t < hi; ++t) rank += buf[t] < k + (t < p ? 1u : 0u);
+    }
     dst[gbase + lo + rank] = k;
   }
-  // the queries of this bin: every key of an earlier sub-bucket is smaller, finish inside q's own
   uint64_t qsum = 0;
   for (uint32_t qi = qlo + tid; qi < qhi; qi += kBsThreads) {
     const uint32_t q = __ldg(q_sorted + qi);
-    const uint32_t sb = (q & mask) >> sshift;
-    const uint32_t lo = s_cnt[sb], hi = s_cnt[sb + 1];
+    const uint32_t sb = sub_of(q, mask, sshift);
+    const uint32_t lo = cur[kFront - 1 + sb], hi = cur[kFront + sb];
     uint32_t c = 0;
 #pragma unroll 1
     for (uint32_t t = lo; t < hi; ++t) c += kStrict ? (buf[t] < q) : (buf[t] <= q);
@@ -293,13 +321,14 @@ __device__ __forceinline__ uint64_t sort_bin(uint32_t* buf, uint32_t m, uint32_t
 
 __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortArgs a) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  uint32_t* s_ks = reinterpret_cast<uint32_t*>(smem_raw);    // [kCap] starts
-  uint32_t* s_ke = s_ks + kCap;                              // [kCap] ends (own + handed over)
-  uint16_t* s_sub0 = reinterpret_cast<uint16_t*>(s_ke + kCap);   // [kSubPad]
-  uint16_t* s_sub1 = s_sub0 + kSubPad;                           // [kSubPad]
+  uint32_t* s_ks = reinterpret_cast<uint32_t*>(smem_raw);          // [kCap] starts
+  uint32_t* s_ke = s_ks + kCap;                                    // [kCap] ends (own + handed over)
+  uint16_t* s_cur_s = reinterpret_cast<uint16_t*>(s_ke + kCap);    // [kCurLen] cursors of the starts
+  uint16_t* s_cur_e = s_cur_s + kCurLen;                           // [kCurLen] cursors of the ends
   __shared__ uint32_t s_w[32], s_w2[32];
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  for (int i = tid; i < kSubPad; i += kBsThreads) { reinterpret_cast<uint32_t*>(s_sub0)[i] = 0; }   // both arrays
+  const uint32_t shift = a.shift, mask = (1u << shift) - 1u;
+  const uint32_t sshift = shift > (uint32_t)kSubBits ? shift - kSubBits : 0u;
   const uint32_t runs = (a.n_tiles + kBsThreads - 1) / kBsThreads;    // tiles per thread (contiguous)
   const uint32_t t0 = min(a.n_tiles, (uint32_t)tid * runs), t1 = min(a.n_tiles, t0 + runs);
   uint64_t qsum = 0;    // two's-complement: + ranks in B_S, - ranks in B_E
@@ -314,8 +343,10 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, incl, o); if (lane >= o) incl += t; }
     ls = __reduce_add_sync(kFullMask, ls);
-    __syncthreads();           // everyone is done with the previous bin's buffers and with s_w / s_w2
+    __syncthreads();           // everyone is done with the previous bin's buffers, cursors and s_w / s_w2
     if (lane == 31) { s_w[w] = incl; s_w2[w] = ls; }
+    // clear both cursor arrays (they are adjacent)
+    for (int i = tid; i < 2 * kCurLen / 8; i += kBsThreads) reinterpret_cast<uint4*>(s_cur_s)[i] = make_uint4(0, 0, 0, 0);
     __syncthreads();
     uint32_t x = lane < kBsThreads / 32 ? s_w[lane] : 0u;
     const uint32_t gbase = __reduce_add_sync(kFullMask, lane < kBsThreads / 32 ? s_w2[lane] : 0u);
@@ -342,10 +373,26 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
     if ((uint32_t)tid < n_in) msd::cp_async4(s_ke + np + tid, a.cross_keys + (size_t)d * kCrossCap + tid);
     msd::cp_async_wait_all();
     __syncthreads();
-    // starts: all np keys belong to bin d; B_S position of the bin = gbase
-    qsum += sort_bin<false, false>(s_ks, np, d, a.shift, s_sub0, s_sub1, s_w, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0, a.flag);
-    // ends: own ends that stay in the bin + the handed-over ones; n_in ends of earlier pairs lie in this bin
-    qsum -= sort_bin<true, true>(s_ke, np + n_in, d, a.shift, s_sub1, s_sub0, s_w, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1, a.flag);
+    // Algorithm 2's Sort(B_S), Sort(B_E) for this bin: count, scan, scatter
+    const uint32_t me = np + n_in;    // ends held: own ones (some belong to the next bin) + handed over
+    {
+      uint32_t* cs = reinterpret_cast<uint32_t*>(s_cur_s);
+      uint32_t* ce = reinterpret_cast<uint32_t*>(s_cur_e);
+      for (uint32_t i = tid; i < me; i += kBsThreads) {
+        if (i < np) count_key(cs, sub_of(s_ks[i], mask, sshift));
+        const uint32_t e = s_ke[i];
+        if ((e >> shift) == d) count_key(ce, sub_of(e, mask, sshift));
+      }
+    }
+    __syncthreads();
+    uint32_t total[2];
+    scan_cursors(s_cur_s, s_cur_e, s_w, total);                         // barriers inside
+    // starts: all np keys belong to bin d; the bin begins at gbase in B_S
+    scatter_in_place<false>(s_ks, np, d, shift, mask, sshift, s_cur_s);
+    qsum += write_and_rank<false>(s_ks, np, mask, sshift, s_cur_s, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0);
+    // ends: n_in ends of earlier pairs lie in this bin, so it begins at gbase - n_in in B_E
+    scatter_in_place<true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
+    qsum -= write_and_rank<true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
   }
   if (blockIdx.x == 0 && tid == 0) {
     // queries beyond the last bin count every key
