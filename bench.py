@@ -48,6 +48,8 @@ def parse_args():
     p.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     p.add_argument("--scale", type=float, default=1.0, help="scale the set sizes (testing only; 1.0 = the named config)")
     p.add_argument("--rounds", type=int, default=0, help="rounds per step (0 = the configuration's own count)")
+    p.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                   help="bits_set_option knob for design studies (DESIGN.md section 10); results never change")
     p.add_argument("--no-extras", action="store_true", help="skip the secondary workloads, e2e and cpu_baseline legs")
     p.add_argument("--no-profile-events", action="store_true", help="do not bracket kernels with events in the timed region")
     return p.parse_args()
@@ -264,6 +266,9 @@ def run_b200(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
     bits.lib()
+    for kv in args.opt:
+        name, _, val = kv.partition("=")
+        bits.set_option(name, int(val))
 
     w = W.make_config(args.config, scale=args.scale)
     if w.which is None:

@@ -23,6 +23,9 @@ struct Options {
   int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+tile sort / bin sort+search (mc_tile.cuh)
   int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
   int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
+  int64_t mc_tile_variant = 2;     // PERMUTE_B fused rounds: shape of place_tile_kernel (0: 2 x 512 threads, 1: 1 x 1024, 2: 1 x 1024 with longer tiles)
+  int64_t mc_bin_variant = 0;      // PERMUTE_B fused rounds: shape of the per-bin sort (0 wide, 1 narrow, 2 small blocks)
+  int64_t mc_gather_group = -1;    // PERMUTE_B fused rounds: log2 of the lanes per gathered segment (-1 = from the mean segment length)
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
 };
 static Options g_opt;
@@ -160,15 +163,18 @@ struct Layout {
 };
 constexpr uint32_t kFlagChunk = 4096;    // fused rounds are checked for raised flags in chunks of this many
 constexpr uint64_t kFusedMaxKeys = 24u << 20;   // beyond this the bins of the fused path cannot hold the set
-constexpr uint32_t kTileBlocks = 2u * 148u;     // place_tile_kernel: two resident blocks per SM
-// Tiles are balanced: every block gets the same number of equally sized tiles.
-static inline uint32_t tile_size_for(uint64_t n) {
-  const uint64_t per_block = ceil_div(n, (uint64_t)kTileBlocks * mct::kTile);
-  uint64_t tile = align_up(ceil_div(n, (uint64_t)kTileBlocks * (per_block ? per_block : 1)), 4);
-  if (tile > (uint64_t)mct::kTile) tile = mct::kTile;
+// Tiles are balanced: every block of place_tile_kernel gets the same number of equally sized tiles.
+static inline uint32_t tile_size_for(uint64_t n, uint32_t blocks, uint32_t max_tile) {
+  const uint64_t per_block = ceil_div(n, (uint64_t)blocks * max_tile);
+  uint64_t tile = align_up(ceil_div(n, (uint64_t)blocks * (per_block ? per_block : 1)), 4);
+  if (tile > (uint64_t)max_tile) tile = max_tile;
   if (tile < 4) tile = 4;
   return (uint32_t)tile;
 }
+template <class C>
+static inline uint32_t tile_size_cfg(uint64_t n) { return tile_size_for(n, (uint32_t)C::kBlocksPerSm * 148u, (uint32_t)C::kTile); }
+// the workspace is sized for the shape with the most tiles, whatever shape a call ends up using
+static inline uint32_t max_tiles_for(uint64_t n) { return (uint32_t)ceil_div(n, tile_size_cfg<mct::TileCfg2x512>(n)); }
 
 static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which) {
   Layout L;
@@ -187,7 +193,7 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
         L.spans = c.take<uint32_t>(align_up(n_b, 4) + 4);
         L.q.carve(c, n_a, false);
         if (n_b <= kFusedMaxKeys) {
-          const uint32_t n_tiles = (uint32_t)ceil_div(n_b, tile_size_for(n_b));
+          const uint32_t n_tiles = max_tiles_for(n_b);
           L.tile_stride = (uint32_t)align_up((uint64_t)n_tiles + 1, 8);
           L.pairs = c.take<uint2>(align_up(n_b, 4) + 4);
           L.tile_off = c.take<uint16_t>((uint64_t)(mct::kMaxBins + 1) * L.tile_stride);
@@ -304,8 +310,19 @@ static int msd_configure() {
   if (done < 0) {
     const cudaError_t e1 = cudaFuncSetAttribute(msd::scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kScSmem);
     const cudaError_t e2 = cudaFuncSetAttribute(msd::bucket_sort_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
-    const cudaError_t e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::kBsSmem);
-    const cudaError_t e4 = cudaFuncSetAttribute(mct::place_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::kPtSmem);
+    cudaError_t e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgWide>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)mct::BinCfgWide::smem_bytes(mct::kMaxTiles));
+    if (e3 == cudaSuccess)
+      e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgNarrow>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)mct::BinCfgNarrow::smem_bytes(mct::kMaxTiles));
+    if (e3 == cudaSuccess)
+      e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)mct::BinCfgSmall::smem_bytes(mct::kMaxTiles));
+    cudaError_t e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg2x512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg2x512::kSmem);
+    if (e4 == cudaSuccess)
+      e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024::kSmem);
+    if (e4 == cudaSuccess)
+      e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024L::kSmem);
     if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { (void)cudaGetLastError(); return BITS_ERR_CUDA; }
     done = 1;
   }
@@ -494,7 +511,7 @@ static int upload_genome(const uint32_t* off, uint32_t n_chrom, const Small& sm,
   t->lut = nullptr;
   t->lut_shift = 0;
   BITS_CUDA_TRY(cudaMemcpyAsync(sm.chrom, off, sizeof(uint32_t) * ((size_t)n_chrom + 1), cudaMemcpyHostToDevice, st));
-  if (n_chrom + 1 <= (uint32_t)kMaxChromSmem && n_chrom < 65536u) {
+  if (n_chrom + 2 <= (uint32_t)kMaxChromSmem && n_chrom < 65536u) {
     uint16_t lut[kLutSize];
     t->lut_shift = make_chrom_lut(off, n_chrom, lut);
     BITS_CUDA_TRY(cudaMemcpyAsync(sm.lut, lut, sizeof(lut), cudaMemcpyHostToDevice, st));   // pageable: staged before return
@@ -520,6 +537,18 @@ static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* en
   }
   BITS_LAUNCH_CHECK();
   return BITS_OK;
+}
+
+template <class C>
+static void launch_place_tile(const mct::PlaceTileArgs& pt, cudaStream_t st) {
+  const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
+  mct::place_tile_kernel<C><<<pt.n_tiles < blocks ? pt.n_tiles : blocks, C::kThreads, C::kSmem, st>>>(pt);
+}
+
+template <class C>
+static void launch_bin_sort(const mct::BinSortArgs& bs, cudaStream_t st) {
+  const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
+  mct::bin_sort_search_kernel<C><<<bs.n_bins < blocks ? bs.n_bins : blocks, C::kThreads, C::smem_bytes(bs.n_tiles), st>>>(bs);
 }
 
 static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
@@ -651,6 +680,9 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   mct::PlaceTileArgs pt;
   mct::BinSortArgs bs;
   bool fused_ok = msd_on && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0 && L.pairs != nullptr;
+  const int variant = (int)g_opt.mc_bin_variant;
+  const int tile_variant = (int)g_opt.mc_tile_variant;
+  const double bin_cap = variant == 0 ? (double)mct::BinCfgWide::kCap : (variant == 1 ? (double)mct::BinCfgNarrow::kCap : (double)mct::BinCfgSmall::kCap);
   if (fused_ok) {
     uint64_t v_min = 0;
     for (uint32_t c = 0; c < n_chrom; ++c) { const uint32_t Lc = off[c + 1] - off[c]; v_min += Lc > h_max_span ? Lc - h_max_span : 0; }
@@ -661,7 +693,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       if (nbins >= (uint64_t)mct::kMaxBins) return false;
       if ((uint64_t)h_max_span >= (1ull << sh)) return false;   // an end may lie at most one bin after its start
       const double avg = (double)n_b * (double)(1ull << sh) / (double)v_min;
-      if (avg * 1.125 + 8.0 * sqrt(avg) + 32.0 > (double)mct::kCap) return false;
+      if (avg * 1.125 + 8.0 * sqrt(avg) + 32.0 > bin_cap) return false;
       const double cross = avg * h_mean_span / (double)(1ull << sh);   // ends handed over per bin
       return cross * 2.0 + 8.0 * sqrt(cross) + 32.0 <= (double)mct::kCrossCap;
     };
@@ -674,13 +706,22 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     if (fused_ok) {
       pt.spans = L.spans; pt.n = (uint32_t)n_b; pt.tag = 1u; pt.key = key; pt.chrom = chrom;
       pt.shift = (uint32_t)best; pt.n_bins = (uint32_t)((G + (1ull << best) - 1) >> best);
-      pt.tile = tile_size_for(n_b); pt.n_tiles = (uint32_t)ceil_div(n_b, pt.tile);
+      pt.tile = tile_variant == 0 ? tile_size_cfg<mct::TileCfg2x512>(n_b)
+                                  : (tile_variant == 1 ? tile_size_cfg<mct::TileCfg1x1024>(n_b) : tile_size_cfg<mct::TileCfg1x1024L>(n_b));
+      pt.n_tiles = (uint32_t)ceil_div(n_b, pt.tile);
       pt.pairs = L.pairs; pt.off = L.tile_off; pt.stride = L.tile_stride; pt.cross_keys = L.cross_keys;
       bs.pairs = L.pairs; bs.off = L.tile_off; bs.stride = L.tile_stride; bs.n_tiles = pt.n_tiles; bs.tile = pt.tile;
       bs.n = (uint32_t)n_b; bs.shift = pt.shift; bs.n_bins = pt.n_bins; bs.cross_keys = L.cross_keys;
       bs.dst[0] = L.b.buf[0][0]; bs.dst[1] = L.b.buf[1][0];
       bs.q_sorted[0] = q_end_sorted; bs.q_sorted[1] = q_start_sorted; bs.qb[0] = L.qb[0]; bs.qb[1] = L.qb[1];
       bs.n_q = (uint32_t)n_a;
+      // lanes per gathered segment: the power of two at or above the mean segment length
+      const double seg = (double)n_b / ((double)pt.n_tiles * (double)pt.n_bins);
+      bs.group_log2 = 0;
+      while (bs.group_log2 < 5 && (double)(1u << bs.group_log2) < seg) ++bs.group_log2;
+      if (g_opt.mc_gather_group >= 0) bs.group_log2 = (uint32_t)g_opt.mc_gather_group;
+      bs.group = 1u << bs.group_log2;
+      if (pt.n_tiles > (uint32_t)mct::kMaxTiles) fused_ok = false;
     }
   }
   if (!fused_ok) {
@@ -708,15 +749,18 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       pt.round = round_begin + k; pt.flag = L.round_flags + j; pt.cross_cnt = L.cross_cnt[par];
       {
         ProfScope prof(kClsPlaceScatter, st);
-        mct::place_tile_kernel<<<pt.n_tiles < kTileBlocks ? pt.n_tiles : kTileBlocks, mct::kPtThreads, mct::kPtSmem, st>>>(pt);
+        if (tile_variant == 0) launch_place_tile<mct::TileCfg2x512>(pt, st);
+        else if (tile_variant == 1) launch_place_tile<mct::TileCfg1x1024>(pt, st);
+        else launch_place_tile<mct::TileCfg1x1024L>(pt, st);
         BITS_LAUNCH_CHECK();
       }
       bs.cross_cnt = L.cross_cnt[par]; bs.cross_cnt_next = L.cross_cnt[par ^ 1]; bs.flag = pt.flag;
       bs.round_total = reinterpret_cast<unsigned long long*>(round_counts_out + k);
       {
-        const uint32_t blocks = 2u * (uint32_t)kSMs;
         ProfScope prof(kClsBucketSortSearch, st);
-        mct::bin_sort_search_kernel<<<pt.n_bins < blocks ? pt.n_bins : blocks, mct::kBsThreads, mct::kBsSmem, st>>>(bs);
+        if (variant == 0) launch_bin_sort<mct::BinCfgWide>(bs, st);
+        else if (variant == 1) launch_bin_sort<mct::BinCfgNarrow>(bs, st);
+        else launch_bin_sort<mct::BinCfgSmall>(bs, st);
         BITS_LAUNCH_CHECK();
       }
     }
@@ -930,6 +974,9 @@ int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
 int bits_set_option(const char* name, int64_t value) {
   if (!name) return BITS_ERR_NULL;
   if (!strcmp(name, "mc_fused")) { g_opt.mc_fused = value; return BITS_OK; }
+  if (!strcmp(name, "mc_tile_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_tile_variant = value; return BITS_OK; }
+  if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }
+  if (!strcmp(name, "mc_gather_group")) { if (value < -1 || value > 5) return BITS_ERR_FLAGS; g_opt.mc_gather_group = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }
   if (!strcmp(name, "place_fused_hist")) { g_opt.place_fused_hist = value; return BITS_OK; }

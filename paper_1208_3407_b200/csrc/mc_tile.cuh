@@ -32,22 +32,52 @@ namespace bits {
 namespace mct {
 
 constexpr int kMaxBins = 4096;
-constexpr int kPtThreads = 512;
-constexpr int kPtIpt = 16;                       // intervals per thread and tile (four groups of four consecutive ones)
-constexpr int kTile = kPtThreads * kPtIpt;       // 8192 intervals
-constexpr size_t kPtSmem = (size_t)kTile * sizeof(uint2) + (size_t)(kMaxBins + kMaxChromSmem) * sizeof(uint32_t) +
-                           (size_t)kLutSize * sizeof(uint16_t);
+// Shape of place_tile_kernel: threads per block, intervals per thread and tile (a multiple of 4),
+// resident blocks per SM.  A tile holds up to kTile intervals, staged as pairs in shared memory.
+template <int kThreads_, int kIpt_, int kBlocksPerSm_>
+struct TileCfg {
+  static constexpr int kThreads = kThreads_, kIpt = kIpt_, kBlocksPerSm = kBlocksPerSm_;
+  static constexpr int kTile = kThreads * kIpt;
+  static constexpr size_t kSmem = (size_t)kTile * sizeof(uint2) + (size_t)(kMaxBins + kMaxChromSmem) * sizeof(uint32_t) +
+                                  (size_t)kLutSize * sizeof(uint16_t);
+};
+using TileCfg2x512 = TileCfg<512, 16, 2>;        // 8192-interval tiles, two blocks per SM
+using TileCfg1x1024 = TileCfg<1024, 16, 1>;      // 16384-interval tiles, one block per SM
+using TileCfg1x1024L = TileCfg<1024, 24, 1>;     // 24576-interval tiles, one block per SM
+constexpr int kMaxTileAny = 24576;
 
-constexpr int kBsThreads = 512;
-constexpr int kBsKpt = 16;
-constexpr int kCap = kBsThreads * kBsKpt;        // 8192 keys per bin and array
-constexpr int kSubBits = 13;
-constexpr int kSub = 1 << kSubBits;              // sub-buckets per bin: 16-bit counters, two per word
 constexpr int kCrossCap = 512;                   // hand-over list entries per bin
-constexpr int kMaxShift = 21;                    // widest bin: 2^21 coordinates, i.e. sub-buckets of 2^8
-constexpr size_t kBsSmem = (size_t)(2 * kCap) * sizeof(uint32_t) + (size_t)(2 * (8 + kSub + 8)) * sizeof(uint16_t);
+constexpr int kMaxShift = 21;                    // widest bin: 2^21 coordinates
+constexpr int kMaxTiles = 3072;                  // segment table of the bin sort: one word per tile
+constexpr int kFront = 8;                        // halfwords in front of a cursor array (one uint4)
+
+// Shape of the per-bin sort (bin_sort_search_kernel): threads per block, keys per thread,
+// sub-bucket bits, resident blocks per SM.  kCap keys per bin and array; 2^kSubBits sub-buckets
+// with 16-bit cursors, two per word.
+template <int kThreads_, int kKpt_, int kSubBits_, int kBlocksPerSm_>
+struct BinCfg {
+  static constexpr int kThreads = kThreads_, kKpt = kKpt_, kSubBits = kSubBits_, kBlocksPerSm = kBlocksPerSm_;
+  static constexpr int kCap = kThreads * kKpt;
+  static constexpr int kSub = 1 << kSubBits;
+  static constexpr int kCurLen = kFront + kSub + 8;      // halfwords per cursor array, a whole number of uint4s
+  static constexpr size_t kSmemFixed = (size_t)(2 * kCap) * sizeof(uint32_t) + (size_t)(2 * kCurLen) * sizeof(uint16_t);
+  static size_t smem_bytes(uint32_t n_tiles) { return kSmemFixed + ((size_t)n_tiles + 8) * sizeof(uint32_t); }
+};
+using BinCfgWide = BinCfg<512, 16, 13, 2>;       // 8192 keys per bin, two blocks per SM
+using BinCfgNarrow = BinCfg<512, 8, 12, 3>;      // 4096 keys per bin, three blocks per SM
+using BinCfgSmall = BinCfg<256, 16, 12, 4>;      // 4096 keys per bin, four blocks of 256 threads per SM
 
 constexpr uint32_t kFlagBinTooBig = 1u, kFlagCrossFull = 4u;
+
+// Bulk asynchronous copy shared -> global (the TMA engine moves the bytes, no LDS / STG issued).
+// dst, src 16-byte aligned, bytes a multiple of 16.
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void bulk_store_smem_to_global(void* gdst, const void* ssrc, uint32_t bytes) {
+  const uint32_t s = (uint32_t)__cvta_generic_to_shared(ssrc);
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_group_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 struct PlaceTileArgs {
   const uint32_t* spans;     // dev uint32[n], padded to a multiple of 4 with zeros, 16-byte aligned
@@ -68,26 +98,28 @@ struct PlaceTileArgs {
   uint32_t* flag;            // round flag
 };
 
-__global__ void __launch_bounds__(kPtThreads, 2) place_tile_kernel(PlaceTileArgs a) {
-  constexpr int kPer = kMaxBins / kPtThreads;   // 8 bin counters per thread
+template <class C>
+__global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kernel(PlaceTileArgs a) {
+  constexpr int kPer = kMaxBins / C::kThreads;   // bin counters per thread (4 or 8)
+  static_assert(kPer % 4 == 0, "uint4 accesses");
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  uint2* s_stage = reinterpret_cast<uint2*>(smem_raw);                   // [kTile]
-  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_stage + kTile);        // [kMaxBins] counts, then bases
+  uint2* s_stage = reinterpret_cast<uint2*>(smem_raw);                   // [C::kTile]
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_stage + C::kTile);        // [kMaxBins] counts, then bases
   uint32_t* s_off = s_cnt + kMaxBins;                                    // [kMaxChromSmem]
   uint16_t* s_lut = reinterpret_cast<uint16_t*>(s_off + kMaxChromSmem);  // [kLutSize]
   __shared__ uint32_t s_w[32];
   const int tid = threadIdx.x;
-  for (int i = tid; i < kMaxBins; i += kPtThreads) s_cnt[i] = 0;
+  for (int i = tid; i < kMaxBins; i += C::kThreads) s_cnt[i] = 0;
   const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);        // barrier inside
   const uint32_t shift = a.shift;
+  bool stage_in_flight = false;   // thread 0: a bulk copy out of s_stage has been issued and not yet waited for
   for (uint32_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
     const uint32_t base = tile * a.tile;
     const uint32_t count = min(a.tile, a.n - base);
-    uint32_t st[kPtIpt], rp[kPtIpt / 2];
+    uint32_t st[C::kIpt];
 #pragma unroll
-    for (int g = 0; g < kPtIpt / 4; ++g) {
-      const uint32_t l0 = 4u * (tid + g * kPtThreads);                   // four consecutive intervals of the tile
-      rp[2 * g] = 0; rp[2 * g + 1] = 0;
+    for (int g = 0; g < C::kIpt / 4; ++g) {
+      const uint32_t l0 = 4u * (tid + g * C::kThreads);                   // four consecutive intervals of the tile
       if (l0 < count) {
         const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l0));
         const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
@@ -98,8 +130,7 @@ __global__ void __launch_bounds__(kPtThreads, 2) place_tile_kernel(PlaceTileArgs
           st[4 * g + j] = ss[j];
           if (l0 + j < count) {
             const uint32_t bin = ss[j] >> shift;
-            const uint32_t r = atomicAdd(&s_cnt[bin], 1u);
-            rp[2 * g + (j >> 1)] |= r << (16 * (j & 1));
+            atomicAdd(&s_cnt[bin], 1u);                                  // count only: the slot is taken in the staging pass
             const uint32_t e = ss[j] + dd[j], ebin = e >> shift;
             if (ebin != bin) {                                           // rare: the end lies in the next bin
               const uint32_t slot = atomicAdd(&a.cross_cnt[ebin], 1u);
@@ -113,17 +144,22 @@ __global__ void __launch_bounds__(kPtThreads, 2) place_tile_kernel(PlaceTileArgs
     __syncthreads();
     // exclusive scan of the bin counts -> bases (kept in s_cnt) and the transposed prefix row entries
     {
-      const uint4 v0 = reinterpret_cast<const uint4*>(s_cnt)[2 * tid], v1 = reinterpret_cast<const uint4*>(s_cnt)[2 * tid + 1];
-      const uint32_t c[kPer] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+      uint32_t c[kPer];
+#pragma unroll
+      for (int j = 0; j < kPer / 4; ++j) {
+        const uint4 v = reinterpret_cast<const uint4*>(s_cnt)[(kPer / 4) * tid + j];
+        c[4 * j] = v.x; c[4 * j + 1] = v.y; c[4 * j + 2] = v.z; c[4 * j + 3] = v.w;
+      }
       uint32_t sum = 0;
 #pragma unroll
       for (int j = 0; j < kPer; ++j) sum += c[j];
-      uint32_t run = msd::block_excl_scan<kPtThreads>(sum, s_w);
+      uint32_t run = msd::block_excl_scan<C::kThreads>(sum, s_w);
       uint32_t lb[kPer];
 #pragma unroll
       for (int j = 0; j < kPer; ++j) { lb[j] = run; run += c[j]; }
-      reinterpret_cast<uint4*>(s_cnt)[2 * tid] = make_uint4(lb[0], lb[1], lb[2], lb[3]);
-      reinterpret_cast<uint4*>(s_cnt)[2 * tid + 1] = make_uint4(lb[4], lb[5], lb[6], lb[7]);
+#pragma unroll
+      for (int j = 0; j < kPer / 4; ++j)
+        reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + j] = make_uint4(lb[4 * j], lb[4 * j + 1], lb[4 * j + 2], lb[4 * j + 3]);
       const uint32_t b0 = (uint32_t)tid * kPer;
       if (b0 <= a.n_bins) {
         uint16_t* o = a.off + (size_t)b0 * a.stride + tile;
@@ -132,11 +168,12 @@ __global__ void __launch_bounds__(kPtThreads, 2) place_tile_kernel(PlaceTileArgs
           if (b0 + j <= a.n_bins) o[(size_t)j * a.stride] = (uint16_t)lb[j];
       }
     }
+    if (tid == 0 && stage_in_flight) { bulk_wait_group_read0(); stage_in_flight = false; }   // the previous tile has left s_stage
     __syncthreads();
-    // stage the pairs in bin order (spans re-read: L1 hits)
+    // stage the pairs in bin order: every bin's base doubles as its cursor (spans re-read: cache hits)
 #pragma unroll
-    for (int g = 0; g < kPtIpt / 4; ++g) {
-      const uint32_t l0 = 4u * (tid + g * kPtThreads);
+    for (int g = 0; g < C::kIpt / 4; ++g) {
+      const uint32_t l0 = 4u * (tid + g * C::kThreads);
       if (l0 < count) {
         const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l0));
         const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
@@ -144,26 +181,27 @@ __global__ void __launch_bounds__(kPtThreads, 2) place_tile_kernel(PlaceTileArgs
         for (int j = 0; j < 4; ++j)
           if (l0 + j < count) {
             const uint32_t s = st[4 * g + j];
-            const uint32_t r = (rp[2 * g + (j >> 1)] >> (16 * (j & 1))) & 0xffffu;
-            s_stage[s_cnt[s >> shift] + r] = make_uint2(s, s + dd[j]);
+            s_stage[atomicAdd(&s_cnt[s >> shift], 1u)] = make_uint2(s, s + dd[j]);
           }
       }
     }
+    fence_proxy_async_smem();   // the staged pairs are about to be read by the bulk-copy engine
     __syncthreads();
-    reinterpret_cast<uint4*>(s_cnt)[2 * tid] = make_uint4(0, 0, 0, 0);
-    reinterpret_cast<uint4*>(s_cnt)[2 * tid + 1] = make_uint4(0, 0, 0, 0);
-    {
-      uint2* __restrict__ dst = a.pairs + base;                          // base % 4 == 0: 32-byte aligned
-      const uint32_t c2 = count >> 1;
 #pragma unroll
-      for (int j = 0; j < kPtIpt / 2; ++j) {
-        const uint32_t i = tid + j * kPtThreads;
-        if (i < c2) reinterpret_cast<uint4*>(dst)[i] = reinterpret_cast<const uint4*>(s_stage)[i];
-      }
-      if ((count & 1u) && tid == 0) dst[count - 1] = s_stage[count - 1];
+    for (int j = 0; j < kPer / 4; ++j) reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + j] = make_uint4(0, 0, 0, 0);
+    if (tid == 0) {
+      // one bulk copy per 32 KB, shared -> global, no LDS / STG: the next tile's placement overlaps it
+      uint2* dst = a.pairs + base;                                       // base % 4 == 0: 32-byte aligned
+      const uint32_t bytes = (count & ~1u) * (uint32_t)sizeof(uint2);    // a multiple of 16
+      for (uint32_t o = 0; o < bytes; o += 32768u)
+        bulk_store_smem_to_global(reinterpret_cast<char*>(dst) + o, reinterpret_cast<const char*>(s_stage) + o, min(32768u, bytes - o));
+      bulk_commit_group();
+      if (count & 1u) dst[count - 1] = s_stage[count - 1];
+      stage_in_flight = true;
     }
-    __syncthreads();   // s_stage and s_cnt are free again
+    __syncthreads();   // s_cnt is clear again; s_stage is free once thread 0 has waited for the bulk copies
   }
+  if (tid == 0 && stage_in_flight) bulk_wait_group_read0();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -183,6 +221,7 @@ struct BinSortArgs {
   const uint32_t* q_sorted[2];          // ascending: A's ends (ranked in B_S, "<="), A's starts (ranked in B_E, "<")
   const uint32_t* qb[2];                // [n_bins + 1]: queries qb[d] .. qb[d+1]-1 fall into bin d's key range
   uint32_t n_q;
+  uint32_t group, group_log2;           // lanes that gather one (tile, bin) segment together: a power of two, 1..32
   unsigned long long* round_total;      // += sum of ranks in B_S - sum of ranks in B_E
   uint32_t* flag;
 };
@@ -190,8 +229,6 @@ struct BinSortArgs {
 // Counter arrays of one bin: uint16 cursors, two per word.  Entry kFront + sb belongs to
 // sub-bucket sb; entry kFront - 1 stays 0, so after the scatter (which leaves every cursor at
 // the END of its sub-bucket) the keys of sub-bucket sb sit at [cur[kFront + sb - 1], cur[kFront + sb]).
-constexpr int kFront = 8;                        // halfwords in front of the cursors (one uint4)
-constexpr int kCurLen = kFront + kSub + 8;       // halfwords per cursor array, a whole number of uint4s
 
 __device__ __forceinline__ uint32_t sub_of(uint32_t key, uint32_t mask, uint32_t sshift) { return (key & mask) >> sshift; }
 
@@ -208,8 +245,9 @@ __device__ __forceinline__ uint32_t take_slot(uint32_t* cur32, uint32_t sb) {
 
 // Counts -> exclusive prefixes, in place, for both cursor arrays (starts, ends) with one pair of
 // barriers.  total[0], total[1] = keys counted per array.  s_w: 64 words of scratch.
+template <class C>
 __device__ __forceinline__ void scan_cursors(uint16_t* cur_s, uint16_t* cur_e, uint32_t* s_w, uint32_t total[2]) {
-  constexpr int kWords = kSub / 2 / kBsThreads;   // cursor words per thread and array
+  constexpr int kWords = C::kSub / 2 / C::kThreads;   // cursor words per thread and array
   static_assert(kWords % 4 == 0, "uint4 accesses");
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   uint32_t c[2][kWords], sum[2] = {0, 0};
@@ -224,14 +262,14 @@ __device__ __forceinline__ void scan_cursors(uint16_t* cur_s, uint16_t* cur_e, u
 #pragma unroll
     for (int j = 0; j < kWords; ++j) sum[a] += (c[a][j] & 0xffffu) + (c[a][j] >> 16);
   }
-  // both sums travel through one scan: starts in the low half, ends in the high half (each <= kCap)
+  // both sums travel through one scan: starts in the low half, ends in the high half (each <= C::kCap)
   uint32_t incl = sum[0] | (sum[1] << 16);
   const uint32_t own = incl;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, incl, o); if (lane >= o) incl += t; }
   if (lane == 31) s_w[w] = incl;
   __syncthreads();
-  uint32_t x = lane < kBsThreads / 32 ? s_w[lane] : 0u;
+  uint32_t x = lane < C::kThreads / 32 ? s_w[lane] : 0u;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, x, o); if (lane >= o) x += t; }
   const uint32_t before = w ? __shfl_sync(kFullMask, x, (w + 31) & 31) : 0u;
@@ -258,23 +296,23 @@ __device__ __forceinline__ void scan_cursors(uint16_t* cur_s, uint16_t* cur_e, u
 // barrier) stored at the slot its sub-bucket's cursor hands out.  With kCheckBin, entries whose
 // bin is not d are dropped.  Ends with a barrier; afterwards buf[0..valid) is ordered by
 // sub-bucket and cur[kFront + sb] is the END of sub-bucket sb.
-template <bool kCheckBin>
+template <class C, bool kCheckBin>
 __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint32_t mask,
                                                  uint32_t sshift, uint16_t* cur) {
   const int tid = threadIdx.x;
   uint32_t* cur32 = reinterpret_cast<uint32_t*>(cur);
-  uint32_t key[kBsKpt];
+  uint32_t key[C::kKpt];
 #pragma unroll
-  for (int j = 0; j < kBsKpt; ++j) {
-    const uint32_t i = tid + j * kBsThreads;
+  for (int j = 0; j < C::kKpt; ++j) {
+    const uint32_t i = tid + j * C::kThreads;
     key[j] = i < m ? buf[i] : 0u;
   }
   __syncthreads();
 #pragma unroll
-  for (int j = 0; j < kBsKpt; ++j) {
-    if ((uint32_t)(j * kBsThreads) >= m) break;
+  for (int j = 0; j < C::kKpt; ++j) {
+    if ((uint32_t)(j * C::kThreads) >= m) break;
     const uint32_t k = key[j];
-    if (tid + j * kBsThreads < m && (!kCheckBin || (k >> shift) == d)) buf[take_slot(cur32, sub_of(k, mask, sshift))] = k;
+    if (tid + j * C::kThreads < m && (!kCheckBin || (k >> shift) == d)) buf[take_slot(cur32, sub_of(k, mask, sshift))] = k;
   }
   __syncthreads();
 }
@@ -284,12 +322,12 @@ __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint
 // candidates without a loop.  Then rank the sorted queries q_sorted[qlo..qhi), all of which fall
 // into this bin's key range: every key of an earlier sub-bucket is smaller, the count is finished
 // inside the query's own sub-bucket.  Returns this thread's sum of query ranks.
-template <bool kStrict>
+template <class C, bool kStrict>
 __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t mv, uint32_t mask, uint32_t sshift,
                                                    const uint16_t* cur, uint32_t gbase, uint32_t* __restrict__ dst,
                                                    const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi) {
   const int tid = threadIdx.x;
-  for (uint32_t p = tid; p < mv; p += kBsThreads) {
+  for (uint32_t p = tid; p < mv; p += C::kThreads) {
     const uint32_t k = buf[p];
     const uint32_t sb = sub_of(k, mask, sshift);
     const uint32_t lo = cur[kFront - 1 + sb], hi = cur[kFront + sb];
@@ -297,7 +335,7 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
 #pragma unroll
     for (uint32_t i = 0; i < 4; ++i) {
       const uint32_t t = lo + i;
-      const uint32_t kk = buf[t];                    // buf is padded: t < kCap + 4
+      const uint32_t kk = buf[t];                    // buf is padded: t < C::kCap + 4
       rank += (t < hi) & (kk < k + (t < p ? 1u : 0u));
     }
     if (hi - lo > 4) {
@@ -307,7 +345,7 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
     dst[gbase + lo + rank] = k;
   }
   uint64_t qsum = 0;
-  for (uint32_t qi = qlo + tid; qi < qhi; qi += kBsThreads) {
+  for (uint32_t qi = qlo + tid; qi < qhi; qi += C::kThreads) {
     const uint32_t q = __ldg(q_sorted + qi);
     const uint32_t sb = sub_of(q, mask, sshift);
     const uint32_t lo = cur[kFront - 1 + sb], hi = cur[kFront + sb];
@@ -319,18 +357,22 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
   return qsum;
 }
 
-__global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortArgs a) {
+template <class C>
+__global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_kernel(BinSortArgs a) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  uint32_t* s_ks = reinterpret_cast<uint32_t*>(smem_raw);          // [kCap] starts
-  uint32_t* s_ke = s_ks + kCap;                                    // [kCap] ends (own + handed over)
-  uint16_t* s_cur_s = reinterpret_cast<uint16_t*>(s_ke + kCap);    // [kCurLen] cursors of the starts
-  uint16_t* s_cur_e = s_cur_s + kCurLen;                           // [kCurLen] cursors of the ends
+  uint32_t* s_ks = reinterpret_cast<uint32_t*>(smem_raw);          // [C::kCap] starts
+  uint32_t* s_ke = s_ks + C::kCap;                                    // [C::kCap] ends (own + handed over)
+  uint16_t* s_cur_s = reinterpret_cast<uint16_t*>(s_ke + C::kCap);    // [C::kCurLen] cursors of the starts
+  uint16_t* s_cur_e = s_cur_s + C::kCurLen;                           // [C::kCurLen] cursors of the ends
   __shared__ uint32_t s_w[32], s_w2[32];
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const uint32_t shift = a.shift, mask = (1u << shift) - 1u;
-  const uint32_t sshift = shift > (uint32_t)kSubBits ? shift - kSubBits : 0u;
-  const uint32_t runs = (a.n_tiles + kBsThreads - 1) / kBsThreads;    // tiles per thread (contiguous)
+  const uint32_t sshift = shift > (uint32_t)C::kSubBits ? shift - C::kSubBits : 0u;
+  uint32_t* s_seg = reinterpret_cast<uint32_t*>(s_cur_e + C::kCurLen);   // [n_tiles + 1] per tile: lo | pos << 16
+  const uint32_t runs = (a.n_tiles + C::kThreads - 1) / C::kThreads;    // tiles per thread (contiguous)
   const uint32_t t0 = min(a.n_tiles, (uint32_t)tid * runs), t1 = min(a.n_tiles, t0 + runs);
+  const uint32_t gl = (uint32_t)tid & (a.group - 1u), gid = (uint32_t)tid >> a.group_log2;   // gather groups of a.group lanes
+  const uint32_t n_groups = (uint32_t)C::kThreads >> a.group_log2;
   uint64_t qsum = 0;    // two's-complement: + ranks in B_S, - ranks in B_E
   for (uint32_t d = blockIdx.x; d < a.n_bins; d += gridDim.x) {
     a.cross_cnt_next[d] = 0;   // (every thread writes the same zero: harmless, and no divergence)
@@ -343,13 +385,13 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, incl, o); if (lane >= o) incl += t; }
     ls = __reduce_add_sync(kFullMask, ls);
-    __syncthreads();           // everyone is done with the previous bin's buffers, cursors and s_w / s_w2
+    __syncthreads();           // everyone is done with the previous bin's buffers, cursors, s_seg and s_w / s_w2
     if (lane == 31) { s_w[w] = incl; s_w2[w] = ls; }
     // clear both cursor arrays (they are adjacent)
-    for (int i = tid; i < 2 * kCurLen / 8; i += kBsThreads) reinterpret_cast<uint4*>(s_cur_s)[i] = make_uint4(0, 0, 0, 0);
+    for (int i = tid; i < 2 * C::kCurLen / 8; i += C::kThreads) reinterpret_cast<uint4*>(s_cur_s)[i] = make_uint4(0, 0, 0, 0);
     __syncthreads();
-    uint32_t x = lane < kBsThreads / 32 ? s_w[lane] : 0u;
-    const uint32_t gbase = __reduce_add_sync(kFullMask, lane < kBsThreads / 32 ? s_w2[lane] : 0u);
+    uint32_t x = lane < C::kThreads / 32 ? s_w[lane] : 0u;
+    const uint32_t gbase = __reduce_add_sync(kFullMask, lane < C::kThreads / 32 ? s_w2[lane] : 0u);
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, x, o); if (lane >= o) x += t; }
     const uint32_t np = __shfl_sync(kFullMask, x, 31);                  // pairs in this bin
@@ -357,17 +399,26 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
     const uint32_t n_in = min(__ldg(a.cross_cnt + d), (uint32_t)kCrossCap);
     const uint32_t qlo0 = __ldg(a.qb[0] + d), qhi0 = __ldg(a.qb[0] + d + 1);
     const uint32_t qlo1 = __ldg(a.qb[1] + d), qhi1 = __ldg(a.qb[1] + d + 1);
-    if (np + n_in > (uint32_t)kCap) {                                   // block-uniform
+    if (np + n_in > (uint32_t)C::kCap) {                                   // block-uniform
       if (tid == 0) atomicOr(a.flag, kFlagBinTooBig);
       continue;
     }
-    // gather the bin's pairs from every tile; starts and ends go to separate arrays
+    // where each tile's segment of this bin sits in the tile (lo) and goes in the bin's buffers (pos)
     for (uint32_t t = t0; t < t1; ++t) {
       const uint32_t lo = __ldg(row0 + t), hi = __ldg(row1 + t);
-      const uint2* src = a.pairs + (size_t)t * a.tile + lo;
-      for (uint32_t j = 0; j < hi - lo; ++j, ++pos) {
-        msd::cp_async4(s_ks + pos, &src[j].x);
-        msd::cp_async4(s_ke + pos, &src[j].y);
+      s_seg[t] = lo | (pos << 16);
+      pos += hi - lo;
+    }
+    if (tid == 0) s_seg[a.n_tiles] = np << 16;
+    __syncthreads();
+    // gather: a group of lanes per segment, so that one instruction touches few cache lines
+    // (a scattered access costs the L1 one cycle per line); starts and ends go to separate arrays
+    for (uint32_t t = gid; t < a.n_tiles; t += n_groups) {
+      const uint32_t seg = s_seg[t], p0 = seg >> 16, len = (s_seg[t + 1] >> 16) - p0;
+      const uint2* src = a.pairs + (size_t)t * a.tile + (seg & 0xffffu);
+      for (uint32_t j = gl; j < len; j += a.group) {
+        msd::cp_async4(s_ks + p0 + j, &src[j].x);
+        msd::cp_async4(s_ke + p0 + j, &src[j].y);
       }
     }
     if ((uint32_t)tid < n_in) msd::cp_async4(s_ke + np + tid, a.cross_keys + (size_t)d * kCrossCap + tid);
@@ -378,7 +429,7 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
     {
       uint32_t* cs = reinterpret_cast<uint32_t*>(s_cur_s);
       uint32_t* ce = reinterpret_cast<uint32_t*>(s_cur_e);
-      for (uint32_t i = tid; i < me; i += kBsThreads) {
+      for (uint32_t i = tid; i < me; i += C::kThreads) {
         if (i < np) count_key(cs, sub_of(s_ks[i], mask, sshift));
         const uint32_t e = s_ke[i];
         if ((e >> shift) == d) count_key(ce, sub_of(e, mask, sshift));
@@ -386,26 +437,26 @@ __global__ void __launch_bounds__(kBsThreads, 2) bin_sort_search_kernel(BinSortA
     }
     __syncthreads();
     uint32_t total[2];
-    scan_cursors(s_cur_s, s_cur_e, s_w, total);                         // barriers inside
+    scan_cursors<C>(s_cur_s, s_cur_e, s_w, total);                         // barriers inside
     // starts: all np keys belong to bin d; the bin begins at gbase in B_S
-    scatter_in_place<false>(s_ks, np, d, shift, mask, sshift, s_cur_s);
-    qsum += write_and_rank<false>(s_ks, np, mask, sshift, s_cur_s, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0);
+    scatter_in_place<C, false>(s_ks, np, d, shift, mask, sshift, s_cur_s);
+    qsum += write_and_rank<C, false>(s_ks, np, mask, sshift, s_cur_s, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0);
     // ends: n_in ends of earlier pairs lie in this bin, so it begins at gbase - n_in in B_E
-    scatter_in_place<true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
-    qsum -= write_and_rank<true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
+    scatter_in_place<C, true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
+    qsum -= write_and_rank<C, true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
   }
   if (blockIdx.x == 0 && tid == 0) {
     // queries beyond the last bin count every key
     qsum += (uint64_t)(a.n_q - __ldg(a.qb[0] + a.n_bins)) * a.n;
     qsum -= (uint64_t)(a.n_q - __ldg(a.qb[1] + a.n_bins)) * a.n;
   }
-  __shared__ uint64_t s_red[kBsThreads / 32];
+  __shared__ uint64_t s_red[C::kThreads / 32];
   __syncthreads();
   qsum = warp_sum_u64(qsum);
   if (lane == 0) s_red[w] = qsum;
   __syncthreads();
   if (w == 0) {
-    uint64_t t = lane < kBsThreads / 32 ? s_red[lane] : 0;
+    uint64_t t = lane < C::kThreads / 32 ? s_red[lane] : 0;
     t = warp_sum_u64(t);
     if (lane == 0 && t != 0) atomicAdd(a.round_total, (unsigned long long)t);
   }

@@ -88,8 +88,14 @@ __device__ __forceinline__ uint32_t place_start(uint32_t xl, uint32_t xh, uint32
     if (cv.lut) {
       // the thresholds off[c] - c*d only move down as d grows, so the chromosome of u for d = 0
       // (read from the table at the start of u's block) is a lower bound: step up from there
+      // (two steps without a loop -- almost always enough -- then the general loop)
       c = cv.lut[u >> t.lut_shift];
-      while (c + 1 < t.n_chrom && off[c + 1] - (c + 1) * d <= u) ++c;
+      const uint32_t o1 = off[c + 1], o2 = off[c + 2];                 // staged table: >= n_chrom + 2 words
+      const bool s1 = c + 1 < t.n_chrom && o1 - (c + 1) * d <= u;
+      const bool s2 = s1 && c + 2 < t.n_chrom && o2 - (c + 2) * d <= u;
+      c += (uint32_t)s1 + (uint32_t)s2;
+      if (s2)
+        while (c + 1 < t.n_chrom && off[c + 1] - (c + 1) * d <= u) ++c;
     } else {
       for (uint32_t s = t.step0; s > 0; s >>= 1) {
         const uint32_t m = c + s;
@@ -118,7 +124,7 @@ __device__ __forceinline__ uint32_t place_start(uint32_t xl, uint32_t xh, uint32
 // Stage the offset table (and the look-up table, s_lut = kLutSize entries) in shared memory when
 // it fits; returns the view to search through.  Ends with __syncthreads().
 __device__ __forceinline__ ChromView stage_chrom_table(const ChromTable& t, uint32_t* s_off, uint16_t* s_lut) {
-  const bool fits = t.n_chrom + 1 <= (uint32_t)kMaxChromSmem;
+  const bool fits = t.n_chrom + 2 <= (uint32_t)kMaxChromSmem;
   const bool with_lut = fits && t.lut != nullptr && s_lut != nullptr;
   if (fits)
     for (uint32_t i = threadIdx.x; i <= t.n_chrom; i += blockDim.x) s_off[i] = t.off[i];
