@@ -35,7 +35,11 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
-NCU_TRAFFIC_BYTES: dict = {}
+NCU_TRAFFIC_BYTES: dict = {
+    # profiles/r1b_fused_ncu_full_summary.txt (config 5, one launch)
+    "bin_sort_search_kernel": 127_712_768,     # 89.93 MB read + 37.79 MB written
+    "place_tile_kernel": 70_995_200,           # 40.76 MB read + 30.24 MB written
+}
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
@@ -219,13 +223,14 @@ def secondary_workloads(device, peak_gbs):
     bits.set_option("profile", 2); bits.set_option("profile", 1)
     med, mn = time_device(lambda: bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total), 10)
     prof = bits.profile_read(); bits.set_option("profile", 0)
-    ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in prof.items()}
-    sort_ms = ms["histogram"] + 4 * ms["sort_pass"]
+    calls = 13                                    # 3 warm-ups + 10 timed repeats, all with events on
+    ms = {k: v[0] / calls for k, v in prof.items()}     # device ms per call and kernel class
+    sort_ms = ms["histogram"] + ms["plan"] + ms["scatter"] + ms["bucket_sort"]   # MSD bucket sort of B's starts and ends
     out["cfg4_large_count_10M"] = {
         "intervals_searched_per_s": w.n_a / (med * 1e-3), "ms_median": med, "ms_min": mn,
         "sort_keys_per_s": 2 * w.n_b / (sort_ms * 1e-3) if sort_ms else None,
-        "kernel_ms": {"histogram": ms["histogram"], "sort_pass": ms["sort_pass"], "index_build": ms["index_build"],
-                      "count": ms["count"]},
+        "kernel_ms": {"histogram": ms["histogram"], "plan": ms["plan"], "scatter": ms["scatter"], "bucket_sort": ms["bucket_sort"],
+                      "lsd_fallback_pass": ms["sort_pass"], "index_build": ms["index_build"], "count": ms["count"]},
         "hbm_bytes_model": 72 * w.n_b + 12 * w.n_a + 8 * w.n_b,
         "hbm_frac_of_peak": (72 * w.n_b + 12 * w.n_a + 8 * w.n_b) / (med * 1e-3) / 1e9 / peak_gbs,
     }
@@ -293,9 +298,7 @@ def run_b200(args):
     for _ in range(max(args.warmup, 0)):
         step()
     barrier()
-    profile_events = not args.no_profile_events
-    bits.set_option("profile", 2)
-    bits.set_option("profile", 1 if profile_events else 0)
+    bits.set_option("profile", 0)                 # no per-kernel events inside the timed region
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -309,6 +312,16 @@ def run_b200(args):
     barrier()
     elapsed_ms = ev0.elapsed_time(ev1)
     launches = bits.launch_count() - launches0
+    # per-kernel durations: the same step repeated right behind the timed region (clocks still sampled),
+    # every launch bracketed by CUDA events on the launching stream (they cost ~5 % of throughput,
+    # which is why they stay out of `value`)
+    profile_events = not args.no_profile_events
+    prof_steps = min(args.steps, 2) if profile_events else 0
+    bits.set_option("profile", 2)
+    bits.set_option("profile", 1 if profile_events else 0)
+    for _ in range(prof_steps):
+        step()
+    barrier()
     clocks = sampler.stop() if rank == 0 else None
     prof = bits.profile_read()
     bits.set_option("profile", 0)
@@ -348,7 +361,8 @@ def run_b200(args):
                         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(kname), "peak_source": peak_src,
                         "avg_launch_ms": launch_ms, "launches_timed": timed[dom][1],
                         "algorithmic_bytes_per_launch": alg_bytes,
-                        "kernel_ms_per_round": {k: v[0] / (R * args.steps) for k, v in timed.items()},
+                        "kernel_ms_per_round": {k: v[0] / (R * prof_steps) for k, v in timed.items()},
+                        "timed_in": f"{prof_steps} extra step(s) right behind the timed region, one event pair per launch",
                         "kernel_share_of_step": {k: v[0] / tot for k, v in timed.items()}}
             if n_sorted:
                 # SURVEY 8(d) per-round model: place 12 M + sort 72 M (histogram fused: - 8 M) + search 8 N_q
@@ -367,7 +381,7 @@ def run_b200(args):
         "config": config_block(w, R, world), "gpu_launches": launches,
         "intervals_searched_per_s": value * w.n_a,
         "sort_keys_per_s": (2 * n_sorted * value) if n_sorted else None,
-        "profile_events_in_timed_region": profile_events,
+        "profile_events_in_timed_region": False,
     }
     if roofline:
         line["roofline"] = roofline

@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
           st[4 * g + j] = ss[j];
           if (l0 + j < count) {
             const uint32_t bin = ss[j] >> shift;
-            atomicAdd(&s_cnt[bin], 1u);                                  // count only: the slot is taken in the staging pass
+            atomicAdd(&s_cnt[bin], 1u);                             // count only: the slot is taken in the staging pass
             const uint32_t e = ss[j] + dd[j], ebin = e >> shift;
             if (ebin != bin) {                                           // rare: the end lies in the next bin
               const uint32_t slot = atomicAdd(&a.cross_cnt[ebin], 1u);
@@ -171,20 +171,29 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
     if (tid == 0 && stage_in_flight) { bulk_wait_group_read0(); stage_in_flight = false; }   // the previous tile has left s_stage
     __syncthreads();
     // stage the pairs in bin order: every bin's base doubles as its cursor (spans re-read: cache hits)
+    // (the four slots of a group are taken first and filled afterwards, so the atomics overlap)
+    {
+      uint4 d4 = make_uint4(0, 0, 0, 0);
+      if (4u * tid < count) d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + 4u * tid));
 #pragma unroll
-    for (int g = 0; g < C::kIpt / 4; ++g) {
-      const uint32_t l0 = 4u * (tid + g * C::kThreads);
-      if (l0 < count) {
-        const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l0));
+      for (int g = 0; g < C::kIpt / 4; ++g) {
+        const uint32_t l0 = 4u * (tid + g * C::kThreads);
         const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
+        if (g + 1 < C::kIpt / 4) {                                       // the next group's spans are on their way
+          const uint32_t l1 = l0 + 4u * C::kThreads;
+          if (l1 < count) d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l1));
+        }
+        if (l0 < count) {
+          uint32_t slot[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-          if (l0 + j < count) {
-            const uint32_t s = st[4 * g + j];
-            s_stage[atomicAdd(&s_cnt[s >> shift], 1u)] = make_uint2(s, s + dd[j]);
-          }
+          for (int j = 0; j < 4; ++j) slot[j] = l0 + j < count ? atomicAdd(&s_cnt[st[4 * g + j] >> shift], 1u) : 0xffffffffu;
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (slot[j] != 0xffffffffu) s_stage[slot[j]] = make_uint2(st[4 * g + j], st[4 * g + j] + dd[j]);
+        }
       }
     }
+    __syncthreads();
     fence_proxy_async_smem();   // the staged pairs are about to be read by the bulk-copy engine
     __syncthreads();
 #pragma unroll
@@ -309,10 +318,18 @@ __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint
   }
   __syncthreads();
 #pragma unroll
-  for (int j = 0; j < C::kKpt; ++j) {
-    if ((uint32_t)(j * C::kThreads) >= m) break;
-    const uint32_t k = key[j];
-    if (tid + j * C::kThreads < m && (!kCheckBin || (k >> shift) == d)) buf[take_slot(cur32, sub_of(k, mask, sshift))] = k;
+  for (int j0 = 0; j0 < C::kKpt; j0 += 4) {           // four slots are taken, then filled: the atomics overlap
+    if ((uint32_t)(j0 * C::kThreads) >= m) break;
+    uint32_t slot[4];
+#pragma unroll
+    for (int j = j0; j < j0 + 4; ++j) {
+      const uint32_t k = key[j];
+      const bool ok = tid + j * C::kThreads < m && (!kCheckBin || (k >> shift) == d);
+      slot[j - j0] = ok ? take_slot(cur32, sub_of(k, mask, sshift)) : 0xffffffffu;
+    }
+#pragma unroll
+    for (int j = j0; j < j0 + 4; ++j)
+      if (slot[j - j0] != 0xffffffffu) buf[slot[j - j0]] = key[j];
   }
   __syncthreads();
 }
@@ -374,7 +391,14 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
   const uint32_t gl = (uint32_t)tid & (a.group - 1u), gid = (uint32_t)tid >> a.group_log2;   // gather groups of a.group lanes
   const uint32_t n_groups = (uint32_t)C::kThreads >> a.group_log2;
   uint64_t qsum = 0;    // two's-complement: + ranks in B_S, - ranks in B_E
-  for (uint32_t d = blockIdx.x; d < a.n_bins; d += gridDim.x) {
+  // bins are handed out dynamically: the first one is the block's index, the rest come from a ticket
+  // counter (spare word kMaxBins + 1 of this round's hand-over counts; zero on entry, reset for the
+  // round after next by block 0 through the other parity's array)
+  __shared__ uint32_t s_next;
+  if (blockIdx.x == 0 && tid == 0) a.cross_cnt_next[kMaxBins + 1] = 0;
+  uint32_t d = blockIdx.x;
+  while (d < a.n_bins) {
+    if (tid == 0) s_next = gridDim.x + atomicAdd(const_cast<uint32_t*>(a.cross_cnt) + kMaxBins + 1, 1u);
     a.cross_cnt_next[d] = 0;   // (every thread writes the same zero: harmless, and no divergence)
     const uint16_t* __restrict__ row0 = a.off + (size_t)d * a.stride;
     const uint16_t* __restrict__ row1 = row0 + a.stride;
@@ -396,11 +420,13 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(kFullMask, x, o); if (lane >= o) x += t; }
     const uint32_t np = __shfl_sync(kFullMask, x, 31);                  // pairs in this bin
     uint32_t pos = incl - len_sum + (w ? __shfl_sync(kFullMask, x, (w + 31) & 31) : 0u);
+    const uint32_t d_next = s_next;
     const uint32_t n_in = min(__ldg(a.cross_cnt + d), (uint32_t)kCrossCap);
     const uint32_t qlo0 = __ldg(a.qb[0] + d), qhi0 = __ldg(a.qb[0] + d + 1);
     const uint32_t qlo1 = __ldg(a.qb[1] + d), qhi1 = __ldg(a.qb[1] + d + 1);
     if (np + n_in > (uint32_t)C::kCap) {                                   // block-uniform
       if (tid == 0) atomicOr(a.flag, kFlagBinTooBig);
+      d = d_next;
       continue;
     }
     // where each tile's segment of this bin sits in the tile (lo) and goes in the bin's buffers (pos)
@@ -444,6 +470,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     // ends: n_in ends of earlier pairs lie in this bin, so it begins at gbase - n_in in B_E
     scatter_in_place<C, true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
     qsum -= write_and_rank<C, true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
+    d = d_next;
   }
   if (blockIdx.x == 0 && tid == 0) {
     // queries beyond the last bin count every key
