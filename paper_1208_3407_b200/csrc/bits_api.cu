@@ -23,6 +23,7 @@ struct Options {
   int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+tile sort / bin sort+search (mc_tile.cuh)
   int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
   int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
+  int64_t mc_force_redo = 0;       // PERMUTE_B fused rounds: n > 0 redoes every n-th round by the general path as if its flag were raised (tests)
   int64_t mc_tile_variant = 2;     // PERMUTE_B fused rounds: shape of place_tile_kernel (0: 2 x 512 threads, 1: 1 x 1024, 2: 1 x 1024 with longer tiles)
   int64_t mc_bin_variant = 0;      // PERMUTE_B fused rounds: shape of the per-bin sort (0 wide, 1 narrow, 2 small blocks)
   int64_t mc_gather_group = -1;    // PERMUTE_B fused rounds: log2 of the lanes per gathered segment (-1 = from the mean segment length)
@@ -769,7 +770,8 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     BITS_CUDA_TRY(cudaMemcpyAsync(h_flags.data(), L.round_flags, sizeof(uint32_t) * chunk, cudaMemcpyDeviceToHost, st));
     BITS_CUDA_TRY(cudaStreamSynchronize(st));
     for (uint32_t j = 0; j < chunk; ++j) {
-      if (!h_flags[j]) continue;
+      const bool forced = g_opt.mc_force_redo > 0 && (done + j) % (uint32_t)g_opt.mc_force_redo == 0;
+      if (!h_flags[j] && !forced) continue;
       BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out + done + j, 0, sizeof(uint64_t), st));
       BITS_TRY(general_round(done + j));
     }
@@ -974,6 +976,7 @@ int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
 int bits_set_option(const char* name, int64_t value) {
   if (!name) return BITS_ERR_NULL;
   if (!strcmp(name, "mc_fused")) { g_opt.mc_fused = value; return BITS_OK; }
+  if (!strcmp(name, "mc_force_redo")) { if (value < 0) return BITS_ERR_FLAGS; g_opt.mc_force_redo = value; return BITS_OK; }
   if (!strcmp(name, "mc_tile_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_tile_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_gather_group")) { if (value < -1 || value > 5) return BITS_ERR_FLAGS; g_opt.mc_gather_group = value; return BITS_OK; }

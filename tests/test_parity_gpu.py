@@ -312,6 +312,82 @@ def test_mc_config5_full_size_sampled_rounds():
     assert np.array_equal(rc2, rc[:3])
 
 
+def _mc_b_case(a_s, a_e, b_s, b_e, off, seed, r0, n, expect_fused=None):
+    bits.set_option("profile", 2)
+    bits.set_option("profile", 1)
+    try:
+        obs, rc = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, 1, seed, r0, n)
+        sync()
+        fused_launches = bits.profile_read()["place_scatter"][1]
+    finally:
+        bits.set_option("profile", 0)
+    if expect_fused is not None:                              # which path ran: the two fused launches per round, or the general one
+        assert fused_launches == (n if expect_fused else 0)
+    o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, 1, seed, r0, n)
+    assert int(host_u64(obs)[0]) == o_obs
+    assert np.array_equal(host_u64(rc), o_rc)
+
+
+@pytest.mark.parametrize("tile_variant", [0, 1, 2])
+@pytest.mark.parametrize("bin_variant", [0, 1, 2])
+def test_mc_permute_b_kernel_shapes(tile_variant, bin_variant):
+    """Every shape of the two fused kernels gives the oracle's integers (config 5 at 3 % and config 1)."""
+    bits.set_option("mc_tile_variant", tile_variant)
+    bits.set_option("mc_bin_variant", bin_variant)
+    try:
+        for k, scale, rounds in ((5, 0.03, 3), (1, 1.0, 4)):
+            w = W.make_config(k, scale=scale)
+            _mc_b_case(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 3, 7, rounds, expect_fused=True)
+    finally:
+        bits.set_option("mc_tile_variant", 2)
+        bits.set_option("mc_bin_variant", 0)
+
+
+def test_mc_permute_b_redo_path_gives_the_same_counts():
+    """Rounds whose flag is raised are redone by the general path: force that for every 2nd round."""
+    w = W.make_config(5, scale=0.02)
+    bits.set_option("mc_force_redo", 2)
+    try:
+        _mc_b_case(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 0, 5, expect_fused=True)
+    finally:
+        bits.set_option("mc_force_redo", 0)
+    bits.set_option("mc_fused", 0)                            # and the general path for every round
+    try:
+        _mc_b_case(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 0, 3, expect_fused=False)
+    finally:
+        bits.set_option("mc_fused", 1)
+
+
+def test_mc_permute_b_hand_over_lists_and_crowded_sub_buckets():
+    rng = np.random.default_rng(8)
+    # (1) long spans against narrow bins: many ends fall into the bin after their start's
+    off = W.genome_offsets([x // 1000 for x in W.GENOME24_LENGTHS])
+    G = int(off[-1])
+    n_b, n_a = 200_000, 5_000
+    def draw(n, max_len):
+        ln = rng.integers(1, max_len, n)
+        c = rng.integers(0, 24, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        ln = np.minimum(ln, hi - lo - 1)
+        s = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        return s.astype(np.uint32), (s + ln - 1).astype(np.uint32)
+    b_s, b_e = draw(n_b, 4000)
+    a_s, a_e = draw(n_a, 3000)
+    _mc_b_case(a_s, a_e, b_s, b_e, off, 5, 0, 4, expect_fused=True)
+    # (2) a tiny genome: every coordinate is hit many times, so runs of equal keys go far beyond the
+    # 4-wide tie window; short spans keep it on the fused path, long ones send it to the general path
+    off2 = np.array([0, 3000, 5000], dtype=np.uint32)
+    a_s2 = rng.integers(0, 2500, 700).astype(np.uint32); a_e2 = np.minimum(a_s2 + rng.integers(0, 300, 700), 2999).astype(np.uint32)
+    for max_span, fused in ((40, True), (400, False)):
+        b_s2 = rng.integers(0, 2500, 12_000).astype(np.uint32)
+        b_e2 = np.minimum(b_s2 + rng.integers(0, max_span, 12_000), 2999).astype(np.uint32)
+        _mc_b_case(a_s2, a_e2, b_s2, b_e2, off2, 6, 1, 4, expect_fused=fused)
+    # (3) very small sets
+    for n in (1, 2, 5, 33):
+        _mc_b_case(a_s2[:7], a_e2[:7], b_s2[:n], b_e2[:n], off2, 7, 0, 3)
+        _mc_b_case(a_s2[:n], a_e2[:n], b_s2[:100], b_e2[:100], off2, 7, 0, 3)
+
+
 @pytest.mark.parametrize("k,scale,rounds", [(1, 1.0, 3), (5, 0.02, 2), (5, 1.0, 2)])
 def test_mc_permute_b_leaves_sorted_arrays_of_last_round(k, scale, rounds):
     """The sort step inside the Monte Carlo loop: after R rounds the workspace holds B_S and B_E of round
