@@ -23,6 +23,7 @@ struct Options {
   int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+tile sort / bin sort+search (mc_tile.cuh)
   int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
   int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
+  int64_t mc_pdl = 1;              // PERMUTE_B fused rounds: launch the two kernels with programmatic stream serialization
   int64_t mc_force_redo = 0;       // PERMUTE_B fused rounds: n > 0 redoes every n-th round by the general path as if its flag were raised (tests)
   int64_t mc_tile_variant = 2;     // PERMUTE_B fused rounds: shape of place_tile_kernel (0: 2 x 512 threads, 1: 1 x 1024, 2: 1 x 1024 with longer tiles)
   int64_t mc_bin_variant = 0;      // PERMUTE_B fused rounds: shape of the per-bin sort (0 wide, 1 narrow, 2 small blocks)
@@ -540,16 +541,30 @@ static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* en
   return BITS_OK;
 }
 
+// The two kernels of a fused round are launched with programmatic stream serialization (unless the
+// per-kernel event timers are on): each may be scheduled while its predecessor drains and waits
+// on the device (griddepcontrol.wait) before it touches shared buffers.
+template <typename Kernel, typename Args>
+static void launch_pdl(Kernel kernel, unsigned grid, unsigned block, size_t smem, cudaStream_t st, const Args& args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = (g_opt.mc_pdl != 0 && !g_prof.on) ? 1 : 0;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  (void)cudaLaunchKernelEx(&cfg, kernel, args);
+}
+
 template <class C>
 static void launch_place_tile(const mct::PlaceTileArgs& pt, cudaStream_t st) {
   const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
-  mct::place_tile_kernel<C><<<pt.n_tiles < blocks ? pt.n_tiles : blocks, C::kThreads, C::kSmem, st>>>(pt);
+  launch_pdl(mct::place_tile_kernel<C>, pt.n_tiles < blocks ? pt.n_tiles : blocks, C::kThreads, C::kSmem, st, pt);
 }
 
 template <class C>
 static void launch_bin_sort(const mct::BinSortArgs& bs, cudaStream_t st) {
   const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
-  mct::bin_sort_search_kernel<C><<<bs.n_bins < blocks ? bs.n_bins : blocks, C::kThreads, C::smem_bytes(bs.n_tiles), st>>>(bs);
+  launch_pdl(mct::bin_sort_search_kernel<C>, bs.n_bins < blocks ? bs.n_bins : blocks, C::kThreads, C::smem_bytes(bs.n_tiles), st, bs);
 }
 
 static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
@@ -976,6 +991,7 @@ int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
 int bits_set_option(const char* name, int64_t value) {
   if (!name) return BITS_ERR_NULL;
   if (!strcmp(name, "mc_fused")) { g_opt.mc_fused = value; return BITS_OK; }
+  if (!strcmp(name, "mc_pdl")) { g_opt.mc_pdl = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_force_redo")) { if (value < 0) return BITS_ERR_FLAGS; g_opt.mc_force_redo = value; return BITS_OK; }
   if (!strcmp(name, "mc_tile_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_tile_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }

@@ -77,6 +77,11 @@ __device__ __forceinline__ void bulk_store_smem_to_global(void* gdst, const void
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void bulk_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// Programmatic dependent launch: a kernel launched with the programmatic-stream-serialization attribute
+// may start while its predecessor on the stream drains; it must not touch what the predecessor wrote (or
+// overwrite what it reads) before grid_dependency_wait().  Both are no-ops in a plain launch.
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_group_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 struct PlaceTileArgs {
@@ -112,6 +117,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
   for (int i = tid; i < kMaxBins; i += C::kThreads) s_cnt[i] = 0;
   const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);        // barrier inside
   const uint32_t shift = a.shift;
+  grid_dependency_wait();     // the previous round's bin sort has finished reading pairs / off / hand-over lists
   bool stage_in_flight = false;   // thread 0: a bulk copy out of s_stage has been issued and not yet waited for
   for (uint32_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
     const uint32_t base = tile * a.tile;
@@ -395,6 +401,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
   // counter (spare word kMaxBins + 1 of this round's hand-over counts; zero on entry, reset for the
   // round after next by block 0 through the other parity's array)
   __shared__ uint32_t s_next;
+  grid_dependency_wait();     // this round's placement has written pairs / off / hand-over lists
   if (blockIdx.x == 0 && tid == 0) a.cross_cnt_next[kMaxBins + 1] = 0;
   uint32_t d = blockIdx.x;
   while (d < a.n_bins) {
