@@ -318,6 +318,9 @@ static int msd_configure() {
       e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgNarrow>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)mct::BinCfgNarrow::smem_bytes(mct::kMaxTiles));
     if (e3 == cudaSuccess)
+      e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgHuge>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)mct::BinCfgHuge::smem_bytes(mct::kMaxTiles));
+    if (e3 == cudaSuccess)
       e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)mct::BinCfgSmall::smem_bytes(mct::kMaxTiles));
     cudaError_t e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg2x512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg2x512::kSmem);
@@ -698,7 +701,8 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   bool fused_ok = msd_on && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0 && L.pairs != nullptr;
   const int variant = (int)g_opt.mc_bin_variant;
   const int tile_variant = (int)g_opt.mc_tile_variant;
-  const double bin_cap = variant == 0 ? (double)mct::BinCfgWide::kCap : (variant == 1 ? (double)mct::BinCfgNarrow::kCap : (double)mct::BinCfgSmall::kCap);
+  const double bin_cap = variant == 0 ? (double)mct::BinCfgWide::kCap
+                       : (variant == 1 ? (double)mct::BinCfgNarrow::kCap : (variant == 2 ? (double)mct::BinCfgSmall::kCap : (double)mct::BinCfgHuge::kCap));
   if (fused_ok) {
     uint64_t v_min = 0;
     for (uint32_t c = 0; c < n_chrom; ++c) { const uint32_t Lc = off[c + 1] - off[c]; v_min += Lc > h_max_span ? Lc - h_max_span : 0; }
@@ -776,7 +780,8 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
         ProfScope prof(kClsBucketSortSearch, st);
         if (variant == 0) launch_bin_sort<mct::BinCfgWide>(bs, st);
         else if (variant == 1) launch_bin_sort<mct::BinCfgNarrow>(bs, st);
-        else launch_bin_sort<mct::BinCfgSmall>(bs, st);
+        else if (variant == 2) launch_bin_sort<mct::BinCfgSmall>(bs, st);
+        else launch_bin_sort<mct::BinCfgHuge>(bs, st);
         BITS_LAUNCH_CHECK();
       }
     }
@@ -994,7 +999,7 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "mc_pdl")) { g_opt.mc_pdl = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_force_redo")) { if (value < 0) return BITS_ERR_FLAGS; g_opt.mc_force_redo = value; return BITS_OK; }
   if (!strcmp(name, "mc_tile_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_tile_variant = value; return BITS_OK; }
-  if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }
+  if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 3) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_gather_group")) { if (value < -1 || value > 5) return BITS_ERR_FLAGS; g_opt.mc_gather_group = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }

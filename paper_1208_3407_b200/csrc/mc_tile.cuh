@@ -47,7 +47,7 @@ using TileCfg1x1024L = TileCfg<1024, 24, 1>;     // 24576-interval tiles, one bl
 constexpr int kMaxTileAny = 24576;
 
 constexpr int kCrossCap = 512;                   // hand-over list entries per bin
-constexpr int kMaxShift = 21;                    // widest bin: 2^21 coordinates
+constexpr int kMaxShift = 22;                    // widest bin: 2^22 coordinates
 constexpr int kMaxTiles = 3072;                  // segment table of the bin sort: one word per tile
 constexpr int kFront = 8;                        // halfwords in front of a cursor array (one uint4)
 
@@ -66,6 +66,7 @@ struct BinCfg {
 using BinCfgWide = BinCfg<512, 16, 13, 2>;       // 8192 keys per bin, two blocks per SM
 using BinCfgNarrow = BinCfg<512, 8, 12, 3>;      // 4096 keys per bin, three blocks per SM
 using BinCfgSmall = BinCfg<256, 16, 12, 4>;      // 4096 keys per bin, four blocks of 256 threads per SM
+using BinCfgHuge = BinCfg<1024, 16, 14, 1>;      // 16384 keys per bin, one block of 1024 threads per SM
 
 constexpr uint32_t kFlagBinTooBig = 1u, kFlagCrossFull = 4u;
 

@@ -329,7 +329,7 @@ def _mc_b_case(a_s, a_e, b_s, b_e, off, seed, r0, n, expect_fused=None):
 
 
 @pytest.mark.parametrize("tile_variant", [0, 1, 2])
-@pytest.mark.parametrize("bin_variant", [0, 1, 2])
+@pytest.mark.parametrize("bin_variant", [0, 1, 2, 3])
 def test_mc_permute_b_kernel_shapes(tile_variant, bin_variant):
     """Every shape of the two fused kernels gives the oracle's integers (config 5 at 3 % and config 1)."""
     bits.set_option("mc_tile_variant", tile_variant)
