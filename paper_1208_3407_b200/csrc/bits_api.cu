@@ -33,6 +33,7 @@ struct Options {
 static Options g_opt;
 
 constexpr int kSMs = 148;
+constexpr size_t kMaxSmemPerBlock = 232448 - 2048;   // 227 KB opt-in limit of shared memory per block on sm_100, less room for static shared memory
 
 // ---------------------------------------------------------------------------------------------
 // Optional per-kernel-class timing with CUDA events on the launching stream (bits_set_option
@@ -319,7 +320,7 @@ static int msd_configure() {
                                 (int)mct::BinCfgNarrow::smem_bytes(mct::kMaxTiles));
     if (e3 == cudaSuccess)
       e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgHuge>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)mct::BinCfgHuge::smem_bytes(mct::kMaxTiles));
+                                (int)(mct::BinCfgHuge::smem_bytes(mct::kMaxTiles) < kMaxSmemPerBlock ? mct::BinCfgHuge::smem_bytes(mct::kMaxTiles) : kMaxSmemPerBlock));
     if (e3 == cudaSuccess)
       e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)mct::BinCfgSmall::smem_bytes(mct::kMaxTiles));
@@ -742,6 +743,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       if (g_opt.mc_gather_group >= 0) bs.group_log2 = (uint32_t)g_opt.mc_gather_group;
       bs.group = 1u << bs.group_log2;
       if (pt.n_tiles > (uint32_t)mct::kMaxTiles) fused_ok = false;
+      if (variant == 3 && mct::BinCfgHuge::smem_bytes(pt.n_tiles) > kMaxSmemPerBlock) fused_ok = false;
     }
   }
   if (!fused_ok) {
