@@ -423,6 +423,23 @@ def run_b200(args):
 
     if rank == 0 and world == 1 and not args.no_extras:
         line["other_workloads"] = secondary_workloads(device, peak)
+        if w.which == 1:
+            # SURVEY 8(f).1, reported BESIDE the headline: the sort-free variant of the same rounds
+            # (count(A, B') = count(B', A): fresh B intervals searched against the once-sorted A; no B_S / B_E)
+            Rs = min(R, 200)
+            ws2 = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, w.which), dtype=torch.uint8, device=device)
+            rc2 = torch.empty(Rs, dtype=torch.int64, device=device)
+            bits.set_option("mc_symmetric", 1)
+            try:
+                med, mn = time_device(lambda: bits.mc_rounds(*d, w.chrom_offsets, w.which, w.mc_seed, r0, Rs, workspace=ws2,
+                                                             observed_out=obs, round_counts_out=rc2), 3, warmup=1)
+            finally:
+                bits.set_option("mc_symmetric", 0)
+            line["other_workloads"]["cfg5_symmetric_sort_free"] = {
+                "mc_rounds_per_s": Rs / (med * 1e-3), "rounds_per_call": Rs, "ms_median": med,
+                "intervals_searched_per_s": Rs * w.n_b / (med * 1e-3),
+                "same_counts_as_headline_path": bool(torch.equal(rc2, rc[:Rs]))}
+            del ws2
         n_cpu = 2 if args.config == 5 else 50
         rps, t_obs, t_r = oracle_marginal_rounds_per_s(w, w.which, 0, n_cpu)
         line["cpu_baseline"] = {"value": rps, "unit": "rounds/s", "cores": 1, "kind": "oracle",

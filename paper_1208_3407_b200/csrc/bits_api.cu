@@ -23,6 +23,7 @@ struct Options {
   int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+tile sort / bin sort+search (mc_tile.cuh)
   int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
   int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
+  int64_t mc_symmetric = 0;        // PERMUTE_B rounds: 1 = sort-free variant (fresh B intervals counted against the once-sorted A)
   int64_t mc_pdl = 1;              // PERMUTE_B fused rounds: launch the two kernels with programmatic stream serialization
   int64_t mc_force_redo = 0;       // PERMUTE_B fused rounds: n > 0 redoes every n-th round by the general path as if its flag were raised (tests)
   int64_t mc_tile_variant = 2;     // PERMUTE_B fused rounds: shape of place_tile_kernel (0: 2 x 512 threads, 1: 1 x 1024, 2: 1 x 1024 with longer tiles)
@@ -194,7 +195,7 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
         L.spans = c.take<uint32_t>(align_up(n_a, 4) + 4);
       } else {
         L.spans = c.take<uint32_t>(align_up(n_b, 4) + 4);
-        L.q.carve(c, n_a, false);
+        L.q.carve(c, n_a, true);
         if (n_b <= kFusedMaxKeys) {
           const uint32_t n_tiles = max_tiles_for(n_b);
           L.tile_stride = (uint32_t)align_up((uint64_t)n_tiles + 1, 8);
@@ -619,7 +620,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   const PhiloxKeys key = make_philox_keys(seed);
   if (which == BITS_PERMUTE_A) {
     McAArgs m;
-    m.spans = L.spans; m.n_a = (uint32_t)n_a; m.key = key; m.chrom = chrom;
+    m.spans = L.spans; m.n_a = (uint32_t)n_a; m.tag = 0u; m.key = key; m.chrom = chrom;
     m.bs = sorted_set(L.b, 0); m.be = sorted_set(L.b, 1);
     m.round_counts = reinterpret_cast<unsigned long long*>(round_counts_out);
     const unsigned gx = (unsigned)ceil_div(ceil_div(n_a, 4), 256);
@@ -640,6 +641,26 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   BITS_TRY(sort_arrays(L.q, a_end, a_start, 2, nullptr, false, &q_epoch, st));
   const uint32_t* q_end_sorted = L.q.buf[0][0];
   const uint32_t* q_start_sorted = L.q.buf[1][0];
+  if (g_opt.mc_symmetric) {
+    // SURVEY 8(f).1, the sort-free variant: count(A, B') = count(B', A), so every fresh interval of B is
+    // counted against the once-sorted A (first = #{A.start <= b'.end}, last = #{A.end < b'.start}) and
+    // nothing is sorted per round.  Same integers; B_S / B_E of the round are NOT produced.
+    BITS_TRY(launch_build_index(L.q, st));
+    McAArgs m;
+    m.spans = L.spans; m.n_a = (uint32_t)n_b; m.tag = 1u; m.key = key; m.chrom = chrom;
+    m.bs = sorted_set(L.q, 1); m.be = sorted_set(L.q, 0);
+    m.round_counts = reinterpret_cast<unsigned long long*>(round_counts_out);
+    const unsigned gx = (unsigned)ceil_div(ceil_div(n_b, 4), 256);
+    for (uint32_t done = 0; done < n_rounds;) {
+      const uint32_t chunk = n_rounds - done < 4096u ? n_rounds - done : 4096u;
+      m.round0 = round_begin + done; m.out0 = done;
+      ProfScope prof(kClsMcA, st);
+      mc_permute_a_kernel<<<dim3(gx, chunk), 256, 0, st>>>(m);
+      BITS_LAUNCH_CHECK();
+      done += chunk;
+    }
+    return BITS_OK;
+  }
   const bool msd_on = g_opt.sort_msd != 0;
   const bool hist_in_place = g_opt.place_fused_hist != 0;
   // histograms the placement kernel accumulates into: the MSD sort's bins (left zero by plan_kernel)
@@ -998,6 +1019,7 @@ int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
 int bits_set_option(const char* name, int64_t value) {
   if (!name) return BITS_ERR_NULL;
   if (!strcmp(name, "mc_fused")) { g_opt.mc_fused = value; return BITS_OK; }
+  if (!strcmp(name, "mc_symmetric")) { g_opt.mc_symmetric = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_pdl")) { g_opt.mc_pdl = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_force_redo")) { if (value < 0) return BITS_ERR_FLAGS; g_opt.mc_force_redo = value; return BITS_OK; }
   if (!strcmp(name, "mc_tile_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_tile_variant = value; return BITS_OK; }

@@ -193,6 +193,7 @@ __global__ void __launch_bounds__(256) sorted_query_total_kernel(const uint32_t*
 struct McAArgs {
   const uint32_t* spans;     // dev uint32[n_a], padded to a multiple of 4 with zeros
   uint32_t n_a;
+  uint32_t tag;              // Philox stream of the re-placed set (0: A, 1: B searched the other way round)
   uint32_t round0;           // first round of this launch
   PhiloxKeys key;
   ChromTable chrom;
@@ -214,7 +215,7 @@ __global__ void __launch_bounds__(256) mc_permute_a_kernel(McAArgs a) {
     const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans) + t);
     const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
     uint32_t st[4];
-    place4(i0, round, 0u, a.key, d, off, a.chrom, st);
+    place4(i0, round, a.tag, a.key, d, off, a.chrom, st);
 #pragma unroll
     for (int j = 0; j < 4; ++j)
       if (i0 + j < a.n_a) sum += icount(a.bs, a.be, st[j], st[j] + d[j]);

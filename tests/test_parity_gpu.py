@@ -358,6 +358,17 @@ def test_mc_permute_b_redo_path_gives_the_same_counts():
         bits.set_option("mc_fused", 1)
 
 
+def test_mc_permute_b_symmetric_sort_free_variant():
+    """count(A, B') = count(B', A) -- the fresh B intervals searched against the sorted A."""
+    bits.set_option("mc_symmetric", 1)
+    try:
+        for k, scale, rounds in ((1, 1.0, 6), (5, 0.02, 3)):
+            w = W.make_config(k, scale=scale)
+            _mc_b_case(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 2, 11, rounds, expect_fused=False)
+    finally:
+        bits.set_option("mc_symmetric", 0)
+
+
 def test_mc_permute_b_hand_over_lists_and_crowded_sub_buckets():
     rng = np.random.default_rng(8)
     # (1) long spans against narrow bins: many ends fall into the bin after their start's
