@@ -208,6 +208,25 @@ def time_device(fn, reps: int, warmup: int = 3):
     return statistics.median(ts), min(ts)
 
 
+def l2_yardsticks(device):
+    """L2 denominators for the search kernels: streaming read over 48 MB and random
+    32-byte-sector gather over 80 MB, both L2-resident.  Bench-only code (probe/l2_probe.cu)."""
+    import ctypes as C
+    import torch
+    from paper_1208_3407_b200 import build as B
+    lib = C.CDLL(B.build_probe())
+    for f in (lib.l2_probe_stream_gbs, lib.l2_probe_gather_gsectors):
+        f.restype = C.c_double
+        f.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_int, C.c_void_p]
+    buf = torch.ones(80 << 20, dtype=torch.uint8, device=device)
+    sink = torch.zeros(4, dtype=torch.int32, device=device)
+    st = torch.cuda.current_stream().cuda_stream
+    stream = lib.l2_probe_stream_gbs(buf.data_ptr(), 48 << 20, sink.data_ptr(), 10, st)
+    gather = lib.l2_probe_gather_gsectors(buf.data_ptr(), 80 << 20, sink.data_ptr(), 10, st)
+    return {"l2_stream_read_gbs_48MB": stream, "l2_random_sector_gather_gsectors_per_s_80MB": gather,
+            "l2_random_sector_gather_gbs_80MB": gather * 32}
+
+
 def secondary_workloads(device, peak_gbs):
     """The other throughputs BASELINE.json's metric names, on their own configs (not the timed headline)."""
     import torch
@@ -423,6 +442,7 @@ def run_b200(args):
 
     if rank == 0 and world == 1 and not args.no_extras:
         line["other_workloads"] = secondary_workloads(device, peak)
+        line["l2_yardsticks"] = l2_yardsticks(device)
         if w.which == 1:
             # SURVEY 8(f).1, reported BESIDE the headline: the sort-free variant of the same rounds
             # (count(A, B') = count(B', A): fresh B intervals searched against the once-sorted A; no B_S / B_E)

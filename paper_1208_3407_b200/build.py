@@ -42,5 +42,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+PROBE_SRC = os.path.join(HERE, "probe", "l2_probe.cu")
+PROBE_LIB = os.path.join(HERE, "probe", "libl2_probe.so")
+
+
+def build_probe(force: bool = False) -> str:
+    """Compile the bench-only L2 yardstick (probe/l2_probe.cu); it is not linked into libbits_b200.so."""
+    if not force and os.path.exists(PROBE_LIB) and os.path.getmtime(PROBE_SRC) <= os.path.getmtime(PROBE_LIB):
+        return PROBE_LIB
+    tmp = PROBE_LIB + f".tmp{os.getpid()}"
+    subprocess.check_call([NVCC, *FLAGS, "-o", tmp, PROBE_SRC])
+    os.replace(tmp, PROBE_LIB)
+    return PROBE_LIB
+
+
 if __name__ == "__main__":
+    build_probe(force="--force" in sys.argv)
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -23,6 +23,7 @@ struct Options {
   int64_t mc_fused = 1;            // PERMUTE_B rounds: 1 = place+tile sort / bin sort+search (mc_tile.cuh)
   int64_t mc_sorted_queries = 1;   // PERMUTE_B rounds: 1 = search with A's keys sorted once, 0 = bucket index per round
   int64_t place_fused_hist = 1;    // PERMUTE_B rounds: 1 = histogram inside the placement kernel
+  int64_t search_variant = 0;      // count kernel: 0 bucket index, 1 plain binary search (the paper's), 2 top 11 levels in shared memory
   int64_t mc_symmetric = 0;        // PERMUTE_B rounds: 1 = sort-free variant (fresh B intervals counted against the once-sorted A)
   int64_t mc_pdl = 1;              // PERMUTE_B fused rounds: launch the two kernels with programmatic stream serialization
   int64_t mc_force_redo = 0;       // PERMUTE_B fused rounds: n > 0 redoes every n-th round by the general path as if its flag were raised (tests)
@@ -439,12 +440,20 @@ static int launch_count(const uint32_t* a_start, const uint32_t* a_end, uint32_t
   const bool vec = (((uintptr_t)a_start | (uintptr_t)a_end | (uintptr_t)counts) & 15) == 0;
   const int grid = grid_for(ceil_div(n_a, 4), 256);
   ProfScope prof(kClsCount, st);
-  if (vec)
-    count_kernel<true><<<grid, 256, 0, st>>>(a_start, a_end, n_a, sorted_set(b, 0), sorted_set(b, 1), counts,
-                                             reinterpret_cast<unsigned long long*>(total));
-  else
-    count_kernel<false><<<grid, 256, 0, st>>>(a_start, a_end, n_a, sorted_set(b, 0), sorted_set(b, 1), counts,
-                                              reinterpret_cast<unsigned long long*>(total));
+  const SortedSet s0 = sorted_set(b, 0), s1 = sorted_set(b, 1);
+  unsigned long long* tot = reinterpret_cast<unsigned long long*>(total);
+  const int sv = (int)g_opt.search_variant;
+#define BITS_COUNT_LAUNCH(V, S) count_kernel<V, S><<<grid, 256, 0, st>>>(a_start, a_end, n_a, s0, s1, counts, tot)
+  if (vec) {
+    if (sv == kSearchPlain) BITS_COUNT_LAUNCH(true, kSearchPlain);
+    else if (sv == kSearchStaged) BITS_COUNT_LAUNCH(true, kSearchStaged);
+    else BITS_COUNT_LAUNCH(true, kSearchIndex);
+  } else {
+    if (sv == kSearchPlain) BITS_COUNT_LAUNCH(false, kSearchPlain);
+    else if (sv == kSearchStaged) BITS_COUNT_LAUNCH(false, kSearchStaged);
+    else BITS_COUNT_LAUNCH(false, kSearchIndex);
+  }
+#undef BITS_COUNT_LAUNCH
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -1019,6 +1028,7 @@ int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
 int bits_set_option(const char* name, int64_t value) {
   if (!name) return BITS_ERR_NULL;
   if (!strcmp(name, "mc_fused")) { g_opt.mc_fused = value; return BITS_OK; }
+  if (!strcmp(name, "search_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.search_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_symmetric")) { g_opt.mc_symmetric = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_pdl")) { g_opt.mc_pdl = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_force_redo")) { if (value < 0) return BITS_ERR_FLAGS; g_opt.mc_force_redo = value; return BITS_OK; }

@@ -107,14 +107,58 @@ __global__ void __launch_bounds__(256) build_index_kernel(IndexArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// Search designs of the count kernel (bits_set_option "search_variant"; DESIGN.md section 5 has the numbers):
+//   kSearchIndex   bucket index over the sorted array: one index word + two 32-byte sectors per look-up [default]
+//   kSearchPlain   the paper's design: a binary search over the whole sorted
+//                  array, nothing staged, ~log2|B| dependent probes (fixed trip count, no divergence)
+//   kSearchStaged  the top 11 levels staged in shared memory (2,048 evenly spaced keys per array, 16 KB),
+//                  then a binary search inside one 1/2048th of the array
+enum { kSearchIndex = 0, kSearchPlain = 1, kSearchStaged = 2 };
+constexpr int kStagedLevels = 11, kStaged = 1 << kStagedLevels;
+
+// #{keys <= q} by a fixed-trip binary search over keys[lo .. lo + len)
+__device__ __forceinline__ uint32_t rank_le_range(const uint32_t* __restrict__ keys, uint32_t lo, uint32_t len, uint32_t q) {
+  while (len > 0) {
+    const uint32_t half = len >> 1;
+    const bool right = __ldg(keys + lo + half) <= q;
+    lo = right ? lo + half + 1 : lo;
+    len = right ? len - half - 1 : half;
+  }
+  return lo;
+}
+
+// block j of the staged search = keys[(j * n) >> 11 .. ((j + 1) * n) >> 11); s_top[j] = its last key
+__device__ __forceinline__ uint32_t staged_bound(uint32_t j, uint32_t n) { return (uint32_t)(((uint64_t)j * n) >> kStagedLevels); }
+__device__ __forceinline__ void stage_top_levels(const SortedSet& s, uint32_t* s_top) {
+  for (uint32_t j = threadIdx.x; j < (uint32_t)kStaged; j += blockDim.x) {
+    const uint32_t e = staged_bound(j + 1, s.n);
+    s_top[j] = e ? __ldg(s.keys + e - 1) : 0u;       // (an empty block repeats a smaller key or 0: harmless)
+  }
+}
+__device__ __forceinline__ uint32_t rank_le_staged(const SortedSet& s, const uint32_t* s_top, uint32_t q) {
+  uint32_t j = 0;                                   // #{blocks whose last key <= q}
+#pragma unroll
+  for (uint32_t step = kStaged >> 1; step > 0; step >>= 1) j += (s_top[j + step - 1] <= q) ? step : 0u;
+  j += (j < (uint32_t)kStaged && s_top[j] <= q) ? 1u : 0u;
+  if (j >= (uint32_t)kStaged) return s.n;
+  const uint32_t lo = staged_bound(j, s.n);
+  return rank_le_range(s.keys, lo, staged_bound(j + 1, s.n) - lo, q);
+}
+
 // Count kernel: queries in input order, four per thread.  Writes per-interval counts if
 // counts != nullptr; adds the block's sum to *total if total != nullptr.
-template <bool kVec>
+template <bool kVec, int kSearch>
 __global__ void __launch_bounds__(256) count_kernel(const uint32_t* __restrict__ a_start,
                                                     const uint32_t* __restrict__ a_end, uint32_t n_a,
                                                     SortedSet bs, SortedSet be,
                                                     uint32_t* __restrict__ counts, unsigned long long* total) {
   __shared__ uint64_t s_red[8];
+  __shared__ uint32_t s_top[kSearch == kSearchStaged ? 2 * kStaged : 1];
+  if (kSearch == kSearchStaged) {
+    stage_top_levels(bs, s_top);
+    stage_top_levels(be, s_top + kStaged);
+    __syncthreads();
+  }
   uint64_t sum = 0;
   const uint64_t n4 = ((uint64_t)n_a + 3) >> 2;
   for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n4; t += (uint64_t)gridDim.x * blockDim.x) {
@@ -135,7 +179,15 @@ __global__ void __launch_bounds__(256) count_kernel(const uint32_t* __restrict__
       }
     }
 #pragma unroll
-    for (int j = 0; j < 4; ++j) c[j] = icount(bs, be, qs[j], qe[j]);
+    for (int j = 0; j < 4; ++j) {
+      if (kSearch == kSearchIndex) {
+        c[j] = icount(bs, be, qs[j], qe[j]);
+      } else if (kSearch == kSearchPlain) {
+        c[j] = rank_le_range(bs.keys, 0, bs.n, qe[j]) - (qs[j] == 0 ? 0u : rank_le_range(be.keys, 0, be.n, qs[j] - 1u));
+      } else {
+        c[j] = rank_le_staged(bs, s_top, qe[j]) - (qs[j] == 0 ? 0u : rank_le_staged(be, s_top + kStaged, qs[j] - 1u));
+      }
+    }
     if (!full) {
 #pragma unroll
       for (int j = 0; j < 4; ++j) if (i0 + j >= n_a) c[j] = 0;

@@ -202,6 +202,25 @@ def test_count_config2_full_size():
     assert int(host_u64(t_ba)[0]) == total and int(host_u64(t_aa)[0]) >= w.n_a
 
 
+@pytest.mark.parametrize("variant", [1, 2])
+def test_count_search_design_variants(variant):
+    """The other search designs of the study (plain binary search, top levels in shared memory) give the same counts."""
+    rng = np.random.default_rng(40 + variant)
+    bits.set_option("search_variant", variant)
+    try:
+        w = W.make_config(2, scale=0.05)
+        check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
+        for n_b in (1, 2, 7, 2047, 2048, 2049, 5000):
+            b_s = rng.integers(0, 100_000, n_b).astype(np.uint32)
+            b_e = b_s + rng.integers(0, 300, n_b).astype(np.uint32)
+            a_s = rng.integers(0, 100_000, 777).astype(np.uint32)
+            a_e = a_s + rng.integers(0, 500, 777).astype(np.uint32)
+            a_s[0] = 0; a_e[0] = 0
+            check_counts(a_s, a_e, b_s, b_e)
+    finally:
+        bits.set_option("search_variant", 0)
+
+
 def test_count_config4_full_size():
     w = W.make_config(4)
     total = check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
