@@ -3,27 +3,31 @@
 // structure" every round), as TWO launches with no global atomics on the data path:
 //
 //   place_tile_kernel   place (Philox4x32-10 -> start', end') fused with the
-//                       first half of the sort: every tile of <= 8192 fresh intervals is ordered
-//                       by bin (bin = start' >> shift, fixed per call) in shared memory and
-//                       written out as (start', end') pairs, coalesced; next to it goes the
-//                       tile's exclusive bin prefix, transposed:  off[b][tile] = #{pairs of the
-//                       tile in bins < b}.  Fresh keys never go to HBM unsorted.
+//                       first half of the sort: every tile of up to 24,576 fresh intervals is
+//                       ordered by bin (bin = start' >> shift, fixed per call) in shared memory --
+//                       count pass, scan, staging pass through per-bin cursors -- and leaves as
+//                       (start', end') pairs through cp.async.bulk; next to it goes the tile's
+//                       exclusive bin prefix, transposed:  off[b][tile] = #{pairs of the tile in
+//                       bins < b}.  Fresh keys never go to HBM unsorted.
 //   bin_sort_search_kernel  one bin at a time per block.  Row b of the prefix table gives, per
 //                       tile, where the bin's pairs sit; its row sum is the number of keys in
 //                       all earlier bins, i.e. where the bin starts in the sorted arrays -- no
 //                       histogram pass, no scan over bins, no reservation.  The pairs are
-//                       gathered (cp.async) into shared memory; starts and ends are each sorted
-//                       there (Algorithm 2's Sort(B_S), Sort(B_E): counting
-//                       sort on the next 12 bits, ties inside a sub-bucket ordered by comparison
-//                       counting on the way out), written to B_S / B_E, and -- while the bin is
-//                       still in shared memory -- the queries that fall into its key range are
-//                       ranked against it (Algorithm 1's two BSEARCHes) and
-//                       their ranks summed.
+//                       gathered (cp.async, a group of lanes per segment) into shared memory;
+//                       starts and ends are each sorted there (Algorithm 2's Sort(B_S),
+//                       Sort(B_E): counting sort on the next 13 bits with
+//                       16-bit cursors, ties inside a sub-bucket ordered by comparison counting
+//                       on the way out), written to B_S / B_E, and -- while the bin is still in
+//                       shared memory -- the queries that fall into its key range are ranked
+//                       against it (Algorithm 1's two BSEARCHes) and their ranks
+//                       summed.
 //
 // An end that lies in the bin after its start's bin (span < bin width is a precondition of this
 // path, checked on the host) is handed over through a small per-bin list.  A bin with more than
 // kCap keys or an over-full hand-over list raises the round's flag; the host redoes flagged
 // rounds with the general path (place_kernel -> sort_arrays -> sorted_query_total_kernel).
+// Kernel shapes are template configurations (TileCfg, BinCfg); DESIGN.md section 5 has the
+// measurements behind the defaults.
 #pragma once
 #include "msd_sort.cuh"
 #include "philox_place.cuh"
