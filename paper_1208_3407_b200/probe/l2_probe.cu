@@ -17,22 +17,23 @@ __global__ void __launch_bounds__(256) stream_read_kernel(const uint4* __restric
   if (acc == 0x12345678u) *sink = acc;       // keeps the loads alive
 }
 
-// Every thread reads `per_thread` sectors at pseudo-random 32-byte aligned positions (two uint4 = one sector).
+// Every thread touches `per_thread` pseudo-random 32-byte sectors, one 16-byte load per sector, eight
+// independent loads in flight.
 __global__ void __launch_bounds__(256) gather_sector_kernel(const uint4* __restrict__ p, uint64_t n_sectors, uint32_t per_thread,
                                                             uint32_t* sink) {
   uint32_t s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u, acc = 0;
-  for (uint32_t k = 0; k < per_thread; k += 4) {
-    uint64_t idx[4];
+  for (uint32_t k = 0; k < per_thread; k += 8) {
+    uint64_t idx[8];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < 8; ++j) {
       s = s * 1664525u + 1013904223u;
       idx[j] = ((uint64_t)s * n_sectors) >> 32;
     }
+    uint4 v[8];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const uint4 a = __ldcg(p + 2 * idx[j]), b = __ldcg(p + 2 * idx[j] + 1);
-      acc ^= a.x ^ b.w;
-    }
+    for (int j = 0; j < 8; ++j) v[j] = __ldcg(p + 2 * idx[j]);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc ^= v[j].x;
   }
   if (acc == 0x12345678u) *sink = acc;
 }
