@@ -410,7 +410,8 @@ static int launch_build_index(const SortCtx& c, cudaStream_t st) {
   ia.keys[0] = c.buf[0][0]; ia.keys[1] = c.buf[1][0];
   ia.idx[0] = c.idx[0]; ia.idx[1] = c.idx[1];
   ia.n = c.n; ia.shift = c.shift;
-  const uint64_t threads = (uint64_t)c.n + 1 > (uint64_t)kPad ? (uint64_t)c.n + 1 : (uint64_t)kPad;
+  const uint64_t need = ceil_div((uint64_t)c.n, 4) + 1;   // four positions per thread
+  const uint64_t threads = need > (uint64_t)kPad ? need : (uint64_t)kPad;
   ProfScope prof(kClsIndex, st);
   build_index_kernel<<<dim3((unsigned)ceil_div(threads, 256), 2), 256, 0, st>>>(ia);
   BITS_LAUNCH_CHECK();

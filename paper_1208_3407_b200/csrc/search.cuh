@@ -86,23 +86,47 @@ __global__ void __launch_bounds__(256) build_index_kernel(IndexArgs a) {
   const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;   // warps are never partly out of range
   const uint32_t lane = threadIdx.x & 31;
   if (gid < kPad) keys[(uint64_t)n + gid] = 0xffffffffu;
-  uint32_t lo = 1, hi = 0;   // fill idx[lo..hi] = i  (empty by default)
-  const uint32_t i = (uint32_t)gid;
-  if (gid <= n) {
-    lo = (i == 0) ? 0u : (keys[i - 1] >> s) + 1u;
-    hi = (i == n) ? H : (keys[i] >> s);
+  {
+    // idx[(key[n-1] >> s) + 1 .. H] = n: the entries above the largest key (for a genome that ends well
+    // below 2^32 that is a long run) are filled by the whole grid, not by one thread
+    const uint64_t tail_lo = n ? (uint64_t)(keys[n - 1] >> s) + 1u : 0u;
+    for (uint64_t h = tail_lo + gid; h <= H; h += (uint64_t)gridDim.x * blockDim.x) idx[h] = n;
   }
-  const bool some = lo <= hi;
-  const uint32_t len = some ? hi - lo + 1u : 0u;
-  if (some && len <= 4)
-    for (uint32_t h = lo; h <= hi; ++h) idx[h] = i;
-  uint32_t big = __ballot_sync(kFullMask, len > 4);
-  while (big) {
-    const int src = __ffs(big) - 1;
-    big &= big - 1;
-    const uint32_t l = __shfl_sync(kFullMask, lo, src), hh = __shfl_sync(kFullMask, hi, src);
-    const uint32_t v = __shfl_sync(kFullMask, i, src);
-    for (uint64_t h = (uint64_t)l + lane; h <= hh; h += 32) idx[h] = v;
+  // four consecutive positions per thread (one 16-byte load; the arrays are 32-byte aligned and padded)
+  const uint64_t i0 = gid << 2;
+  uint32_t k[4] = {0, 0, 0, 0};
+  uint32_t prev = 0;
+  if (i0 < n) {
+    if (i0 + 3 < n) {
+      const uint4 v = *reinterpret_cast<const uint4*>(keys + i0);
+      k[0] = v.x; k[1] = v.y; k[2] = v.z; k[3] = v.w;
+    } else {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) k[j] = i0 + j < n ? keys[i0 + j] : 0u;
+    }
+    if (i0) prev = keys[i0 - 1];
+  }
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const uint32_t i = (uint32_t)i0 + j;
+    uint32_t lo = 1, hi = 0;   // fill idx[lo..hi] = i  (empty by default)
+    if (i0 + j < n) {
+      lo = (i == 0) ? 0u : (prev >> s) + 1u;
+      hi = k[j] >> s;
+    }
+    prev = k[j];
+    const bool some = lo <= hi;
+    const uint32_t len = some ? hi - lo + 1u : 0u;
+    if (some && len <= 4)
+      for (uint32_t h = lo; h <= hi; ++h) idx[h] = i;
+    uint32_t big = __ballot_sync(kFullMask, len > 4);
+    while (big) {
+      const int src = __ffs(big) - 1;
+      big &= big - 1;
+      const uint32_t l = __shfl_sync(kFullMask, lo, src), hh = __shfl_sync(kFullMask, hi, src);
+      const uint32_t v = __shfl_sync(kFullMask, i, src);
+      for (uint64_t h = (uint64_t)l + lane; h <= hh; h += 32) idx[h] = v;
+    }
   }
 }
 
