@@ -27,9 +27,12 @@ struct SortedSet {
 };
 
 inline uint32_t index_shift_for(uint64_t n) {
-  // about one bucket per four keys, between 2 and 2^24 buckets
+  // about one bucket per four keys, between 2 and 2^24 buckets; per eight keys once keys + index
+  // outgrow the L2 (measured on config 4: 303 -> 283 us; on config 3, which stays L2-resident, the
+  // finer index is the faster one: 47.6 against 52.8 us)
+  const uint64_t per = n > (4ull << 20) ? 8 : 4;
   uint32_t bits = 1;
-  while (bits < 24 && (1ull << bits) < n / 4) ++bits;
+  while (bits < 24 && (1ull << bits) < n / per) ++bits;
   return 32 - bits;
 }
 inline uint64_t index_entries(uint32_t shift) { return (1ull << (32 - shift)) + 1; }
