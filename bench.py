@@ -377,7 +377,9 @@ def run_b200(args):
             launch_ms = timed[dom][0] / timed[dom][1]
             achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
             roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                        "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(kname), "peak_source": peak_src,
+                        "frac": achieved / peak,
+                        "traffic": NCU_TRAFFIC_BYTES.get(kname) if (args.config == 5 and args.scale == 1.0) else None,
+                        "peak_source": peak_src,
                         "avg_launch_ms": launch_ms, "launches_timed": timed[dom][1],
                         "algorithmic_bytes_per_launch": alg_bytes,
                         "kernel_ms_per_round": {k: v[0] / (R * prof_steps) for k, v in timed.items()},
