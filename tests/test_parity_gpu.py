@@ -377,6 +377,28 @@ def test_mc_permute_b_redo_path_gives_the_same_counts():
         bits.set_option("mc_fused", 1)
 
 
+@pytest.mark.parametrize("n_b,n_chrom,max_len", [(3_300_001, 1, 700), (17_000_003, 24, 400), (1_234_567, 900, 50)])
+def test_mc_permute_b_other_shapes(n_b, n_chrom, max_len):
+    """Fused rounds on set sizes, tile counts and chromosome tables other than config 5's."""
+    rng = np.random.default_rng(n_chrom)
+    if n_chrom == 24:
+        lens = np.array(W.GENOME24_LENGTHS)
+    elif n_chrom == 1:
+        lens = np.array([1_500_000_000])
+    else:
+        lens = rng.integers(200_000, 4_000_000, n_chrom)
+    off = W.genome_offsets(lens)
+    def draw(n):
+        c = rng.integers(0, n_chrom, n)
+        ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        s = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        return s.astype(np.uint32), (s + ln - 1).astype(np.uint32)
+    b_s, b_e = draw(n_b)
+    a_s, a_e = draw(50_000)
+    _mc_b_case(a_s, a_e, b_s, b_e, off, 12, 3, 2, expect_fused=True)
+
+
 def test_mc_permute_b_symmetric_sort_free_variant():
     """count(A, B') = count(B', A) -- the fresh B intervals searched against the sorted A."""
     bits.set_option("mc_symmetric", 1)
