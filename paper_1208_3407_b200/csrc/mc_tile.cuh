@@ -355,6 +355,7 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
                                                    const uint16_t* cur, uint32_t gbase, uint32_t* __restrict__ dst,
                                                    const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi) {
   const int tid = threadIdx.x;
+#pragma unroll 2
   for (uint32_t p = tid; p < mv; p += C::kThreads) {
     const uint32_t k = buf[p];
     const uint32_t sb = sub_of(k, mask, sshift);
@@ -467,6 +468,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     {
       uint32_t* cs = reinterpret_cast<uint32_t*>(s_cur_s);
       uint32_t* ce = reinterpret_cast<uint32_t*>(s_cur_e);
+#pragma unroll 2
       for (uint32_t i = tid; i < me; i += C::kThreads) {
         if (i < np) count_key(cs, sub_of(s_ks[i], mask, sshift));
         const uint32_t e = s_ke[i];
