@@ -127,8 +127,10 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
   for (uint32_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
     const uint32_t base = tile * a.tile;
     const uint32_t count = min(a.tile, a.n - base);
-    uint32_t st[C::kIpt];
-#pragma unroll
+    // the starts wait for the staging pass in the tile's own (not yet written) slice of `pairs`:
+    // 24 fewer live registers in the Philox pass; the loads below hit L2
+    uint32_t* const scratch = reinterpret_cast<uint32_t*>(a.pairs + base);
+#pragma unroll 2
     for (int g = 0; g < C::kIpt / 4; ++g) {
       const uint32_t l0 = 4u * (tid + g * C::kThreads);                   // four consecutive intervals of the tile
       if (l0 < count) {
@@ -136,9 +138,9 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
         const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
         uint32_t ss[4];
         place4(base + l0, a.round, a.tag, a.key, dd, off, a.chrom, ss);
+        *reinterpret_cast<uint4*>(scratch + l0) = make_uint4(ss[0], ss[1], ss[2], ss[3]);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-          st[4 * g + j] = ss[j];
           if (l0 + j < count) {
             const uint32_t bin = ss[j] >> shift;
             atomicAdd(&s_cnt[bin], 1u);                             // count only: the slot is taken in the staging pass
@@ -184,23 +186,30 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
     // stage the pairs in bin order: every bin's base doubles as its cursor (spans re-read: cache hits)
     // (the four slots of a group are taken first and filled afterwards, so the atomics overlap)
     {
-      uint4 d4 = make_uint4(0, 0, 0, 0);
-      if (4u * tid < count) d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + 4u * tid));
-#pragma unroll
+      uint4 d4 = make_uint4(0, 0, 0, 0), s4 = d4;
+      if (4u * tid < count) {
+        d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + 4u * tid));
+        s4 = *reinterpret_cast<const uint4*>(scratch + 4u * tid);
+      }
+#pragma unroll 2
       for (int g = 0; g < C::kIpt / 4; ++g) {
         const uint32_t l0 = 4u * (tid + g * C::kThreads);
         const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
-        if (g + 1 < C::kIpt / 4) {                                       // the next group's spans are on their way
+        const uint32_t st[4] = {s4.x, s4.y, s4.z, s4.w};
+        if (g + 1 < C::kIpt / 4) {                                       // the next group's spans and starts are on their way
           const uint32_t l1 = l0 + 4u * C::kThreads;
-          if (l1 < count) d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l1));
+          if (l1 < count) {
+            d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l1));
+            s4 = *reinterpret_cast<const uint4*>(scratch + l1);
+          }
         }
         if (l0 < count) {
           uint32_t slot[4];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) slot[j] = l0 + j < count ? atomicAdd(&s_cnt[st[4 * g + j] >> shift], 1u) : 0xffffffffu;
+          for (int j = 0; j < 4; ++j) slot[j] = l0 + j < count ? atomicAdd(&s_cnt[st[j] >> shift], 1u) : 0xffffffffu;
 #pragma unroll
           for (int j = 0; j < 4; ++j)
-            if (slot[j] != 0xffffffffu) s_stage[slot[j]] = make_uint2(st[4 * g + j], st[4 * g + j] + dd[j]);
+            if (slot[j] != 0xffffffffu) s_stage[slot[j]] = make_uint2(st[j], st[j] + dd[j]);
         }
       }
     }
