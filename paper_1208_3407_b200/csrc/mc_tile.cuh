@@ -130,11 +130,15 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
     // the starts wait for the staging pass in the tile's own (not yet written) slice of `pairs`:
     // 24 fewer live registers in the Philox pass; the loads below hit L2
     uint32_t* const scratch = reinterpret_cast<uint32_t*>(a.pairs + base);
+    uint4 dn = make_uint4(0, 0, 0, 0);                                    // spans of the next group, loaded one group ahead
+    if (4u * tid < count) dn = __ldg(reinterpret_cast<const uint4*>(a.spans + base + 4u * tid));
 #pragma unroll 2
     for (int g = 0; g < C::kIpt / 4; ++g) {
       const uint32_t l0 = 4u * (tid + g * C::kThreads);                   // four consecutive intervals of the tile
+      const uint4 d4 = dn;
+      if (g + 1 < C::kIpt / 4 && l0 + 4u * C::kThreads < count)
+        dn = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l0 + 4u * C::kThreads));
       if (l0 < count) {
-        const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans + base + l0));
         const uint32_t dd[4] = {d4.x, d4.y, d4.z, d4.w};
         uint32_t ss[4];
         place4(base + l0, a.round, a.tag, a.key, dd, off, a.chrom, ss);
