@@ -399,6 +399,28 @@ def test_mc_permute_b_other_shapes(n_b, n_chrom, max_len):
     _mc_b_case(a_s, a_e, b_s, b_e, off, 12, 3, 2, expect_fused=True)
 
 
+def test_mc_workspace_contents_do_not_matter():
+    """A workspace full of garbage, reused by calls of different sizes and kinds, gives the same integers."""
+    big = W.make_config(5, scale=0.03)
+    small = W.make_config(5, scale=0.01)
+    n_chrom = int(big.chrom_offsets.size - 1)
+    ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, big.n_a, big.n_b, n_chrom, 1), dtype=torch.uint8, device=DEV)
+    for fill, w, which, rounds in ((0xFF, big, 1, 3), (0xAB, small, 1, 4), (0x01, big, 0, 3), (0x80, small, 1, 2), (0x00, big, 1, 2)):
+        ws.fill_(fill)
+        obs, rc = bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, which, 9, 2, rounds,
+                                 workspace=ws)
+        sync()
+        o_obs, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, which, 9, 2, rounds)
+        assert int(host_u64(obs)[0]) == o_obs and np.array_equal(host_u64(rc), o_rc)
+    # back-to-back calls on one workspace without a fill in between
+    for _ in range(2):
+        obs, rc = bits.mc_rounds(dev(small.a_start), dev(small.a_end), dev(small.b_start), dev(small.b_end), small.chrom_offsets, 1,
+                                 9, 2, 3, workspace=ws)
+        sync()
+        _, o_rc = oracle.mc_rounds(small.a_start, small.a_end, small.b_start, small.b_end, small.chrom_offsets, 1, 9, 2, 3)
+        assert np.array_equal(host_u64(rc), o_rc)
+
+
 def test_mc_permute_b_symmetric_sort_free_variant():
     """count(A, B') = count(B', A) -- the fresh B intervals searched against the sorted A."""
     bits.set_option("mc_symmetric", 1)
