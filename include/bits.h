@@ -102,6 +102,14 @@ int bits_count(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
                uint32_t flags, void* workspace, size_t workspace_bytes,
                uint64_t* total_out, void* stream);
 
+/* Decision problem (PAPER.md:47, sub-problem 1; :91): *any_out = 1 if at least one interval of A
+ * intersects an interval of B, else 0 (dev uint32[1]).  Same inputs, workspace (BITS_FN_COUNT) and
+ * flags as bits_count; the search stops early once an intersection is found. */
+int bits_decide(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                uint32_t flags, void* workspace, size_t workspace_bytes,
+                uint32_t* any_out, void* stream);
+
 /* Per-interval counting (Algorithm 1):
  *   counts_out[i] = c(a_i), in A's input order (dev uint32[n_a]);
  *   *total_out = sum_i c(a_i) (dev uint64[1]; may be NULL). */

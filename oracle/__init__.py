@@ -101,6 +101,14 @@ def count(a_start, a_end, b_start, b_end) -> int:
     return count_per_interval(a_start, a_end, b_start, b_end, want_counts=False)[0]
 
 
+def decide(a_start, a_end, b_start, b_end) -> bool:
+    """Decision problem (sub-problem 1): does at least one interval of A intersect one of B?
+    Answered the way PAPER.md:91 states it -- from the sizes |I(B, a_i)|: true iff some per-interval
+    count is non-zero.  Pinned by brute force from the closed predicate (tests/test_oracle_pins.py)."""
+    _, counts = count_per_interval(a_start, a_end, b_start, b_end, want_counts=True)
+    return bool(np.any(counts != 0))
+
+
 def place_from_bits(x: int, d: int, chrom_offsets) -> int:
     off, offp = _a32(chrom_offsets)
     s = C.c_uint32(0)

@@ -32,6 +32,7 @@ _SIGNATURES = {
     "bits_host_staging_bytes": (C.c_size_t, [C.c_int, C.c_uint64, C.c_uint64, C.c_uint32]),
     "bits_count": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t,
                              _u64p, _vp]),
+    "bits_decide": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t, _u32p, _vp]),
     "bits_count_per_interval": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp,
                                           C.c_size_t, _u32p, _u64p, _vp]),
     "bits_mc_rounds": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, _u32p, C.c_uint32, C.c_int,
@@ -182,6 +183,18 @@ def count(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None, total_
     _chk(lib().bits_count(_dev_u32(a_start, "a_start"), _dev_u32(a_end, "a_end"), n_a,
                           _dev_u32(b_start, "b_start"), _dev_u32(b_end, "b_end"), n_b, flags,
                           ws.data_ptr(), ws.numel(), out.data_ptr(), _stream()))
+    return out
+
+
+def decide(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None) -> torch.Tensor:
+    """bits_decide -> device int32[1] tensor: 1 if some interval of A intersects one of B (valid after stream sync)."""
+    dev = a_start.device
+    n_a, n_b = a_start.numel(), b_start.numel()
+    ws = _workspace(workspace_bytes(FN_COUNT, n_a, n_b, 0, 0, flags), workspace, dev)
+    out = torch.empty(1, dtype=torch.int32, device=dev)
+    _chk(lib().bits_decide(_dev_u32(a_start, "a_start"), _dev_u32(a_end, "a_end"), n_a,
+                           _dev_u32(b_start, "b_start"), _dev_u32(b_end, "b_end"), n_b, flags,
+                           ws.data_ptr(), ws.numel(), out.data_ptr(), _stream()))
     return out
 
 

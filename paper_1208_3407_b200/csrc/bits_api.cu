@@ -903,6 +903,27 @@ int bits_count(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, con
                     nullptr, total_out, static_cast<cudaStream_t>(stream));
 }
 
+int bits_decide(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* workspace, size_t workspace_bytes,
+                uint32_t* any_out, void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (!any_out) return BITS_ERR_NULL;
+  const Layout L = make_layout(workspace, BITS_FN_COUNT, n_a, n_b, 0, 0);
+  if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
+  if (flags & BITS_VALIDATE)
+    BITS_TRY(validate_inputs(a_start, a_end, (uint32_t)n_a, b_start, b_end, (uint32_t)n_b, L.small.bad, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(any_out, 0, sizeof(uint32_t), st));
+  if (n_a == 0 || n_b == 0) return BITS_OK;
+  uint32_t epoch = 1;
+  BITS_TRY(reset_sort_ctx(L.b, st));
+  BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
+  ProfScope prof(kClsCount, st);
+  decide_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), sorted_set(L.b, 1), any_out);
+  BITS_LAUNCH_CHECK();
+  return BITS_OK;
+}
+
 int bits_count_per_interval(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
                             const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* workspace,
                             size_t workspace_bytes, uint32_t* counts_out, uint64_t* total_out, void* stream) {

@@ -233,6 +233,18 @@ __global__ void __launch_bounds__(256) count_kernel(const uint32_t* __restrict__
 }
 
 // ---------------------------------------------------------------------------------------------
+// Decision problem (PAPER.md:47, sub-problem 1; :91 "with the size of I(B, a_i) we can directly answer
+// the decision problem"): *any = 1 iff some a in A has c(a) > 0.  Same look-ups as the count kernel;
+// a block stops as soon as anybody has found an intersection.  *any is zero on entry.
+__global__ void __launch_bounds__(256) decide_kernel(const uint32_t* __restrict__ a_start, const uint32_t* __restrict__ a_end,
+                                                     uint32_t n_a, SortedSet bs, SortedSet be, uint32_t* any) {
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_a; i += (uint64_t)gridDim.x * blockDim.x) {
+    if (*reinterpret_cast<volatile uint32_t*>(any)) return;
+    if (icount(bs, be, a_start[i], a_end[i]) != 0) { *any = 1u; return; }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Plain rank look-ups for SORTED queries (the per-round search when B is re-placed: A's ends and
 // A's starts are sorted once per call, so neighbouring threads walk neighbouring keys and the
 // probes coalesce).  sum_first = sum_q #{keys <= q};  sum_last = sum_q #{keys < q}.

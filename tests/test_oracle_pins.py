@@ -354,3 +354,17 @@ def test_pvalue():
     assert oracle.pvalue(2, [1, 2, 3, 2], 0) == 4 / 5
     assert oracle.pvalue(2, [1, 2, 3, 2], 1) == 4 / 5
     assert oracle.pvalue(0, [5] * 99, 1) == 1 / 100
+
+
+def test_decide_equals_brute_force_existence():
+    """PAPER.md:47 decision sub-problem against the closed predicate written out."""
+    rng = np.random.default_rng(77)
+    for trial in range(60):
+        n_a, n_b = int(rng.integers(0, 12)), int(rng.integers(0, 12))
+        a_s = rng.integers(0, 400, n_a); a_e = a_s + rng.integers(0, 15, n_a)
+        b_s = rng.integers(0, 400, n_b); b_e = b_s + rng.integers(0, 15, n_b)
+        want = any(a_s[i] <= b_e[j] and a_e[i] >= b_s[j] for i in range(n_a) for j in range(n_b))
+        assert oracle.decide(a_s, a_e, b_s, b_e) == want
+    assert oracle.decide([10], [20], [20], [30]) is True          # shared end point: closed intervals meet
+    assert oracle.decide([10], [20], [21], [30]) is False
+    assert oracle.decide([], [], [1], [2]) is False

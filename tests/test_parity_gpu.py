@@ -221,6 +221,26 @@ def test_count_search_design_variants(variant):
         bits.set_option("search_variant", 0)
 
 
+def test_decide_matches_oracle():
+    """bits_decide (PAPER.md:47 sub-problem 1): 1 iff some interval of A meets one of B."""
+    rng = np.random.default_rng(3)
+    cases = [([10], [20], [20], [30]), ([10], [20], [21], [30]), ([], [], [1], [2]), ([5], [6], [], [])]
+    for _ in range(6):                                   # sparse sets: some meet, some do not
+        n_a, n_b = int(rng.integers(1, 2000)), int(rng.integers(1, 2000))
+        a_s = rng.integers(0, 2**31, n_a); b_s = rng.integers(0, 2**31, n_b)
+        cases.append((a_s, a_s + rng.integers(0, 40000, n_a), b_s, b_s + rng.integers(0, 40000, n_b)))
+    w = W.make_config(2, scale=0.05)
+    cases.append((w.a_start, w.a_end, w.b_start, w.b_end))
+    seen = set()
+    for a_s, a_e, b_s, b_e in cases:
+        got = bits.decide(dev(a_s), dev(a_e), dev(b_s), dev(b_e))
+        sync()
+        want = oracle.decide(a_s, a_e, b_s, b_e)
+        assert bool(got.cpu().numpy()[0]) == want
+        seen.add(want)
+    assert seen == {True, False}
+
+
 def test_count_config4_full_size():
     w = W.make_config(4)
     total = check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
