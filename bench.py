@@ -271,6 +271,13 @@ def secondary_workloads(device, peak_gbs):
     ws = torch.empty(bits.workspace_bytes(bits.FN_COUNT_PER_INTERVAL, w.n_a, w.n_b), dtype=torch.uint8, device=device)
     med, mn = time_device(lambda: bits.count_per_interval(*d, workspace=ws), 10)
     out["cfg2_genome_count_1M"] = {"intervals_searched_per_s": w.n_a / (med * 1e-3), "ms_median": med, "ms_min": mn}
+    # decision and enumeration on the same sets
+    ws = torch.empty(bits.workspace_bytes(bits.FN_ENUMERATE, w.n_a, w.n_b), dtype=torch.uint8, device=device)
+    n_pairs = bits.enumerate_pairs(*d, workspace=ws)[2]
+    med, mn = time_device(lambda: bits.enumerate_pairs(*d, workspace=ws), 5)      # two calls inside: size, then emit
+    out["cfg2_enumerate"] = {"pairs": n_pairs, "pairs_per_s": n_pairs / (med * 1e-3), "ms_median": med, "ms_min": mn}
+    med, mn = time_device(lambda: bits.decide(*d), 5)
+    out["cfg2_decide"] = {"ms_median": med, "ms_min": mn}
     return out
 
 

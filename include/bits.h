@@ -72,7 +72,8 @@ enum {
   BITS_FN_COUNT_PER_INTERVAL = 1,
   BITS_FN_MC_ROUNDS = 2,
   BITS_FN_PLACE = 3,
-  BITS_FN_SORT = 4
+  BITS_FN_SORT = 4,
+  BITS_FN_ENUMERATE = 5
 };
 
 /* Bytes of device workspace `fn` needs for these sizes (device-pointer entry points).
@@ -109,6 +110,21 @@ int bits_decide(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
                 const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
                 uint32_t flags, void* workspace, size_t workspace_bytes,
                 uint32_t* any_out, void* stream);
+
+/* Enumeration (PAPER.md:47, sub-problem 4; :91: the count |I(B, a_i)| is the termination condition of the
+ * walk): every pair <a_i, b_j> with a_i.start <= b_j.end and a_i.end >= b_j.start, as indices into the
+ * caller's arrays.  The pairs of a_i occupy positions [offset_i, offset_i + c(a_i)) of pair_a_out /
+ * pair_b_out (offset = exclusive prefix of the per-interval counts in A's input order; pair_a_out holds
+ * i there); inside one a_i the order of the b_j is unspecified.  capacity = elements of each output
+ * array (dev uint32[capacity]); pairs at positions >= capacity are not written, *total_out (dev
+ * uint64[1]) is the full count either way, so a first call with capacity 0 sizes the arrays.
+ * BITS_B_SORTED is rejected (BITS_ERR_FLAGS): independently sorted arrays no longer pair starts with ends.
+ * Workspace: bits_workspace_bytes(BITS_FN_ENUMERATE, n_a, n_b, 0, 0, flags). */
+int bits_enumerate(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                   const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                   uint32_t flags, void* workspace, size_t workspace_bytes,
+                   uint32_t* pair_a_out, uint32_t* pair_b_out, uint64_t capacity,
+                   uint64_t* total_out, void* stream);
 
 /* Per-interval counting (Algorithm 1):
  *   counts_out[i] = c(a_i), in A's input order (dev uint32[n_a]);

@@ -109,6 +109,19 @@ def decide(a_start, a_end, b_start, b_end) -> bool:
     return bool(np.any(counts != 0))
 
 
+def enumerate_pairs(a_start, a_end, b_start, b_end):
+    """Enumeration problem (sub-problem 4): the set I(A, B) itself, straight from the closed
+    predicate a.start <= b.end and a.end >= b.start, as an (n, 2) int64 array of
+    (index in A, index in B) sorted lexicographically.  O(|A| * |B|): for small inputs only."""
+    a_s = np.asarray(a_start, dtype=np.int64); a_e = np.asarray(a_end, dtype=np.int64)
+    b_s = np.asarray(b_start, dtype=np.int64); b_e = np.asarray(b_end, dtype=np.int64)
+    out = []
+    for i in range(a_s.size):
+        j = np.nonzero((a_s[i] <= b_e) & (a_e[i] >= b_s))[0]
+        out.append(np.stack([np.full(j.size, i, dtype=np.int64), j.astype(np.int64)], axis=1))
+    return np.concatenate(out, axis=0) if out else np.zeros((0, 2), dtype=np.int64)
+
+
 def place_from_bits(x: int, d: int, chrom_offsets) -> int:
     off, offp = _a32(chrom_offsets)
     s = C.c_uint32(0)

@@ -21,7 +21,7 @@ from . import build as _build
 
 PERMUTE_A, PERMUTE_B = 0, 1
 B_SORTED, VALIDATE = 1, 2
-FN_COUNT, FN_COUNT_PER_INTERVAL, FN_MC_ROUNDS, FN_PLACE, FN_SORT = 0, 1, 2, 3, 4
+FN_COUNT, FN_COUNT_PER_INTERVAL, FN_MC_ROUNDS, FN_PLACE, FN_SORT, FN_ENUMERATE = 0, 1, 2, 3, 4, 5
 
 _u32p, _u64p, _vp = C.c_void_p, C.c_void_p, C.c_void_p   # raw addresses (host or device)
 _lib = None
@@ -33,6 +33,8 @@ _SIGNATURES = {
     "bits_count": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t,
                              _u64p, _vp]),
     "bits_decide": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t, _u32p, _vp]),
+    "bits_enumerate": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t, _u32p, _u32p,
+                                 C.c_uint64, _u64p, _vp]),
     "bits_count_per_interval": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp,
                                           C.c_size_t, _u32p, _u64p, _vp]),
     "bits_mc_rounds": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, _u32p, C.c_uint32, C.c_int,
@@ -196,6 +198,24 @@ def decide(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None) -> to
                            _dev_u32(b_start, "b_start"), _dev_u32(b_end, "b_end"), n_b, flags,
                            ws.data_ptr(), ws.numel(), out.data_ptr(), _stream()))
     return out
+
+
+def enumerate_pairs(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None):
+    """bits_enumerate -> (pair_a, pair_b, total): every intersecting pair as indices into A and B (device int32-typed
+    uint32 tensors of `total` elements).  Two calls: the first (capacity 0) sizes the outputs; synchronises once."""
+    dev = a_start.device
+    n_a, n_b = a_start.numel(), b_start.numel()
+    ws = _workspace(workspace_bytes(FN_ENUMERATE, n_a, n_b, 0, 0, flags), workspace, dev)
+    total = torch.zeros(1, dtype=torch.int64, device=dev)
+    args = (_dev_u32(a_start, "a_start"), _dev_u32(a_end, "a_end"), n_a, _dev_u32(b_start, "b_start"), _dev_u32(b_end, "b_end"), n_b,
+            flags, ws.data_ptr(), ws.numel())
+    _chk(lib().bits_enumerate(*args, 0, 0, 0, total.data_ptr(), _stream()))
+    n = int(total.item())
+    pa = torch.empty(n, dtype=torch.int32, device=dev)
+    pb = torch.empty(n, dtype=torch.int32, device=dev)
+    if n:
+        _chk(lib().bits_enumerate(*args, pa.data_ptr(), pb.data_ptr(), n, total.data_ptr(), _stream()))
+    return pa, pb, n
 
 
 def count_per_interval(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None, counts_out=None,

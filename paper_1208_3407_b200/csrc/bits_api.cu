@@ -13,6 +13,7 @@
 #include "msd_sort.cuh"
 #include "mc_tile.cuh"
 #include "search.cuh"
+#include "enumerate.cuh"
 
 namespace bits {
 
@@ -164,6 +165,13 @@ struct Layout {
   uint32_t* cross_keys = nullptr;        // [kMaxBins * kCrossCap]
   uint32_t* qb[2] = {nullptr, nullptr};
   uint32_t* round_flags = nullptr;       // uint32[kFlagChunk]
+  // enumeration (enumerate.cuh)
+  uint32_t* e_counts = nullptr;                  // [n_a]
+  unsigned long long* e_offsets = nullptr;       // [n_a]
+  unsigned long long* e_tile_sums = nullptr;     // [ceil(n_a / kScanTile) + 1]
+  uint32_t* e_tie = nullptr;                     // [n_b + 1]
+  uint32_t* e_end_by_start = nullptr;            // [n_b]
+  uint32_t* e_idx_by_start = nullptr;            // [n_b]
   size_t bytes = 0;
 };
 constexpr uint32_t kFlagChunk = 4096;    // fused rounds are checked for raised flags in chunks of this many
@@ -210,6 +218,15 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
           L.round_flags = c.take<uint32_t>(kFlagChunk);
         }
       }
+      break;
+    case BITS_FN_ENUMERATE:
+      L.b.carve(c, n_b, true);
+      L.e_counts = c.take<uint32_t>(n_a + 4);
+      L.e_offsets = c.take<unsigned long long>(n_a + 4);
+      L.e_tile_sums = c.take<unsigned long long>(ceil_div(n_a, (uint64_t)enu::kScanTile) + 4);
+      L.e_tie = c.take<uint32_t>(n_b + 4);
+      L.e_end_by_start = c.take<uint32_t>(n_b + 4);
+      L.e_idx_by_start = c.take<uint32_t>(n_b + 4);
       break;
     case BITS_FN_PLACE:
       break;
@@ -875,7 +892,7 @@ extern "C" {
 
 size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which, uint32_t flags) {
   (void)flags;
-  if (fn < BITS_FN_COUNT || fn > BITS_FN_SORT) return 0;
+  if (fn < BITS_FN_COUNT || fn > BITS_FN_ENUMERATE) return 0;
   if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return 0;
   return make_layout(nullptr, fn, n_a, n_b, n_chrom, which).bytes;
 }
@@ -920,6 +937,43 @@ int bits_decide(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, co
   BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
   ProfScope prof(kClsCount, st);
   decide_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), sorted_set(L.b, 1), any_out);
+  BITS_LAUNCH_CHECK();
+  return BITS_OK;
+}
+
+int bits_enumerate(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                   const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* workspace, size_t workspace_bytes,
+                   uint32_t* pair_a_out, uint32_t* pair_b_out, uint64_t capacity, uint64_t* total_out, void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (!total_out || (capacity && (!pair_a_out || !pair_b_out))) return BITS_ERR_NULL;
+  if (flags & BITS_B_SORTED) return BITS_ERR_FLAGS;   // independently sorted arrays have lost which end belongs to which start
+  const Layout L = make_layout(workspace, BITS_FN_ENUMERATE, n_a, n_b, 0, 0);
+  if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
+  if (flags & BITS_VALIDATE)
+    BITS_TRY(validate_inputs(a_start, a_end, (uint32_t)n_a, b_start, b_end, (uint32_t)n_b, L.small.bad, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(total_out, 0, sizeof(uint64_t), st));
+  if (n_a == 0 || n_b == 0) return BITS_OK;
+  uint32_t epoch = 1;
+  BITS_TRY(reset_sort_ctx(L.b, st));
+  BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
+  // per-interval counts (the termination condition), their exclusive scan, B's ends and indices in start order
+  BITS_TRY(launch_count(a_start, a_end, (uint32_t)n_a, L.b, L.e_counts, nullptr, st));
+  const uint32_t n_tiles = (uint32_t)ceil_div(n_a, (uint64_t)enu::kScanTile);
+  ProfScope prof(kClsOther, st);
+  enu::scan_tile_sums_kernel<<<n_tiles, enu::kScanThreads, 0, st>>>(L.e_counts, (uint32_t)n_a, L.e_tile_sums);
+  BITS_LAUNCH_CHECK();
+  enu::scan_tile_prefix_kernel<<<1, 1024, 0, st>>>(L.e_tile_sums, n_tiles, reinterpret_cast<unsigned long long*>(total_out));
+  BITS_LAUNCH_CHECK();
+  enu::scan_apply_kernel<<<n_tiles, enu::kScanThreads, 0, st>>>(L.e_counts, (uint32_t)n_a, L.e_tile_sums, L.e_offsets);
+  BITS_LAUNCH_CHECK();
+  if (capacity == 0) return BITS_OK;
+  BITS_CUDA_TRY(cudaMemsetAsync(L.e_tie, 0, sizeof(uint32_t) * ((size_t)n_b + 1), st));
+  enu::start_order_kernel<<<grid_for(n_b, 256), 256, 0, st>>>(b_start, b_end, (uint32_t)n_b, sorted_set(L.b, 0), L.e_tie,
+                                                              L.e_end_by_start, L.e_idx_by_start);
+  BITS_LAUNCH_CHECK();
+  enu::emit_pairs_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), L.e_counts, L.e_offsets,
+                                                             L.e_end_by_start, L.e_idx_by_start, pair_a_out, pair_b_out, capacity);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }

@@ -368,3 +368,17 @@ def test_decide_equals_brute_force_existence():
     assert oracle.decide([10], [20], [20], [30]) is True          # shared end point: closed intervals meet
     assert oracle.decide([10], [20], [21], [30]) is False
     assert oracle.decide([], [], [1], [2]) is False
+
+
+def test_enumerate_pairs_agrees_with_counts_and_a_worked_example():
+    """PAPER.md:47 enumeration: the pair set has c(a_i) pairs per a_i (the BITS counts) and matches a hand-made case
+    with containment (Fig. 1B situation)."""
+    a = ([5, 100], [9, 100])
+    b = ([0, 6, 9, 10, 50], [200, 7, 9, 12, 60])               # [0,200] contains everything
+    assert oracle.enumerate_pairs(*a, *b).tolist() == [[0, 0], [0, 1], [0, 2], [1, 0]]
+    rng = np.random.default_rng(5)
+    a_s = rng.integers(0, 5000, 300); a_e = a_s + rng.integers(0, 200, 300)
+    b_s = rng.integers(0, 5000, 400); b_e = b_s + rng.integers(0, 900, 400)
+    pairs = oracle.enumerate_pairs(a_s, a_e, b_s, b_e)
+    total, counts = oracle.count_per_interval(a_s, a_e, b_s, b_e)
+    assert len(pairs) == total and np.array_equal(np.bincount(pairs[:, 0], minlength=300), counts)

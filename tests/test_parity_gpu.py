@@ -241,6 +241,46 @@ def test_decide_matches_oracle():
     assert seen == {True, False}
 
 
+def _enumerated(a_s, a_e, b_s, b_e):
+    pa, pb, n = bits.enumerate_pairs(dev(a_s), dev(a_e), dev(b_s), dev(b_e))
+    sync()
+    got = np.stack([host_u32(pa).astype(np.int64), host_u32(pb).astype(np.int64)], axis=1) if n else np.zeros((0, 2), dtype=np.int64)
+    return got[np.lexsort((got[:, 1], got[:, 0]))]
+
+
+def test_enumerate_small_sets_equal_the_definition():
+    """bits_enumerate (PAPER.md:47 sub-problem 4): the emitted set of pairs is exactly I(A, B)."""
+    rng = np.random.default_rng(21)
+    w = W.make_config(1)
+    cases = [(w.a_start, w.a_end, w.b_start, w.b_end), ([10], [20], [20, 21, 0, 0], [30, 30, 10, 9]), ([], [], [1], [2]), ([1], [2], [], [])]
+    for n_a, n_b, span in ((700, 3000, 3000), (2500, 900, 50), (300, 5000, 200_000)):
+        a_s = rng.integers(0, 1_000_000, n_a); b_s = rng.integers(0, 1_000_000, n_b)
+        cases.append((a_s, a_s + rng.integers(0, span, n_a), b_s, b_s + rng.integers(0, span, n_b)))
+    b_s = rng.integers(0, 50, 4000)                       # many equal starts, long and short intervals mixed (containment)
+    cases.append((rng.integers(0, 60, 500), rng.integers(60, 90, 500), b_s, b_s + rng.integers(0, 40, 4000)))
+    for a_s, a_e, b_s, b_e in cases:
+        want = oracle.enumerate_pairs(a_s, a_e, b_s, b_e)
+        got = _enumerated(a_s, a_e, b_s, b_e)
+        assert got.shape == want.shape and np.array_equal(got, want)
+
+
+def test_enumerate_config2_is_valid_and_complete():
+    """At a size the definition is too slow for: every emitted pair intersects, no pair twice, and every
+    a_i has exactly c(a_i) pairs in its own slice of the output -- together that is the set I(A, B)."""
+    w = W.make_config(2, scale=0.3)
+    pa, pb, n = bits.enumerate_pairs(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end))
+    sync()
+    pa, pb = host_u32(pa).astype(np.int64), host_u32(pb).astype(np.int64)
+    o_total, o_counts = oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end)
+    assert n == o_total
+    a_s, a_e = w.a_start.astype(np.int64), w.a_end.astype(np.int64)
+    b_s, b_e = w.b_start.astype(np.int64), w.b_end.astype(np.int64)
+    assert np.all((a_s[pa] <= b_e[pb]) & (a_e[pa] >= b_s[pb]))
+    assert np.array_equal(np.bincount(pa, minlength=w.n_a), o_counts)
+    assert np.all(np.diff(pa) >= 0)                        # A-major order: slices by exclusive prefix of the counts
+    assert np.unique(pa * (1 << 32) + pb).size == n
+
+
 def test_count_config4_full_size():
     w = W.make_config(4)
     total = check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
