@@ -194,6 +194,12 @@ int bits_mc_rounds_host(const uint32_t* a_start, const uint32_t* a_end, uint64_t
  * Returns NaN for a bad tail or a NULL array with n_rounds > 0. */
 double bits_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n_rounds, int tail);
 
+/* Enrichment score of the paper's screen (Fig. 3 caption :224): log2 of the observed
+ * count over the MEDIAN count of the Monte Carlo rounds (host pointers).  Median of an even number of
+ * rounds = mean of the two middle order statistics.  Median 0: +inf if observed > 0, else NaN;
+ * observed 0 with a positive median: -inf.  NaN for n_rounds == 0 or a NULL array. */
+double bits_enrichment(uint64_t observed, const uint64_t* round_counts, uint32_t n_rounds);
+
 /* Kernels launched by this library in this process since load (for bench.py's gpu_launches). */
 uint64_t bits_launch_count(void);
 

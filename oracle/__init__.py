@@ -47,6 +47,8 @@ def lib():
                                        C.c_int, C.c_uint64, C.c_uint32, C.c_uint32, _u64p, _u64p]
         L.oracle_pvalue.argtypes = [C.c_uint64, _u64p, C.c_uint32, C.c_int]
         L.oracle_pvalue.restype = C.c_double
+        L.oracle_enrichment.argtypes = [C.c_uint64, _u64p, C.c_uint32]
+        L.oracle_enrichment.restype = C.c_double
         _lib = L
     return _lib
 
@@ -153,6 +155,11 @@ def mc_rounds(a_start, a_end, b_start, b_end, chrom_offsets, which: int, seed: i
                                 C.c_uint64(seed), C.c_uint32(round_begin), C.c_uint32(n_rounds),
                                 C.byref(obs), rc.ctypes.data_as(_u64p)))
     return int(obs.value), rc[:n_rounds]
+
+
+def enrichment(observed: int, round_counts) -> float:
+    rc = np.ascontiguousarray(round_counts, dtype=np.uint64)
+    return float(lib().oracle_enrichment(C.c_uint64(observed), rc.ctypes.data_as(_u64p), rc.size))
 
 
 def pvalue(observed: int, round_counts, tail: int = 0) -> float:

@@ -34,6 +34,8 @@
 // PARITY UNPINNED BY THE PAPER: per-round Monte Carlo counts (the paper prints no counts
 // and does not specify its RNG); pinned only by the procedure + brute force on config 1.
 #include <algorithm>
+#include <cmath>
+#include <limits>
 #include <cstdint>
 #include <cstring>
 #include <vector>
@@ -205,6 +207,19 @@ double oracle_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n
   for (uint32_t r = 0; r < n_rounds; ++r)
     k += (tail == 0) ? (round_counts[r] >= observed) : (round_counts[r] <= observed);
   return static_cast<double>(k + 1) / static_cast<double>(static_cast<uint64_t>(n_rounds) + 1);
+}
+
+// Enrichment score of the screen (Fig. 3 caption :224): log2(observed / median of the
+// round counts); median of an even number of rounds = mean of the two middle order statistics
+// (reading R13).  Median 0: +inf if observed > 0, else NaN.
+double oracle_enrichment(uint64_t observed, const uint64_t* round_counts, uint32_t n_rounds) {
+  if (n_rounds == 0) return std::nan("");
+  std::vector<uint64_t> v(round_counts, round_counts + n_rounds);
+  std::sort(v.begin(), v.end());
+  const double median = (n_rounds % 2) ? static_cast<double>(v[n_rounds / 2])
+                                       : (static_cast<double>(v[n_rounds / 2 - 1]) + static_cast<double>(v[n_rounds / 2])) / 2.0;
+  if (median == 0.0) return observed ? std::numeric_limits<double>::infinity() : std::nan("");
+  return std::log2(static_cast<double>(observed) / median);
 }
 
 }  // extern "C"

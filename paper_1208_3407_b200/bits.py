@@ -50,6 +50,7 @@ _SIGNATURES = {
                                       C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _vp, C.c_size_t, _u64p, _u64p,
                                       _vp]),
     "bits_pvalue": (C.c_double, [C.c_uint64, _u64p, C.c_uint32, C.c_int]),
+    "bits_enrichment": (C.c_double, [C.c_uint64, _u64p, C.c_uint32]),
     "bits_launch_count": (C.c_uint64, []),
     "bits_profile_read": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p]),
     "bits_set_option": (C.c_int, [C.c_char_p, C.c_int64]),
@@ -285,6 +286,36 @@ class McResult:
 def pvalue(observed: int, round_counts, tail: int = 0) -> float:
     rc = np.ascontiguousarray(round_counts, dtype=np.uint64)
     return float(lib().bits_pvalue(int(observed), rc.ctypes.data if rc.size else 0, rc.size, tail))
+
+
+def enrichment(observed: int, round_counts) -> float:
+    """bits_enrichment: log2(observed / median of the round counts)."""
+    rc = np.ascontiguousarray(round_counts, dtype=np.uint64)
+    return float(lib().bits_enrichment(int(observed), rc.ctypes.data if rc.size else 0, rc.size))
+
+
+def screen(tracks, chrom_offsets, seed: int, n_rounds: int, which: int = PERMUTE_A, round_begin: int = 0):
+    """The paper's co-localisation screen (Fig. 3): for every ordered pair (i, j) of the K
+    interval sets in `tracks` (each a (start, end) pair of device tensors) the observed count, `n_rounds`
+    Monte Carlo rounds and log2(observed / median).  Returns (observed int64[K, K], enrichment float64[K, K],
+    round_counts uint64[K, K, n_rounds]) as numpy arrays.  Marshalling only: every count comes from
+    bits_mc_rounds; one workspace sized for the largest pair is reused."""
+    K = len(tracks)
+    off = _offsets(chrom_offsets)
+    n_max = max(t[0].numel() for t in tracks)
+    dev = tracks[0][0].device
+    ws = torch.empty(max(workspace_bytes(FN_MC_ROUNDS, n_max, n_max, off.size - 1, which), 256), dtype=torch.uint8, device=dev)
+    obs = torch.empty((K, K), dtype=torch.int64, device=dev)
+    rc = torch.empty((K, K, n_rounds), dtype=torch.int64, device=dev)
+    for i in range(K):
+        for j in range(K):
+            mc_rounds(tracks[i][0], tracks[i][1], tracks[j][0], tracks[j][1], off, which, seed, round_begin, n_rounds,
+                      workspace=ws, observed_out=obs[i, j:j + 1], round_counts_out=rc[i, j])
+    torch.cuda.synchronize(dev)
+    obs_h = obs.cpu().numpy()
+    rc_h = rc.cpu().numpy().view(np.uint64)
+    enr = np.array([[enrichment(int(obs_h[i, j]), rc_h[i, j]) for j in range(K)] for i in range(K)], dtype=np.float64)
+    return obs_h, enr, rc_h
 
 
 def host_workspace(fn: int, n_a: int, n_b: int, n_chrom: int = 0, which: int = 0, n_rounds: int = 0,

@@ -4,6 +4,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "common.cuh"
@@ -1089,6 +1090,20 @@ double bits_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n_r
   for (uint32_t r = 0; r < n_rounds; ++r)
     k += tail == 0 ? (round_counts[r] >= observed) : (round_counts[r] <= observed);
   return (double)(k + 1) / (double)((uint64_t)n_rounds + 1);
+}
+
+double bits_enrichment(uint64_t observed, const uint64_t* round_counts, uint32_t n_rounds) {
+  if (n_rounds == 0 || !round_counts) return NAN;
+  std::vector<uint64_t> v(round_counts, round_counts + n_rounds);
+  const size_t m = n_rounds / 2;
+  std::nth_element(v.begin(), v.begin() + m, v.end());
+  double median = (double)v[m];
+  if ((n_rounds & 1u) == 0) {
+    const uint64_t lower = *std::max_element(v.begin(), v.begin() + m);   // the order statistic just below
+    median = ((double)lower + (double)v[m]) / 2.0;
+  }
+  if (median == 0.0) return observed ? INFINITY : NAN;
+  return log2((double)observed / median);
 }
 
 uint64_t bits_launch_count(void) { return g_launches; }

@@ -52,6 +52,20 @@ def test_workspace_sizes():
     assert bits.host_staging_bytes(bits.FN_MC_ROUNDS, 1000, 1000, 100) >= 4 * 4 * 1000 + 8 * 100
 
 
+def test_enrichment_matches_the_oracle_formula():
+    """bits_enrichment is host arithmetic on integers: it must equal the oracle's double bit for bit (tolerance 0;
+    both are log2 of one double division of the observed count by the median)."""
+    import math
+    import oracle
+    rng = np.random.default_rng(9)
+    for n in (1, 2, 3, 10, 999, 1000):
+        rc = rng.integers(0, 50_000, n).astype(np.uint64)
+        for obs in (0, 1, 777, 10**7):
+            a, b = bits.enrichment(obs, rc), oracle.enrichment(obs, rc)
+            assert (math.isnan(a) and math.isnan(b)) or a == b
+    assert math.isnan(bits.enrichment(5, [])) and bits.enrichment(3, [0, 0, 0]) == math.inf
+
+
 def test_pvalue():
     assert bits.pvalue(10, [], 0) == 1.0
     assert bits.pvalue(10, [1, 2, 3], 0) == 1 / 4

@@ -382,3 +382,16 @@ def test_enumerate_pairs_agrees_with_counts_and_a_worked_example():
     pairs = oracle.enumerate_pairs(a_s, a_e, b_s, b_e)
     total, counts = oracle.count_per_interval(a_s, a_e, b_s, b_e)
     assert len(pairs) == total and np.array_equal(np.bincount(pairs[:, 0], minlength=300), counts)
+
+
+def test_enrichment_score_closed_cases():
+    """log2(observed / median): odd and even numbers of rounds, zero cases."""
+    import math
+    assert oracle.enrichment(8, [1, 2, 3]) == 2.0                       # median 2
+    assert oracle.enrichment(5, [4, 1, 3, 2]) == 1.0                    # median (2 + 3) / 2 = 2.5
+    assert oracle.enrichment(1, [4, 4, 4, 4, 4]) == -2.0
+    assert oracle.enrichment(3, [0, 0, 0]) == math.inf and math.isnan(oracle.enrichment(0, [0, 0]))
+    assert oracle.enrichment(0, [2, 2]) == -math.inf and math.isnan(oracle.enrichment(5, []))
+    rng = np.random.default_rng(1)
+    x = rng.integers(1, 10**9, 1001)
+    assert oracle.enrichment(12345, x) == math.log2(12345 / float(np.median(x)))

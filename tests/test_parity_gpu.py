@@ -539,6 +539,28 @@ def test_mc_permute_b_leaves_sorted_arrays_of_last_round(k, scale, rounds):
     assert np.array_equal(host_u32(b_e), oracle.sort_u32(o_e))
 
 
+def test_screen_of_tracks_matches_oracle():
+    """The co-localisation screen: K x K observed counts, round counts and log2(observed / median)."""
+    rng = np.random.default_rng(31)
+    off = W.genome_offsets([3_000_000, 2_000_000, 1_200_000])
+    G = int(off[-1])
+    tracks = []
+    for n, max_len in ((4000, 400), (2500, 2000), (6000, 120)):
+        c = rng.integers(0, 3, n)
+        ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        s = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        tracks.append((s.astype(np.uint32), (s + ln - 1).astype(np.uint32)))
+    R = 21
+    obs, enr, rc = bits.screen([(dev(s), dev(e)) for s, e in tracks], off, 4, R)
+    for i in range(3):
+        for j in range(3):
+            o_obs, o_rc = oracle.mc_rounds(tracks[i][0], tracks[i][1], tracks[j][0], tracks[j][1], off, 0, 4, 0, R)
+            assert int(obs[i, j]) == o_obs and np.array_equal(rc[i, j], o_rc)
+            want = oracle.enrichment(o_obs, o_rc)
+            assert enr[i, j] == want or (np.isnan(enr[i, j]) and np.isnan(want))
+
+
 # ------------------------------------------------------------------------------------- host-buffer entry points
 def test_host_variants_config1():
     w = W.make_config(1)
