@@ -276,7 +276,7 @@ def secondary_workloads(device, peak_gbs):
     n_pairs = bits.enumerate_pairs(*d, workspace=ws)[2]
     med, mn = time_device(lambda: bits.enumerate_pairs(*d, workspace=ws), 5)      # two calls inside: size, then emit
     out["cfg2_enumerate"] = {"pairs": n_pairs, "pairs_per_s": n_pairs / (med * 1e-3), "ms_median": med, "ms_min": mn}
-    med, mn = time_device(lambda: bits.decide(*d), 5)
+    med, mn = time_device(lambda: bits.decide(*d, workspace=ws), 5)
     out["cfg2_decide"] = {"ms_median": med, "ms_min": mn}
     # the paper's screen on synthetic tracks (8 tracks of 1e5 intervals from config 2's recipe,
     # 64 ordered pairs x 1000 rounds, queries re-placed); wall clock, the enrichment scores are host arithmetic
