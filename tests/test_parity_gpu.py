@@ -561,6 +561,40 @@ def test_screen_of_tracks_matches_oracle():
             assert enr[i, j] == want or (np.isnan(enr[i, j]) and np.isnan(want))
 
 
+def test_cli_on_bed_files(tmp_path, capsys):
+    """The command line end to end on small BED files: counts, per-interval counts, pairs and Monte Carlo summary."""
+    from paper_1208_3407_b200 import cli, frontend as F
+    rng = np.random.default_rng(12)
+    (tmp_path / "g.txt").write_text("chr1 50000\nchr2 30000\nchr3 20000\n")
+    names, lens = ["chr1", "chr2", "chr3"], [50000, 30000, 20000]
+    def bed(n, max_len):
+        out = []
+        for _ in range(n):
+            c = int(rng.integers(0, 3)); ln = int(rng.integers(1, max_len)); s = int(rng.integers(0, lens[c] - ln))
+            out.append(f"{names[c]}\t{s}\t{s + ln}\n")
+        return "".join(out)
+    (tmp_path / "a.bed").write_text(bed(400, 300))
+    (tmp_path / "b.bed").write_text("track x\n" + bed(900, 600))
+    base = ["-a", str(tmp_path / "a.bed"), "-b", str(tmp_path / "b.bed"), "-g", str(tmp_path / "g.txt")]
+    g = F.read_genome(str(tmp_path / "g.txt"))
+    a_s, a_e = F.read_bed(str(tmp_path / "a.bed"), g)
+    b_s, b_e = F.read_bed(str(tmp_path / "b.bed"), g)
+    total, counts = oracle.count_per_interval(a_s, a_e, b_s, b_e)
+    assert cli.main(["count"] + base) == 0 and int(capsys.readouterr().out) == total
+    assert cli.main(["per-interval"] + base) == 0 and list(map(int, capsys.readouterr().out.split())) == counts.tolist()
+    assert cli.main(["decide"] + base) == 0 and int(capsys.readouterr().out) == int(total > 0)
+    assert cli.main(["enumerate"] + base) == 0
+    pairs = sorted(tuple(map(int, l.split())) for l in capsys.readouterr().out.splitlines())
+    assert pairs == [tuple(p) for p in oracle.enumerate_pairs(a_s, a_e, b_s, b_e).tolist()]
+    for permute, which in (("a", 0), ("b", 1)):
+        assert cli.main(["mc"] + base + ["-n", "25", "--permute", permute, "--seed", "3"]) == 0
+        out = dict(l.split("\t") for l in capsys.readouterr().out.splitlines())
+        o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, g.offsets, which, 3, 0, 25)
+        assert int(out["observed"]) == o_obs and float(out["p_enrichment"]) == oracle.pvalue(o_obs, o_rc, 0)
+        assert float(out["log2_observed_over_median"]) == oracle.enrichment(o_obs, o_rc)
+    assert cli.main(["count", "-a", str(tmp_path / "nope.bed"), "-b", str(tmp_path / "b.bed"), "-g", str(tmp_path / "g.txt")]) == 2
+
+
 # ------------------------------------------------------------------------------------- host-buffer entry points
 def test_host_variants_config1():
     w = W.make_config(1)
