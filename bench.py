@@ -126,7 +126,7 @@ def config_block(w, rounds: int, n_gpus: int) -> dict:
             "rounds_per_step": rounds, "which": {0: "permute_A", 1: "permute_B", None: "count"}[w.which],
             "mc_seed": w.mc_seed, "data_seed": w.spec.get("seed"), "scale": w.spec.get("scale", 1.0),
             "parallelism": f"rounds sharded over {n_gpus} GPU(s), no collective",
-            "l2": "no flush: every round re-writes and re-sorts 160 MB of keys plus 160 MB of ping-pong buffers (> 126 MB L2)"}
+            "l2": "no flush: inputs larger than L2 -- every round streams 40 MB of spans, 80 MB of pairs and 80 MB of sorted keys (200 MB > 126 MB L2)"}
 
 
 # ------------------------------------------------------------------------------------------ reference arm
