@@ -329,7 +329,7 @@ __device__ __forceinline__ void scan_cursors(uint16_t* cur_s, uint16_t* cur_e, u
 // barrier) stored at the slot its sub-bucket's cursor hands out.  With kCheckBin, entries whose
 // bin is not d are dropped.  Ends with a barrier; afterwards buf[0..valid) is ordered by
 // sub-bucket and cur[kFront + sb] is the END of sub-bucket sb.
-template <class C, bool kCheckBin>
+template <class C, bool kCheckBin, bool kTrailingBarrier = true>
 __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint32_t mask,
                                                  uint32_t sshift, uint16_t* cur) {
   const int tid = threadIdx.x;
@@ -355,7 +355,7 @@ __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint
     for (int j = j0; j < j0 + 4; ++j)
       if (slot[j - j0] != 0xffffffffu) buf[slot[j - j0]] = key[j];
   }
-  __syncthreads();
+  if (kTrailingBarrier) __syncthreads();
 }
 
 // Write buf[0..mv) (ordered by sub-bucket) to dst[gbase ..] in ascending order: the keys that
@@ -492,10 +492,11 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     uint32_t total[2];
     scan_cursors<C>(s_cur_s, s_cur_e, s_w, total);                         // barriers inside
     // starts: all np keys belong to bin d; the bin begins at gbase in B_S
-    scatter_in_place<C, false>(s_ks, np, d, shift, mask, sshift, s_cur_s);
+    // (both scatters first: the two long write-out phases then follow each other with no barrier between them)
+    scatter_in_place<C, false, false>(s_ks, np, d, shift, mask, sshift, s_cur_s);   // (the barriers of the next call cover it)
+    scatter_in_place<C, true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
     qsum += write_and_rank<C, false>(s_ks, np, mask, sshift, s_cur_s, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0);
     // ends: n_in ends of earlier pairs lie in this bin, so it begins at gbase - n_in in B_E
-    scatter_in_place<C, true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
     qsum -= write_and_rank<C, true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
     d = d_next;
   }
