@@ -359,7 +359,7 @@ __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint
 }
 
 // Write buf[0..mv) (ordered by sub-bucket) to dst[gbase ..] in ascending order: the keys that
-// share a sub-bucket are ordered by comparison counting (ties by position), the first four
+// share a sub-bucket are ordered by comparison counting (ties by position), the first three
 // candidates without a loop.  Then rank the sorted queries q_sorted[qlo..qhi), all of which fall
 // into this bin's key range: every key of an earlier sub-bucket is smaller, the count is finished
 // inside the query's own sub-bucket.  Returns this thread's sum of query ranks.
@@ -375,14 +375,14 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
     const uint32_t lo = cur[kFront - 1 + sb], hi = cur[kFront + sb];
     uint32_t rank = 0;
 #pragma unroll
-    for (uint32_t i = 0; i < 4; ++i) {
+    for (uint32_t i = 0; i < 3; ++i) {
       const uint32_t t = lo + i;
       const uint32_t kk = buf[t];                    // buf is padded: t < C::kCap + 4
       rank += (t < hi) & (kk < k + (t < p ? 1u : 0u));
     }
-    if (hi - lo > 4) {
+    if (hi - lo > 3) {
 #pragma unroll 1
-      for (uint32_t t = lo + 4; t < hi; ++t) rank += buf[t] < k + (t < p ? 1u : 0u);
+      for (uint32_t t = lo + 3; t < hi; ++t) rank += buf[t] < k + (t < p ? 1u : 0u);
     }
     dst[gbase + lo + rank] = k;
   }
