@@ -238,9 +238,16 @@ __global__ void __launch_bounds__(256) count_kernel(const uint32_t* __restrict__
 // a block stops as soon as anybody has found an intersection.  *any is zero on entry.
 __global__ void __launch_bounds__(256) decide_kernel(const uint32_t* __restrict__ a_start, const uint32_t* __restrict__ a_end,
                                                      uint32_t n_a, SortedSet bs, SortedSet be, uint32_t* any) {
-  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_a; i += (uint64_t)gridDim.x * blockDim.x) {
+  // (whole warps iterate together; one lane reports for the warp, and only if nobody has yet: a store
+  // from every thread that finds an intersection would serialise on the one word)
+  const uint64_t n_pad = ((uint64_t)n_a + 31) & ~31ull;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pad; i += (uint64_t)gridDim.x * blockDim.x) {
     if (*reinterpret_cast<volatile uint32_t*>(any)) return;
-    if (icount(bs, be, a_start[i], a_end[i]) != 0) { *any = 1u; return; }
+    const bool hit = i < n_a && icount(bs, be, a_start[i], a_end[i]) != 0;
+    if (__any_sync(kFullMask, hit)) {
+      if ((threadIdx.x & 31) == 0) *any = 1u;
+      return;
+    }
   }
 }
 
