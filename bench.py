@@ -37,8 +37,8 @@ if ROOT not in sys.path:
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
 NCU_TRAFFIC_BYTES: dict = {
     # profiles/r1b_fused_ncu_full_summary.txt (config 5, one launch)
-    "bin_sort_search_kernel": 127_939_072,     # 89.93 MB read + 38.01 MB written
-    "place_tile_kernel": 65_654_272,           # 40.10 MB read + 25.55 MB written
+    "bin_sort_search_kernel": 127_229_184,     # 89.93 MB read + 37.30 MB written
+    "place_tile_kernel": 66_431_232,           # 40.11 MB read + 26.33 MB written
 }
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
