@@ -459,6 +459,12 @@ def test_mc_permute_b_other_shapes(n_b, n_chrom, max_len):
     _mc_b_case(a_s, a_e, b_s, b_e, off, 12, 3, 2, expect_fused=True)
 
 
+def test_mc_permute_b_many_rounds_back_to_back():
+    """120 fused rounds in one call (programmatic dependent launches, buffers reused by parity): every round's count."""
+    w = W.make_config(5, scale=0.03)
+    _mc_b_case(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 17, 1000, 120, expect_fused=True)
+
+
 def test_mc_workspace_contents_do_not_matter():
     """A workspace full of garbage, reused by calls of different sizes and kinds, gives the same integers."""
     big = W.make_config(5, scale=0.03)
