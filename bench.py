@@ -40,6 +40,13 @@ NCU_TRAFFIC_BYTES: dict = {
     "bin_sort_search_kernel": 127_229_184,     # 89.93 MB read + 37.30 MB written
     "place_tile_kernel": 66_431_232,           # 40.11 MB read + 26.33 MB written
 }
+# what the same capture says bounds each kernel (neither is near its HBM roofline)
+NCU_LIMITER: dict = {
+    "bin_sort_search_kernel": {"issue_slots_busy": 0.694, "shared_memory_pipe": 0.612, "dram_throughput": 0.119,
+                               "note": "instruction issue and the shared-memory pipe, not HBM"},
+    "place_tile_kernel": {"issue_slots_busy": 0.497, "shared_memory_pipe": 0.471, "dram_throughput": 0.111,
+                          "note": "dependent-instruction latency at one 1024-thread block per SM"},
+}
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
@@ -402,6 +409,7 @@ def run_b200(args):
             roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                         "frac": achieved / peak,
                         "traffic": NCU_TRAFFIC_BYTES.get(kname) if (args.config == 5 and args.scale == 1.0) else None,
+                        "ncu_limiter": NCU_LIMITER.get(kname) if (args.config == 5 and args.scale == 1.0) else None,
                         "peak_source": peak_src,
                         "avg_launch_ms": launch_ms, "launches_timed": timed[dom][1],
                         "algorithmic_bytes_per_launch": alg_bytes,
