@@ -112,3 +112,28 @@ def test_host_side_argument_checks_return_before_cuda():
     assert L.bits_place(fake, 4, bad1.ctypes.data, 1, 1, 0, 0, ws, 1 << 40, fake, fake, None) == 3
     assert L.bits_sort_u32(None, fake, 4, ws, 1 << 40, None) == 1
     assert L.bits_sort_u32(fake, fake, 2**32, ws, 1 << 40, None) == 2
+
+
+def test_new_entry_points_reject_bad_arguments_on_the_host():
+    """bits_decide / bits_enumerate / bits_workspace_sorted_offset: argument errors come back before any CUDA call."""
+    L = bits.lib()
+    one = (C.c_uint32 * 4)(1, 2, 3, 4)
+    p = C.addressof(one)
+    tot = C.c_uint64(0)
+    # NULL outputs
+    assert L.bits_decide(p, p, 1, p, p, 1, 0, 0, 0, 0, 0) == 1
+    assert L.bits_enumerate(p, p, 1, p, p, 1, 0, 0, 0, 0, 0, 0, 0, 0) == 1
+    assert L.bits_enumerate(p, p, 1, p, p, 1, 0, 0, 0, 0, 0, 5, C.addressof(tot), 0) == 1      # capacity without arrays
+    # independently sorted B has lost the pairing of starts and ends: enumeration refuses it
+    assert L.bits_enumerate(p, p, 1, p, p, 1, bits.B_SORTED, 0, 0, p, p, 4, C.addressof(tot), 0) == 6
+    # unknown flag bits, sizes
+    assert L.bits_decide(p, p, 1, p, p, 1, 64, 0, 0, p, 0) == 6
+    assert L.bits_decide(p, p, 2**32, p, p, 1, 0, 0, 0, p, 0) == 2
+    # workspace missing
+    assert L.bits_decide(p, p, 1, p, p, 1, 0, 0, 0, p, 0) == 5
+    assert L.bits_enumerate(p, p, 1, p, p, 1, 0, 0, 0, 0, 0, 0, C.addressof(tot), 0) == 5
+    assert bits.workspace_bytes(bits.FN_ENUMERATE, 1000, 1000) > bits.workspace_bytes(bits.FN_COUNT, 1000, 1000)
+    off = C.c_size_t(0)
+    assert L.bits_workspace_sorted_offset(bits.FN_COUNT, 10, 1000, 0, 0, 1, C.addressof(off)) == 0 and off.value > 0
+    assert L.bits_workspace_sorted_offset(bits.FN_SORT, 10, 1000, 0, 0, 0, C.addressof(off)) == 6
+    assert L.bits_workspace_sorted_offset(bits.FN_COUNT, 10, 1000, 0, 0, 2, C.addressof(off)) == 6
