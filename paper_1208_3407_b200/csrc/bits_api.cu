@@ -275,12 +275,12 @@ static int launch_sort_passes(const SortPlan& p, uint32_t* epoch, cudaStream_t s
       a.arr[k].dst = (pass & 1) ? p.y[kk] : p.x[kk];
       a.arr[k].hist = p.hist[kk] + pass * rs::kRadix;
       a.arr[k].status = p.status[kk];
-      a.arr[k].ticket = p.ticket + k;
+      a.arr[k].ticket = p.ticket + 4 * k + pass;
     }
     a.n = p.n; a.n_tiles = p.n_tiles; a.shift = 8 * pass; a.epoch = (*epoch)++;
     a.run_if[0] = p.run_if; a.run_if[1] = p.run_if ? p.run_if + (p.n_arrays > 1 ? 1 : 0) : nullptr;
     ProfScope prof(kClsSortPass, st);
-    rs::onesweep_pass_kernel<<<dim3(p.n_tiles, p.n_arrays), rs::kThreads, 0, st>>>(a);
+    rs::onesweep_pass_kernel<<<dim3(p.n_tiles < 2u * kSMs ? p.n_tiles : 2u * kSMs, p.n_arrays), rs::kThreads, 0, st>>>(a);
     BITS_LAUNCH_CHECK();
   }
   return BITS_OK;
@@ -294,7 +294,9 @@ static int launch_histogram(const uint32_t* k0, const uint32_t* k1, uint32_t* h0
   h.n = n;
   h.run_if[0] = run_if; h.run_if[1] = run_if ? run_if + (n_arrays > 1 ? 1 : 0) : nullptr;
   ProfScope prof(kClsHist, st);
-  rs::histogram_kernel<<<dim3(grid_for(ceil_div(n, 4), 512), n_arrays), 512, 0, st>>>(h);
+  // (a gated launch is almost always skipped: fewer blocks to start and retire)
+  const int grid = grid_for(ceil_div(n, 4), 512);
+  rs::histogram_kernel<<<dim3(run_if && grid > 2 * kSMs ? 2 * kSMs : grid, n_arrays), 512, 0, st>>>(h);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -367,6 +369,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
   if (!g_opt.sort_msd) {
     BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
     if (n_arrays > 1) BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
+    BITS_CUDA_TRY(cudaMemsetAsync(c.ticket, 0, sizeof(uint32_t) * 8, st));
     BITS_TRY(launch_histogram(src0, src1, c.hist[0][0], c.hist[0][1], c.n, n_arrays, st));
     return launch_sort_passes(p, epoch, st);
   }
@@ -384,7 +387,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     msd::PlanArgs pa;
     for (int a = 0; a < 2; ++a) {
       pa.p[a].hist = c.bin_hist[a]; pa.p[a].bin_cursor = c.bin_cursor[a]; pa.p[a].bucket_start = c.bucket_start[a];
-      pa.p[a].n_buckets = c.n_buckets + a; pa.p[a].flag = c.msd_flag + a; pa.p[a].lsd_hist = c.hist[0][a];
+      pa.p[a].n_buckets = c.n_buckets + a; pa.p[a].flag = c.msd_flag + a; pa.p[a].lsd_hist = c.hist[0][a]; pa.p[a].lsd_ticket = c.ticket + 4 * a;
     }
     ProfScope prof(kClsPlan, st);
     msd::plan_kernel<<<n_arrays, 1024, 0, st>>>(pa);
@@ -728,6 +731,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
         BITS_CUDA_TRY(cudaMemsetAsync(L.b.hist[par][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
         BITS_TRY(launch_histogram(L.b.buf[0][0], L.b.buf[1][0], L.b.hist[par][0], L.b.hist[par][1], (uint32_t)n_b, 2, st));
       }
+      BITS_CUDA_TRY(cudaMemsetAsync(L.b.ticket, 0, sizeof(uint32_t) * 8, st));
       BITS_TRY(launch_sort_passes(plan_for(L.b, L.b.buf[0][0], L.b.buf[1][0], par), &epoch, st));
     }
     unsigned long long* out = reinterpret_cast<unsigned long long*>(round_counts_out + k);

@@ -137,6 +137,7 @@ struct PlanArr {
   uint32_t* n_buckets;      // [1] out
   uint32_t* flag;           // [1] out: kFlagBucketTooBig or 0 (plain store: this also resets it)
   uint32_t* lsd_hist;       // [1024] cleared here for the fallback sort's digit histograms (may be null)
+  uint32_t* lsd_ticket;     // [4] cleared here: the fallback sort's tile tickets, one per pass (may be null)
 };
 struct PlanArgs { PlanArr p[2]; };
 
@@ -148,6 +149,7 @@ __global__ void __launch_bounds__(1024) plan_kernel(PlanArgs a) {
   const PlanArr P = blockIdx.x ? a.p[1] : a.p[0];
   const int t = threadIdx.x;
   if (P.lsd_hist) P.lsd_hist[t] = 0;
+  if (P.lsd_ticket && t < 4) P.lsd_ticket[t] = 0;
   uint32_t h[4], ex[4];
   {
     const uint4 v = reinterpret_cast<const uint4*>(P.hist)[t];

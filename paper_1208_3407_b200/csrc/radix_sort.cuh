@@ -32,7 +32,7 @@ struct SortArray {
   uint32_t* dst;
   const uint32_t* hist;   // global histogram of THIS pass's digit: uint32[256]
   uint64_t* status;       // uint64[n_tiles * 256]
-  uint32_t* ticket;       // tile ticket counter, taken modulo n_tiles
+  uint32_t* ticket;       // tile ticket counter of THIS pass and array: zero when the pass starts
 };
 
 struct SortPassArgs {
@@ -141,14 +141,20 @@ __global__ void __launch_bounds__(kThreads, 2) onesweep_pass_kernel(SortPassArgs
   if (skip_launch(a.run_if)) return;
   const SortArray A = blockIdx.y ? a.arr[1] : a.arr[0];   // (no dynamic indexing of the parameter block)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) s_tile = atomicAdd(A.ticket, 1u) % a.n_tiles;
+  const uint32_t shift = a.shift;
+  // Persistent blocks: tiles are handed out in ticket order, so a block only ever waits (look-back) for
+  // tiles whose owners are already running.  A skipped launch (the fallback that is not needed) costs
+  // a few hundred blocks that exit at once instead of one block per tile.
+  for (;;) {
+  __syncthreads();                                         // the previous tile of this block is done with shared memory
+  if (tid == 0) s_tile = atomicAdd(A.ticket, 1u);
   for (int i = tid; i < kWarps * kRadix / 2; i += kThreads) reinterpret_cast<uint32_t*>(&s_whist[0][0])[i] = 0;
   __syncthreads();
 
   const uint32_t tile = s_tile;
+  if (tile >= a.n_tiles) break;                            // block-uniform
   const uint32_t base = tile * (uint32_t)kTile;
   const uint32_t count = min((uint32_t)kTile, a.n - base);
-  const uint32_t shift = a.shift;
 
   // ---- load: warp-striped, key order inside the tile = warp*512 + j*32 + lane ----
   uint32_t key[kKeysPerThread];
@@ -250,6 +256,7 @@ __global__ void __launch_bounds__(kThreads, 2) onesweep_pass_kernel(SortPassArgs
       dst[s_dstbase[(k >> shift) & 255u] + i] = k;
     }
   }
+  }   // tile loop
 }
 
 }  // namespace rs

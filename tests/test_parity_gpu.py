@@ -63,6 +63,24 @@ def test_sort_structured(kind):
     assert np.array_equal(host_u32(bits.sort_u32(dev(k))), oracle.sort_u32(k))
 
 
+@pytest.mark.parametrize("n", [1, 8191, 8193, 300_007, 5_000_011])
+def test_sort_lsd_only(n):
+    """The stable LSD onesweep sort on its own (sort_msd = 0): persistent blocks, tiles by ticket, look-back."""
+    rng = np.random.default_rng(n)
+    k = rng.integers(0, 2**32, n, dtype=np.uint64).astype(np.uint32)
+    bits.set_option("sort_msd", 0)
+    try:
+        ws = torch.empty(bits.workspace_bytes(bits.FN_SORT, 0, n), dtype=torch.uint8, device=DEV)
+        for _ in range(2):                               # twice on one workspace: tickets and epochs restart per call
+            assert np.array_equal(host_u32(bits.sort_u32(dev(k), workspace=ws)), oracle.sort_u32(k))
+        w = W.make_config(5, scale=0.01)                 # and inside the Monte Carlo loop (general path, LSD per round)
+        obs, rc = run_mc(w, 1, 4, 0, 3)
+        o_obs, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 4, 0, 3)
+        assert obs == o_obs and np.array_equal(rc, o_rc)
+    finally:
+        bits.set_option("sort_msd", 1)
+
+
 def test_sort_repeated_calls_share_workspace():
     rng = np.random.default_rng(17)
     n = 50_000
