@@ -246,10 +246,13 @@ def secondary_workloads(device, peak_gbs):
     ws = torch.empty(bits.workspace_bytes(bits.FN_COUNT_PER_INTERVAL, w.n_a, w.n_b), dtype=torch.uint8, device=device)
     counts = torch.empty(w.n_a, dtype=torch.int32, device=device)
     total = torch.empty(1, dtype=torch.int64, device=device)
-    bits.set_option("profile", 2); bits.set_option("profile", 1)
     med, mn = time_device(lambda: bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total), 10)
+    bits.set_option("profile", 2); bits.set_option("profile", 1)          # per-kernel events in separate calls: they cost time
+    calls = 5
+    for _ in range(calls):
+        bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total)
+    torch.cuda.synchronize()
     prof = bits.profile_read(); bits.set_option("profile", 0)
-    calls = 13                                    # 3 warm-ups + 10 timed repeats, all with events on
     ms = {k: v[0] / calls for k, v in prof.items()}     # device ms per call and kernel class
     sort_ms = ms["histogram"] + ms["plan"] + ms["scatter"] + ms["bucket_sort"]   # MSD bucket sort of B's starts and ends
     out["cfg4_large_count_10M"] = {
