@@ -160,7 +160,7 @@ struct Layout {
   uint32_t* spans = nullptr;
   // PERMUTE_B fused rounds (mc_tile.cuh); null when the set is too large for that path
   uint2* pairs = nullptr;                // [n_b] tile-sorted (start, end) pairs
-  uint16_t* tile_off = nullptr;          // [(kMaxBins + 1) * tile_stride] transposed per-tile bin prefixes
+  uint32_t* tile_off = nullptr;          // [n_tiles * tile_stride] per tile and bin: start of the bin's pairs in the tile | count << 16
   uint32_t tile_stride = 0;
   uint32_t* cross_cnt[2] = {nullptr, nullptr};   // [kMaxBins + 1] by round parity
   uint32_t* cross_keys = nullptr;        // [kMaxBins * kCrossCap]
@@ -208,9 +208,9 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
         L.q.carve(c, n_a, true);
         if (n_b <= kFusedMaxKeys) {
           const uint32_t n_tiles = max_tiles_for(n_b);
-          L.tile_stride = (uint32_t)align_up((uint64_t)n_tiles + 1, 8);
+          L.tile_stride = (uint32_t)mct::kMaxBins;       // entries per tile row
           L.pairs = c.take<uint2>(align_up(n_b, 4) + 4);
-          L.tile_off = c.take<uint16_t>((uint64_t)(mct::kMaxBins + 1) * L.tile_stride);
+          L.tile_off = c.take<uint32_t>((uint64_t)(n_tiles + 1) * L.tile_stride);
           for (int a = 0; a < 2; ++a) {
             L.cross_cnt[a] = c.take<uint32_t>(mct::kMaxBins + 4);
             L.qb[a] = c.take<uint32_t>(mct::kMaxBins + 4);

@@ -6,11 +6,11 @@
 //                       first half of the sort: every tile of up to 24,576 fresh intervals is
 //                       ordered by bin (bin = start' >> shift, fixed per call) in shared memory --
 //                       count pass, scan, staging pass through per-bin cursors -- and leaves as
-//                       (start', end') pairs through cp.async.bulk; next to it goes the tile's
-//                       exclusive bin prefix, transposed:  off[b][tile] = #{pairs of the tile in
-//                       bins < b}.  Fresh keys never go to HBM unsorted.
-//   bin_sort_search_kernel  one bin at a time per block.  Row b of the prefix table gives, per
-//                       tile, where the bin's pairs sit; its row sum is the number of keys in
+//                       (start', end') pairs through cp.async.bulk; next to it goes the tile's row
+//                       of the segment table:  off[tile][b] = #{pairs of the tile in bins < b} |
+//                       #{in bin b} << 16 (written coalesced).  Fresh keys never go to HBM unsorted.
+//   bin_sort_search_kernel  one bin at a time per block.  Column b of the segment table gives, per
+//                       tile, where the bin's pairs sit; the sum of the starts is the number of keys in
 //                       all earlier bins, i.e. where the bin starts in the sorted arrays -- no
 //                       histogram pass, no scan over bins, no reservation.  The pairs are
 //                       gathered (cp.async, a group of lanes per segment) into shared memory;
@@ -101,8 +101,8 @@ struct PlaceTileArgs {
   uint32_t shift;            // bin = key >> shift, 1..31
   uint32_t n_bins;           // <= kMaxBins
   uint2* pairs;              // [n]: tile t holds its intervals [t * tile, ...) ordered by bin
-  uint16_t* off;             // [(n_bins + 1) * stride]: off[b * stride + t] = #{pairs of tile t in bins < b}
-  uint32_t stride;
+  uint32_t* off;             // [n_tiles * stride]: off[t * stride + b] = #{pairs of tile t in bins < b} | #{in bin b} << 16
+  uint32_t stride;           // entries per tile row: kMaxBins
   uint32_t* cross_cnt;       // [n_bins + 1] ends handed over to each bin this round (zero on entry)
   uint32_t* cross_keys;      // [n_bins * kCrossCap]
   uint32_t* flag;            // round flag
@@ -177,13 +177,13 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
 #pragma unroll
       for (int j = 0; j < kPer / 4; ++j)
         reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + j] = make_uint4(lb[4 * j], lb[4 * j + 1], lb[4 * j + 2], lb[4 * j + 3]);
-      const uint32_t b0 = (uint32_t)tid * kPer;
-      if (b0 <= a.n_bins) {
-        uint16_t* o = a.off + (size_t)b0 * a.stride + tile;
+      // the tile's row of the segment table, one word per bin (where the bin's pairs start in the tile | how many
+      // << 16), all kMaxBins entries: coalesced
+      uint32_t* o = a.off + (size_t)tile * a.stride + (size_t)tid * kPer;
 #pragma unroll
-        for (int j = 0; j < kPer; ++j)
-          if (b0 + j <= a.n_bins) o[(size_t)j * a.stride] = (uint16_t)lb[j];
-      }
+      for (int j = 0; j < kPer / 4; ++j)
+        reinterpret_cast<uint4*>(o)[j] = make_uint4(lb[4 * j] | (c[4 * j] << 16), lb[4 * j + 1] | (c[4 * j + 1] << 16),
+                                                    lb[4 * j + 2] | (c[4 * j + 2] << 16), lb[4 * j + 3] | (c[4 * j + 3] << 16));
     }
     if (tid == 0 && stage_in_flight) { bulk_wait_group_read0(); stage_in_flight = false; }   // the previous tile has left s_stage
     __syncthreads();
@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
 // ---------------------------------------------------------------------------------------------
 struct BinSortArgs {
   const uint2* pairs;
-  const uint16_t* off;
+  const uint32_t* off;
   uint32_t stride;
   uint32_t n_tiles;
   uint32_t tile;
@@ -426,10 +426,16 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
   while (d < a.n_bins) {
     if (tid == 0) s_next = gridDim.x + atomicAdd(const_cast<uint32_t*>(a.cross_cnt) + kMaxBins + 1, 1u);
     a.cross_cnt_next[d] = 0;   // (every thread writes the same zero: harmless, and no divergence)
-    const uint16_t* __restrict__ row0 = a.off + (size_t)d * a.stride;
-    const uint16_t* __restrict__ row1 = row0 + a.stride;
+    // column d (and d + 1) of the per-tile prefix table: one scattered read per tile here instead of one
+    // scattered write per (tile, bin) in the placement kernel
+    const uint32_t* __restrict__ col = a.off + d;
     uint32_t len_sum = 0, lo_sum = 0;
-    for (uint32_t t = t0; t < t1; ++t) { const uint32_t lo = __ldg(row0 + t), hi = __ldg(row1 + t); len_sum += hi - lo; lo_sum += lo; }
+    uint32_t seg0 = 0, seg1 = 0;                     // lo | len << 16 of this thread's first two tiles (usually all it has)
+    for (uint32_t t = t0; t < t1; ++t) {
+      const uint32_t sg = __ldg(col + (size_t)t * a.stride);
+      len_sum += sg >> 16; lo_sum += sg & 0xffffu;
+      if (t == t0) seg0 = sg; else if (t == t0 + 1u) seg1 = sg;
+    }
     // exclusive scan of len_sum (where this thread's pairs go) and block sum of lo_sum (keys in earlier bins)
     uint32_t incl = len_sum, ls = lo_sum;
 #pragma unroll
@@ -457,9 +463,10 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     }
     // where each tile's segment of this bin sits in the tile (lo) and goes in the bin's buffers (pos)
     for (uint32_t t = t0; t < t1; ++t) {
-      const uint32_t lo = __ldg(row0 + t), hi = __ldg(row1 + t);
+      const uint32_t sg = t == t0 ? seg0 : (t == t0 + 1u ? seg1 : __ldg(col + (size_t)t * a.stride));
+      const uint32_t lo = sg & 0xffffu, len = sg >> 16;
       s_seg[t] = lo | (pos << 16);
-      pos += hi - lo;
+      pos += len;
     }
     if (tid == 0) s_seg[a.n_tiles] = np << 16;
     __syncthreads();
