@@ -115,23 +115,27 @@ struct SortCtx {
   uint32_t* bucket_start[2] = {nullptr, nullptr};   // uint32[kBins + 1]
   uint32_t* n_buckets = nullptr;                    // uint32[2]
   uint32_t* msd_flag = nullptr;                     // uint32[2]
+  size_t zero_bytes = 0;                            // from hist[0][0]: digit histograms, tickets, bin histograms, bucket counts, flags, status words
   void carve(Carver& c, uint64_t n_keys, bool with_index) {
     n = (uint32_t)n_keys;
     n_tiles = rs::num_tiles(n_keys);
     const uint64_t padded = align_up(n_keys + kPad, 64);
     for (int a = 0; a < 2; ++a)
       for (int b = 0; b < 2; ++b) buf[a][b] = c.take<uint32_t>(padded);
+    // everything a call clears before its first sort sits in one stretch, so that one memset does it
+    const size_t z0 = align_up(c.used, 256);
     for (int p = 0; p < 2; ++p)
       for (int a = 0; a < 2; ++a) hist[p][a] = c.take<uint32_t>(rs::kPasses * rs::kRadix);
-    for (int a = 0; a < 2; ++a) status[a] = c.take<uint64_t>((uint64_t)n_tiles * rs::kRadix);
     ticket = c.take<uint32_t>(64);
+    for (int a = 0; a < 2; ++a) bin_hist[a] = c.take<uint32_t>(msd::kBins);
+    n_buckets = c.take<uint32_t>(64);
+    msd_flag = n_buckets ? n_buckets + 8 : nullptr;
+    for (int a = 0; a < 2; ++a) status[a] = c.take<uint64_t>((uint64_t)n_tiles * rs::kRadix);
+    zero_bytes = c.used - z0;
     for (int a = 0; a < 2; ++a) {
-      bin_hist[a] = c.take<uint32_t>(msd::kBins);
       bin_cursor[a] = c.take<uint32_t>(msd::kBins);
       bucket_start[a] = c.take<uint32_t>(msd::kBins + 4);
     }
-    n_buckets = c.take<uint32_t>(64);
-    msd_flag = n_buckets ? n_buckets + 8 : nullptr;
     shift = index_shift_for(n_keys);
     if (with_index)
       for (int a = 0; a < 2; ++a) idx[a] = c.take<uint32_t>(index_entries(shift));
@@ -303,16 +307,7 @@ static int launch_histogram(const uint32_t* k0, const uint32_t* k1, uint32_t* h0
 
 // Clear the sort bookkeeping of a context (once per library call); epochs restart at 1.
 static int reset_sort_ctx(const SortCtx& c, cudaStream_t st) {
-  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[1][0], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[1][1], 0, sizeof(uint32_t) * rs::kPasses * rs::kRadix, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.status[0], 0, sizeof(uint64_t) * (uint64_t)c.n_tiles * rs::kRadix, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.status[1], 0, sizeof(uint64_t) * (uint64_t)c.n_tiles * rs::kRadix, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.ticket, 0, sizeof(uint32_t) * 64, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.bin_hist[0], 0, sizeof(uint32_t) * msd::kBins, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.bin_hist[1], 0, sizeof(uint32_t) * msd::kBins, st));
-  BITS_CUDA_TRY(cudaMemsetAsync(c.n_buckets, 0, sizeof(uint32_t) * 64, st));
+  BITS_CUDA_TRY(cudaMemsetAsync(c.hist[0][0], 0, c.zero_bytes, st));   // one stretch of the workspace (SortCtx::carve)
   return BITS_OK;
 }
 
