@@ -85,6 +85,22 @@ struct ProfScope {
   ~ProfScope() { if (k >= 0) cudaEventRecord(g_prof.ev[2 * k + 1], st); }
 };
 
+// Kernels that follow another kernel of the same call are launched with programmatic stream serialization
+// (unless the per-kernel event timers are on, or option mc_pdl = 0): each may be scheduled while its predecessor
+// drains, and waits on the device (griddepcontrol.wait, its first statement) before it touches global memory.
+// Only kernels that carry that wait may be launched through here.
+template <typename... KArgs, typename... Args>
+static void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = (g_opt.mc_pdl != 0 && !g_prof.on) ? 1 : 0;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  (void)cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
+
 // ---------------------------------------------------------------------------------------------
 // Workspace: a bump allocator that is run twice -- once with base == nullptr to size, once to carve.
 struct Carver {
@@ -284,7 +300,7 @@ static int launch_sort_passes(const SortPlan& p, uint32_t* epoch, cudaStream_t s
     a.n = p.n; a.n_tiles = p.n_tiles; a.shift = 8 * pass; a.epoch = (*epoch)++;
     a.run_if[0] = p.run_if; a.run_if[1] = p.run_if ? p.run_if + (p.n_arrays > 1 ? 1 : 0) : nullptr;
     ProfScope prof(kClsSortPass, st);
-    rs::onesweep_pass_kernel<<<dim3(p.n_tiles < 2u * kSMs ? p.n_tiles : 2u * kSMs, p.n_arrays), rs::kThreads, 0, st>>>(a);
+    launch_pdl(rs::onesweep_pass_kernel, dim3(p.n_tiles < 2u * kSMs ? p.n_tiles : 2u * kSMs, p.n_arrays), rs::kThreads, 0, st, a);
     BITS_LAUNCH_CHECK();
   }
   return BITS_OK;
@@ -300,7 +316,7 @@ static int launch_histogram(const uint32_t* k0, const uint32_t* k1, uint32_t* h0
   ProfScope prof(kClsHist, st);
   // (a gated launch is almost always skipped: fewer blocks to start and retire)
   const int grid = grid_for(ceil_div(n, 4), 512);
-  rs::histogram_kernel<<<dim3(run_if && grid > 2 * kSMs ? 2 * kSMs : grid, n_arrays), 512, 0, st>>>(h);
+  launch_pdl(rs::histogram_kernel, dim3(run_if && grid > 2 * kSMs ? 2 * kSMs : grid, n_arrays), 512, 0, st, h);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -375,7 +391,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     h.hist[0] = c.bin_hist[0]; h.hist[1] = c.bin_hist[1];
     h.n = c.n;
     ProfScope prof(kClsHist, st);
-    msd::bin_hist_kernel<<<dim3(grid_for(ceil_div(c.n, 4), 512), n_arrays), 512, 0, st>>>(h);
+    launch_pdl(msd::bin_hist_kernel, dim3(grid_for(ceil_div(c.n, 4), 512), n_arrays), 512, 0, st, h);
     BITS_LAUNCH_CHECK();
   }
   {
@@ -385,7 +401,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
       pa.p[a].n_buckets = c.n_buckets + a; pa.p[a].flag = c.msd_flag + a; pa.p[a].lsd_hist = c.hist[0][a]; pa.p[a].lsd_ticket = c.ticket + 4 * a;
     }
     ProfScope prof(kClsPlan, st);
-    msd::plan_kernel<<<n_arrays, 1024, 0, st>>>(pa);
+    launch_pdl(msd::plan_kernel, n_arrays, 1024, 0, st, pa);
     BITS_LAUNCH_CHECK();
   }
   {
@@ -397,7 +413,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     sa.n = c.n; sa.n_tiles = (uint32_t)ceil_div(c.n, msd::kScTile);
     const uint32_t per = (uint32_t)kSMs / (uint32_t)n_arrays;
     ProfScope prof(kClsScatter, st);
-    msd::scatter_kernel<<<dim3(sa.n_tiles < per ? sa.n_tiles : per, n_arrays), msd::kScThreads, msd::kScSmem, st>>>(sa);
+    launch_pdl(msd::scatter_kernel, dim3(sa.n_tiles < per ? sa.n_tiles : per, n_arrays), msd::kScThreads, msd::kScSmem, st, sa);
     BITS_LAUNCH_CHECK();
   }
   {
@@ -412,7 +428,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     ProfScope prof(kClsBucketSort, st);
     ba.slab = 0; ba.round_flag = nullptr; ba.round_total = nullptr;
     for (int a = 0; a < 2; ++a) { ba.arr[a].q_sorted = nullptr; ba.arr[a].qb = nullptr; }
-    msd::bucket_sort_kernel<false, false><<<dim3(want < per ? want : per, n_arrays), msd::kBkThreads, msd::kBkSmem, st>>>(ba);
+    launch_pdl(msd::bucket_sort_kernel<false, false>, dim3(want < per ? want : per, n_arrays), msd::kBkThreads, msd::kBkSmem, st, ba);
     BITS_LAUNCH_CHECK();
   }
   // fallback: the stable LSD sort redoes everything if a flag was raised, else these launches exit at once
@@ -429,7 +445,7 @@ static int launch_build_index(const SortCtx& c, cudaStream_t st) {
   const uint64_t need = ceil_div((uint64_t)c.n, 4) + 1;   // four positions per thread
   const uint64_t threads = need > (uint64_t)kPad ? need : (uint64_t)kPad;
   ProfScope prof(kClsIndex, st);
-  build_index_kernel<<<dim3((unsigned)ceil_div(threads, 256), 2), 256, 0, st>>>(ia);
+  launch_pdl(build_index_kernel, dim3((unsigned)ceil_div(threads, 256), 2), 256, 0, st, ia);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -460,7 +476,7 @@ static int launch_count(const uint32_t* a_start, const uint32_t* a_end, uint32_t
   const SortedSet s0 = sorted_set(b, 0), s1 = sorted_set(b, 1);
   unsigned long long* tot = reinterpret_cast<unsigned long long*>(total);
   const int sv = (int)g_opt.search_variant;
-#define BITS_COUNT_LAUNCH(V, S) count_kernel<V, S><<<grid, 256, 0, st>>>(a_start, a_end, n_a, s0, s1, counts, tot)
+#define BITS_COUNT_LAUNCH(V, S) launch_pdl(count_kernel<V, S>, grid, 256, 0, st, a_start, a_end, n_a, s0, s1, counts, tot)
   if (vec) {
     if (sv == kSearchPlain) BITS_COUNT_LAUNCH(true, kSearchPlain);
     else if (sv == kSearchStaged) BITS_COUNT_LAUNCH(true, kSearchStaged);
@@ -570,20 +586,6 @@ static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* en
   }
   BITS_LAUNCH_CHECK();
   return BITS_OK;
-}
-
-// The two kernels of a fused round are launched with programmatic stream serialization (unless the
-// per-kernel event timers are on): each may be scheduled while its predecessor drains and waits
-// on the device (griddepcontrol.wait) before it touches shared buffers.
-template <typename Kernel, typename Args>
-static void launch_pdl(Kernel kernel, unsigned grid, unsigned block, size_t smem, cudaStream_t st, const Args& args) {
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = (g_opt.mc_pdl != 0 && !g_prof.on) ? 1 : 0;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  (void)cudaLaunchKernelEx(&cfg, kernel, args);
 }
 
 template <class C>

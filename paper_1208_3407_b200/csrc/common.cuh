@@ -35,6 +35,12 @@ extern unsigned long long g_launches;
 __host__ __device__ inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 __host__ __device__ inline uint64_t ceil_div(uint64_t x, uint64_t a) { return (x + a - 1) / a; }
 
+// Programmatic dependent launch: a kernel launched with the programmatic-stream-serialization attribute may be
+// scheduled while its predecessor on the stream drains; it must not touch what the predecessor wrote (or overwrite
+// what it reads) before grid_dependency_wait().  A no-op in a plain launch.
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // 64-bit warp sum (all 32 lanes participate; every lane gets the total).
 __device__ __forceinline__ uint64_t warp_sum_u64(uint64_t v) {
 #pragma unroll

@@ -82,11 +82,6 @@ __device__ __forceinline__ void bulk_store_smem_to_global(void* gdst, const void
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void bulk_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-// Programmatic dependent launch: a kernel launched with the programmatic-stream-serialization attribute
-// may start while its predecessor on the stream drains; it must not touch what the predecessor wrote (or
-// overwrite what it reads) before grid_dependency_wait().  Both are no-ops in a plain launch.
-__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_group_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 struct PlaceTileArgs {

@@ -102,6 +102,7 @@ struct BinHistArgs {
 
 __global__ void __launch_bounds__(512) bin_hist_kernel(BinHistArgs a) {
   __shared__ uint32_t s_h[kBins];
+  grid_dependency_wait();
   for (int i = threadIdx.x; i < kBins; i += blockDim.x) s_h[i] = 0;
   __syncthreads();
   const uint32_t* __restrict__ keys = blockIdx.y ? a.keys[1] : a.keys[0];
@@ -148,6 +149,7 @@ __global__ void __launch_bounds__(1024) plan_kernel(PlanArgs a) {
   __shared__ uint32_t s_start[kBins + 1];
   const PlanArr P = blockIdx.x ? a.p[1] : a.p[0];
   const int t = threadIdx.x;
+  grid_dependency_wait();
   if (P.lsd_hist) P.lsd_hist[t] = 0;
   if (P.lsd_ticket && t < 4) P.lsd_ticket[t] = 0;
   uint32_t h[4], ex[4];
@@ -207,6 +209,7 @@ __global__ void __launch_bounds__(kScThreads, 1) scatter_kernel(ScatterArgs a) {
   uint32_t* s_delta = s_cnt + kBins;                                    // [kBins] global dst - local base
   __shared__ uint32_t s_w[32];
   const ScatterArr A = blockIdx.y ? a.arr[1] : a.arr[0];
+  grid_dependency_wait();
   if (*A.flag) return;
   const int tid = threadIdx.x;
   const uint32_t mis = misalign_words(A.src);   // tiles start at multiples of kScTile keys: same misalignment
@@ -310,6 +313,7 @@ __global__ void __launch_bounds__(kBkThreads, 2) bucket_sort_kernel(BucketArgs a
   __shared__ uint32_t s_min[32], s_max[32];
   __shared__ uint32_t s_nwl;                                 // pairs | larger groups << 16
   const BucketArr A = blockIdx.y ? a.arr[1] : a.arr[0];
+  grid_dependency_wait();
   if (*A.flag & kFlagBucketTooBig) return;
   const uint32_t nb = *A.n_buckets;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;

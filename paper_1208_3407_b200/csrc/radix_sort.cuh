@@ -92,6 +92,7 @@ struct HistArgs {
 
 __global__ void __launch_bounds__(512) histogram_kernel(HistArgs a) {
   __shared__ uint32_t s_h[kPasses * kRadix];
+  grid_dependency_wait();
   if (skip_launch(a.run_if)) return;
   for (int i = threadIdx.x; i < kPasses * kRadix; i += blockDim.x) s_h[i] = 0;
   __syncthreads();
@@ -138,6 +139,7 @@ __global__ void __launch_bounds__(kThreads, 2) onesweep_pass_kernel(SortPassArgs
   __shared__ uint32_t s_wsum[8];
   __shared__ uint32_t s_tile;
 
+  grid_dependency_wait();
   if (skip_launch(a.run_if)) return;
   const SortArray A = blockIdx.y ? a.arr[1] : a.arr[0];   // (no dynamic indexing of the parameter block)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;

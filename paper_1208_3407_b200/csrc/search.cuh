@@ -86,6 +86,7 @@ __global__ void __launch_bounds__(256) build_index_kernel(IndexArgs a) {
   uint32_t* __restrict__ idx = blockIdx.y ? a.idx[1] : a.idx[0];
   const uint32_t n = a.n, s = a.shift;
   const uint32_t H = 1u << (32 - s);
+  grid_dependency_wait();
   const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;   // warps are never partly out of range
   const uint32_t lane = threadIdx.x & 31;
   if (gid < kPad) keys[(uint64_t)n + gid] = 0xffffffffu;
@@ -181,6 +182,7 @@ __global__ void __launch_bounds__(256) count_kernel(const uint32_t* __restrict__
                                                     uint32_t* __restrict__ counts, unsigned long long* total) {
   __shared__ uint64_t s_red[8];
   __shared__ uint32_t s_top[kSearch == kSearchStaged ? 2 * kStaged : 1];
+  grid_dependency_wait();
   if (kSearch == kSearchStaged) {
     stage_top_levels(bs, s_top);
     stage_top_levels(be, s_top + kStaged);
