@@ -938,7 +938,7 @@ int bits_decide(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, co
   BITS_TRY(reset_sort_ctx(L.b, st));
   BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
   ProfScope prof(kClsCount, st);
-  decide_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), sorted_set(L.b, 1), any_out);
+  launch_pdl(decide_kernel, grid_for(n_a, 256), 256, 0, st, a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), sorted_set(L.b, 1), any_out);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -963,19 +963,19 @@ int bits_enumerate(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   BITS_TRY(launch_count(a_start, a_end, (uint32_t)n_a, L.b, L.e_counts, nullptr, st));
   const uint32_t n_tiles = (uint32_t)ceil_div(n_a, (uint64_t)enu::kScanTile);
   ProfScope prof(kClsOther, st);
-  enu::scan_tile_sums_kernel<<<n_tiles, enu::kScanThreads, 0, st>>>(L.e_counts, (uint32_t)n_a, L.e_tile_sums);
+  launch_pdl(enu::scan_tile_sums_kernel, n_tiles, enu::kScanThreads, 0, st, L.e_counts, (uint32_t)n_a, L.e_tile_sums);
   BITS_LAUNCH_CHECK();
-  enu::scan_tile_prefix_kernel<<<1, 1024, 0, st>>>(L.e_tile_sums, n_tiles, reinterpret_cast<unsigned long long*>(total_out));
+  launch_pdl(enu::scan_tile_prefix_kernel, 1, 1024, 0, st, L.e_tile_sums, n_tiles, reinterpret_cast<unsigned long long*>(total_out));
   BITS_LAUNCH_CHECK();
-  enu::scan_apply_kernel<<<n_tiles, enu::kScanThreads, 0, st>>>(L.e_counts, (uint32_t)n_a, L.e_tile_sums, L.e_offsets);
+  launch_pdl(enu::scan_apply_kernel, n_tiles, enu::kScanThreads, 0, st, L.e_counts, (uint32_t)n_a, L.e_tile_sums, L.e_offsets);
   BITS_LAUNCH_CHECK();
   if (capacity == 0) return BITS_OK;
   BITS_CUDA_TRY(cudaMemsetAsync(L.e_tie, 0, sizeof(uint32_t) * ((size_t)n_b + 1), st));
-  enu::start_order_kernel<<<grid_for(n_b, 256), 256, 0, st>>>(b_start, b_end, (uint32_t)n_b, sorted_set(L.b, 0), L.e_tie,
-                                                              L.e_end_by_start, L.e_idx_by_start);
+  launch_pdl(enu::start_order_kernel, grid_for(n_b, 256), 256, 0, st, b_start, b_end, (uint32_t)n_b, sorted_set(L.b, 0), L.e_tie,
+             L.e_end_by_start, L.e_idx_by_start);
   BITS_LAUNCH_CHECK();
-  enu::emit_pairs_kernel<<<grid_for(n_a, 256), 256, 0, st>>>(a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), L.e_counts, L.e_offsets,
-                                                             L.e_end_by_start, L.e_idx_by_start, pair_a_out, pair_b_out, capacity);
+  launch_pdl(enu::emit_pairs_kernel, grid_for(n_a, 256), 256, 0, st, a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), L.e_counts, L.e_offsets,
+             L.e_end_by_start, L.e_idx_by_start, pair_a_out, pair_b_out, capacity);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }

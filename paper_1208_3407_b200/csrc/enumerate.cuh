@@ -25,6 +25,7 @@ __device__ __forceinline__ uint32_t rank_lt(const SortedSet& s, uint32_t q) { re
 __global__ void __launch_bounds__(256) start_order_kernel(const uint32_t* __restrict__ b_start, const uint32_t* __restrict__ b_end,
                                                           uint32_t n_b, SortedSet bs, uint32_t* tie,
                                                           uint32_t* __restrict__ end_by_start, uint32_t* __restrict__ idx_by_start) {
+  grid_dependency_wait();
   for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n_b; j += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t p = rank_lt(bs, b_start[j]);
     const uint32_t pos = p + atomicAdd(&tie[p], 1u);
@@ -39,6 +40,7 @@ constexpr int kScanThreads = 256, kScanPer = 16, kScanTile = kScanThreads * kSca
 __global__ void __launch_bounds__(kScanThreads) scan_tile_sums_kernel(const uint32_t* __restrict__ counts, uint32_t n,
                                                                       unsigned long long* __restrict__ tile_sums) {
   __shared__ uint64_t s_red[kScanThreads / 32];
+  grid_dependency_wait();
   const uint64_t base = (uint64_t)blockIdx.x * kScanTile;
   uint64_t sum = 0;
   for (int j = 0; j < kScanPer; ++j) {
@@ -60,6 +62,7 @@ __global__ void __launch_bounds__(1024) scan_tile_prefix_kernel(unsigned long lo
                                                                 unsigned long long* total) {
   __shared__ uint64_t s_w[32];
   __shared__ uint64_t s_carry;
+  grid_dependency_wait();
   if (threadIdx.x == 0) s_carry = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -87,6 +90,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(const uint32_t
                                                                   const unsigned long long* __restrict__ tile_prefix,
                                                                   unsigned long long* __restrict__ offsets) {
   __shared__ uint64_t s_w[kScanThreads / 32];
+  grid_dependency_wait();
   const uint64_t i0 = (uint64_t)blockIdx.x * kScanTile + (uint64_t)threadIdx.x * kScanPer;
   uint32_t c[kScanPer];
   uint64_t sum = 0;
@@ -115,6 +119,7 @@ __global__ void __launch_bounds__(256) emit_pairs_kernel(const uint32_t* __restr
                                                          const uint32_t* __restrict__ idx_by_start,
                                                          uint32_t* __restrict__ pair_a, uint32_t* __restrict__ pair_b,
                                                          unsigned long long capacity) {
+  grid_dependency_wait();
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_a; i += (uint64_t)gridDim.x * blockDim.x) {
     uint32_t left = counts[i];
     if (left == 0) continue;

@@ -242,6 +242,7 @@ __global__ void __launch_bounds__(256) decide_kernel(const uint32_t* __restrict_
                                                      uint32_t n_a, SortedSet bs, SortedSet be, uint32_t* any) {
   // (whole warps iterate together; one lane reports for the warp, and only if nobody has yet: a store
   // from every thread that finds an intersection would serialise on the one word)
+  grid_dependency_wait();
   const uint64_t n_pad = ((uint64_t)n_a + 31) & ~31ull;
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pad; i += (uint64_t)gridDim.x * blockDim.x) {
     if (*reinterpret_cast<volatile uint32_t*>(any)) return;

@@ -299,6 +299,34 @@ def test_enumerate_config2_is_valid_and_complete():
     assert np.unique(pa * (1 << 32) + pb).size == n
 
 
+def test_results_do_not_depend_on_programmatic_launch():
+    """The kernels of a call are chained by programmatic dependent launch (option mc_pdl, on by default):
+    with it off every launch is fully serialised.  Counts, pairs, decisions and Monte Carlo rounds must be
+    the same integers either way, call after call on one workspace (a kernel that touched memory before its
+    griddepcontrol.wait would show up as a difference or as a mismatch with the oracle)."""
+    w = W.make_config(2, scale=0.2)
+    g = W.make_config(5, scale=0.02)
+    o_total, o_counts = oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end)
+    o_obs, o_rc = oracle.mc_rounds(g.a_start, g.a_end, g.b_start, g.b_end, g.chrom_offsets, bits.PERMUTE_B, 7, 0, 3)
+    d = [dev(x) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    dg = [dev(x) for x in (g.a_start, g.a_end, g.b_start, g.b_end)]
+    try:
+        for pdl in (1, 0, 1):
+            bits.set_option("mc_pdl", pdl)
+            for _ in range(3):
+                counts, total = bits.count_per_interval(*d)
+                pa, pb, n = bits.enumerate_pairs(*d)
+                any_ = bits.decide(*d)
+                obs, rc = bits.mc_rounds(*dg, g.chrom_offsets, bits.PERMUTE_B, 7, 0, 3)
+                sync()
+                assert int(host_u64(total)[0]) == o_total and np.array_equal(host_u32(counts), o_counts)
+                assert n == o_total and np.array_equal(np.bincount(host_u32(pa).astype(np.int64), minlength=w.n_a), o_counts)
+                assert bool(any_.cpu().numpy()[0]) == (o_total > 0)
+                assert int(host_u64(obs)[0]) == o_obs and np.array_equal(host_u64(rc), o_rc)
+    finally:
+        bits.set_option("mc_pdl", 1)
+
+
 def test_count_config4_full_size():
     w = W.make_config(4)
     total = check_counts(w.a_start, w.a_end, w.b_start, w.b_end)
