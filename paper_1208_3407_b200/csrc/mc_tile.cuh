@@ -361,7 +361,8 @@ __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint
 template <class C, bool kStrict>
 __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t mv, uint32_t mask, uint32_t sshift,
                                                    const uint16_t* cur, uint32_t gbase, uint32_t* __restrict__ dst,
-                                                   const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi) {
+                                                   const uint32_t* __restrict__ q_sorted, uint32_t qlo, uint32_t qhi,
+                                                   uint32_t q_first) {
   const int tid = threadIdx.x;
 #pragma unroll 2
   for (uint32_t p = tid; p < mv; p += C::kThreads) {
@@ -383,7 +384,7 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
   }
   uint64_t qsum = 0;
   for (uint32_t qi = qlo + tid; qi < qhi; qi += C::kThreads) {
-    const uint32_t q = __ldg(q_sorted + qi);
+    const uint32_t q = qi == qlo + tid ? q_first : __ldg(q_sorted + qi);   // (the thread's first query was fetched before the sort)
     const uint32_t sb = sub_of(q, mask, sshift);
     const uint32_t lo = cur[kFront - 1 + sb], hi = cur[kFront + sb];
     uint32_t c = 0;
@@ -451,6 +452,9 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     const uint32_t n_in = min(__ldg(a.cross_cnt + d), (uint32_t)kCrossCap);
     const uint32_t qlo0 = __ldg(a.qb[0] + d), qhi0 = __ldg(a.qb[0] + d + 1);
     const uint32_t qlo1 = __ldg(a.qb[1] + d), qhi1 = __ldg(a.qb[1] + d + 1);
+    // each thread's first query of either kind (usually its only one): in flight during the gather and the sort
+    const uint32_t qf0 = qlo0 + tid < qhi0 ? __ldg(a.q_sorted[0] + qlo0 + tid) : 0u;
+    const uint32_t qf1 = qlo1 + tid < qhi1 ? __ldg(a.q_sorted[1] + qlo1 + tid) : 0u;
     if (np + n_in > (uint32_t)C::kCap) {                                   // block-uniform
       if (tid == 0) atomicOr(a.flag, kFlagBinTooBig);
       d = d_next;
@@ -497,9 +501,9 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     // (both scatters first: the two long write-out phases then follow each other with no barrier between them)
     scatter_in_place<C, false, false>(s_ks, np, d, shift, mask, sshift, s_cur_s);   // (the barriers of the next call cover it)
     scatter_in_place<C, true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
-    qsum += write_and_rank<C, false>(s_ks, np, mask, sshift, s_cur_s, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0);
+    qsum += write_and_rank<C, false>(s_ks, np, mask, sshift, s_cur_s, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0, qf0);
     // ends: n_in ends of earlier pairs lie in this bin, so it begins at gbase - n_in in B_E
-    qsum -= write_and_rank<C, true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1);
+    qsum -= write_and_rank<C, true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1, qf1);
     d = d_next;
   }
   if (blockIdx.x == 0 && tid == 0) {
