@@ -425,6 +425,10 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     // column d (and d + 1) of the per-tile prefix table: one scattered read per tile here instead of one
     // scattered write per (tile, bin) in the placement kernel
     const uint32_t* __restrict__ col = a.off + d;
+    // (loaded here, used after the scan: the latency overlaps the segment words')
+    const uint32_t n_in = min(__ldg(a.cross_cnt + d), (uint32_t)kCrossCap);
+    const uint32_t qlo0 = __ldg(a.qb[0] + d), qhi0 = __ldg(a.qb[0] + d + 1);
+    const uint32_t qlo1 = __ldg(a.qb[1] + d), qhi1 = __ldg(a.qb[1] + d + 1);
     uint32_t len_sum = 0, lo_sum = 0;
     uint32_t seg0 = 0, seg1 = 0;                     // lo | len << 16 of this thread's first two tiles (usually all it has)
     for (uint32_t t = t0; t < t1; ++t) {
@@ -432,6 +436,9 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
       len_sum += sg >> 16; lo_sum += sg & 0xffffu;
       if (t == t0) seg0 = sg; else if (t == t0 + 1u) seg1 = sg;
     }
+    // each thread's first query of either kind (usually its only one): in flight during the gather and the sort
+    const uint32_t qf0 = qlo0 + tid < qhi0 ? __ldg(a.q_sorted[0] + qlo0 + tid) : 0u;
+    const uint32_t qf1 = qlo1 + tid < qhi1 ? __ldg(a.q_sorted[1] + qlo1 + tid) : 0u;
     // exclusive scan of len_sum (where this thread's pairs go) and block sum of lo_sum (keys in earlier bins)
     uint32_t incl = len_sum, ls = lo_sum;
 #pragma unroll
@@ -449,12 +456,6 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     const uint32_t np = __shfl_sync(kFullMask, x, 31);                  // pairs in this bin
     uint32_t pos = incl - len_sum + (w ? __shfl_sync(kFullMask, x, (w + 31) & 31) : 0u);
     const uint32_t d_next = s_next;
-    const uint32_t n_in = min(__ldg(a.cross_cnt + d), (uint32_t)kCrossCap);
-    const uint32_t qlo0 = __ldg(a.qb[0] + d), qhi0 = __ldg(a.qb[0] + d + 1);
-    const uint32_t qlo1 = __ldg(a.qb[1] + d), qhi1 = __ldg(a.qb[1] + d + 1);
-    // each thread's first query of either kind (usually its only one): in flight during the gather and the sort
-    const uint32_t qf0 = qlo0 + tid < qhi0 ? __ldg(a.q_sorted[0] + qlo0 + tid) : 0u;
-    const uint32_t qf1 = qlo1 + tid < qhi1 ? __ldg(a.q_sorted[1] + qlo1 + tid) : 0u;
     if (np + n_in > (uint32_t)C::kCap) {                                   // block-uniform
       if (tid == 0) atomicOr(a.flag, kFlagBinTooBig);
       d = d_next;
