@@ -37,14 +37,14 @@ if ROOT not in sys.path:
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
 NCU_TRAFFIC_BYTES: dict = {
     # profiles/r1b_fused_ncu_full_summary.txt (config 5, one launch)
-    "bin_sort_search_kernel": 127_440_128,     # 91.31 MB read + 36.13 MB written
-    "place_tile_kernel": 70_380_800,           # 40.11 MB read + 30.27 MB written
+    "bin_sort_search_kernel": 128_288_000,     # 91.32 MB read + 36.97 MB written
+    "place_tile_kernel": 71_345_152,           # 40.10 MB read + 31.24 MB written
 }
 # what the same capture says bounds each kernel (neither is near its HBM roofline)
 NCU_LIMITER: dict = {
-    "bin_sort_search_kernel": {"issue_slots_busy": 0.678, "shared_memory_pipe": 0.622, "dram_throughput": 0.119,
+    "bin_sort_search_kernel": {"issue_slots_busy": 0.709, "shared_memory_pipe": 0.646, "dram_throughput": 0.123,
                                "note": "instruction issue and the shared-memory pipe, not HBM"},
-    "place_tile_kernel": {"issue_slots_busy": 0.543, "shared_memory_pipe": 0.472, "dram_throughput": 0.125,
+    "place_tile_kernel": {"issue_slots_busy": 0.525, "shared_memory_pipe": 0.472, "dram_throughput": 0.132,
                           "note": "dependent-instruction latency at one 1024-thread block per SM"},
 }
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
