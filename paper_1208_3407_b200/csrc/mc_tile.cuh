@@ -322,11 +322,11 @@ __device__ __forceinline__ void scan_cursors(uint16_t* cur_s, uint16_t* cur_e, u
 
 // Counting-sort scatter of buf[0..m) in place: every key is read into a register, then (after a
 // barrier) stored at the slot its sub-bucket's cursor hands out.  With kCheckBin, entries whose
-// bin is not d are dropped.  Ends with a barrier; afterwards buf[0..valid) is ordered by
-// sub-bucket and cur[kFront + sb] is the END of sub-bucket sb.
+// bin is not d are dropped.  Ends with a barrier; afterwards buf[0..mv) (mv = the keys that stay) is ordered
+// by sub-bucket, buf[mv..mv+3) holds 0xffffffff and cur[kFront + sb] is the END of sub-bucket sb.
 template <class C, bool kCheckBin, bool kTrailingBarrier = true>
 __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint32_t d, uint32_t shift, uint32_t mask,
-                                                 uint32_t sshift, uint16_t* cur) {
+                                                 uint32_t sshift, uint16_t* cur, uint32_t mv) {
   const int tid = threadIdx.x;
   uint32_t* cur32 = reinterpret_cast<uint32_t*>(cur);
   uint32_t key[C::kKpt];
@@ -336,6 +336,7 @@ __device__ __forceinline__ void scatter_in_place(uint32_t* buf, uint32_t m, uint
     key[j] = i < m ? buf[i] : 0u;
   }
   __syncthreads();
+  if (tid < 3) buf[mv + tid] = 0xffffffffu;           // sentinels behind the mv keys that stay (no slot lies there)
 #pragma unroll
   for (int j0 = 0; j0 < C::kKpt; j0 += 4) {           // four slots are taken, then filled: the atomics overlap
     if ((uint32_t)(j0 * C::kThreads) >= m) break;
@@ -373,8 +374,8 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
 #pragma unroll
     for (uint32_t i = 0; i < 3; ++i) {
       const uint32_t t = lo + i;
-      const uint32_t kk = buf[t];                    // buf is padded: t < C::kCap + 4
-      rank += (t < hi) & (kk < k + (t < p ? 1u : 0u));
+      const uint32_t kk = buf[t];                    // t < mv + 3: beyond the sub-bucket lie larger keys, beyond mv sentinels
+      rank += kk < k + (t < p ? 1u : 0u);            // (k + 1 cannot wrap: coordinates are < 2^32 - 1)
     }
     if (hi - lo > 3) {
 #pragma unroll 1
@@ -456,7 +457,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     const uint32_t np = __shfl_sync(kFullMask, x, 31);                  // pairs in this bin
     uint32_t pos = incl - len_sum + (w ? __shfl_sync(kFullMask, x, (w + 31) & 31) : 0u);
     const uint32_t d_next = s_next;
-    if (np + n_in > (uint32_t)C::kCap) {                                   // block-uniform
+    if (np + n_in + 4u > (uint32_t)C::kCap) {                              // block-uniform (4: room for the sentinels)
       if (tid == 0) atomicOr(a.flag, kFlagBinTooBig);
       d = d_next;
       continue;
@@ -500,8 +501,8 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     scan_cursors<C>(s_cur_s, s_cur_e, s_w, total);                         // barriers inside
     // starts: all np keys belong to bin d; the bin begins at gbase in B_S
     // (both scatters first: the two long write-out phases then follow each other with no barrier between them)
-    scatter_in_place<C, false, false>(s_ks, np, d, shift, mask, sshift, s_cur_s);   // (the barriers of the next call cover it)
-    scatter_in_place<C, true>(s_ke, me, d, shift, mask, sshift, s_cur_e);
+    scatter_in_place<C, false, false>(s_ks, np, d, shift, mask, sshift, s_cur_s, np);   // (the barriers of the next call cover it)
+    scatter_in_place<C, true>(s_ke, me, d, shift, mask, sshift, s_cur_e, total[1]);
     qsum += write_and_rank<C, false>(s_ks, np, mask, sshift, s_cur_s, gbase, a.dst[0], a.q_sorted[0], qlo0, qhi0, qf0);
     // ends: n_in ends of earlier pairs lie in this bin, so it begins at gbase - n_in in B_E
     qsum -= write_and_rank<C, true>(s_ke, total[1], mask, sshift, s_cur_e, gbase - n_in, a.dst[1], a.q_sorted[1], qlo1, qhi1, qf1);
