@@ -483,7 +483,7 @@ def test_mc_permute_b_redo_path_gives_the_same_counts():
         bits.set_option("mc_fused", 1)
 
 
-@pytest.mark.parametrize("n_b,n_chrom,max_len", [(3_300_001, 1, 700), (17_000_003, 24, 400), (1_234_567, 900, 50)])
+@pytest.mark.parametrize("n_b,n_chrom,max_len", [(3_300_001, 1, 700), (17_000_003, 24, 400), (1_234_567, 900, 50), (4_000_003, 2, 300)])
 def test_mc_permute_b_other_shapes(n_b, n_chrom, max_len):
     """Fused rounds on set sizes, tile counts and chromosome tables other than config 5's."""
     rng = np.random.default_rng(n_chrom)
@@ -491,6 +491,8 @@ def test_mc_permute_b_other_shapes(n_b, n_chrom, max_len):
         lens = np.array(W.GENOME24_LENGTHS)
     elif n_chrom == 1:
         lens = np.array([1_500_000_000])
+    elif n_chrom == 2:
+        lens = np.array([2**32 - 1 - 3_000_000, 3_000_000])      # the largest genome the coordinate space holds: keys up to 2^32 - 2
     else:
         lens = rng.integers(200_000, 4_000_000, n_chrom)
     off = W.genome_offsets(lens)
