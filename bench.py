@@ -47,6 +47,14 @@ NCU_LIMITER: dict = {
     "place_tile_kernel": {"issue_slots_busy": 0.525, "shared_memory_pipe": 0.472, "dram_throughput": 0.132,
                           "note": "dependent-instruction latency at one 1024-thread block per SM"},
 }
+# warp instructions per launch from the same capture (smsp__inst_executed.sum): with the live launch duration and
+# SM clock they give the share of the issue slots the kernel fills (148 SMs x 4 schedulers x 1 warp instruction per
+# cycle, B300_MICROARCH.md / DESIGN.md section 7) -- the bound the two kernels actually run into
+NCU_WARP_INSTRUCTIONS: dict = {
+    "bin_sort_search_kernel": 94_840_309,
+    "place_tile_kernel": 35_762_284,
+}
+N_SMS, SCHEDULERS_PER_SM = 148, 4
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
@@ -419,6 +427,9 @@ def run_b200(args):
                         "kernel_ms_per_round": {k: v[0] / (R * prof_steps) for k, v in timed.items()},
                         "timed_in": f"{prof_steps} extra step(s) right behind the timed region, one event pair per launch",
                         "kernel_share_of_step": {k: v[0] / tot for k, v in timed.items()}}
+            if kname in NCU_WARP_INSTRUCTIONS and args.config == 5 and args.scale == 1.0:
+                roofline["issue_slots"] = {"warp_instructions_per_launch": NCU_WARP_INSTRUCTIONS[kname],
+                                           "peak_per_s_formula": "148 SMs x 4 schedulers x sm_mhz (filled in below)"}
             if n_sorted:
                 # SURVEY 8(d) per-round model: place 12 M + sort 72 M (histogram fused: - 8 M) + search 8 N_q
                 model = 12 * n_sorted + 72 * n_sorted - 8 * n_sorted + 8 * w.n_a
@@ -442,6 +453,18 @@ def run_b200(args):
         line["roofline"] = roofline
     if clocks is not None:
         line["clocks"] = clocks
+    if roofline and "issue_slots" in roofline:
+        mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz")
+        if mhz:
+            iss = roofline["issue_slots"]
+            iss.pop("peak_per_s_formula", None)
+            iss["achieved_per_s"] = iss["warp_instructions_per_launch"] / (roofline["avg_launch_ms"] * 1e-3)
+            iss["peak_per_s"] = N_SMS * SCHEDULERS_PER_SM * mhz * 1e6
+            iss["frac"] = iss["achieved_per_s"] / iss["peak_per_s"]
+            iss["note"] = ("share of the issue slots (148 SMs x 4 schedulers x sm_mhz) filled during the launch: instruction "
+                           "count from the committed ncu capture, duration and clock measured in this run")
+        else:
+            del roofline["issue_slots"]
 
     # ---- end to end through the host-buffer entry point (H2D + run + D2H inside the timed region) ----
     if not args.no_extras:
