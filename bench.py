@@ -37,21 +37,21 @@ if ROOT not in sys.path:
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
 NCU_TRAFFIC_BYTES: dict = {
     # profiles/r1b_fused_ncu_full_summary.txt (config 5, one launch)
-    "bin_sort_search_kernel": 128_288_000,     # 91.32 MB read + 36.97 MB written
-    "place_tile_kernel": 71_345_152,           # 40.10 MB read + 31.24 MB written
+    "bin_sort_search_kernel": 128_459_264,     # 91.32 MB read + 37.14 MB written
+    "place_tile_kernel": 70_430_464,           # 40.11 MB read + 30.32 MB written
 }
 # what the same capture says bounds each kernel (neither is near its HBM roofline)
 NCU_LIMITER: dict = {
-    "bin_sort_search_kernel": {"issue_slots_busy": 0.709, "shared_memory_pipe": 0.646, "dram_throughput": 0.123,
+    "bin_sort_search_kernel": {"issue_slots_busy": 0.707, "shared_memory_pipe": 0.654, "dram_throughput": 0.124,
                                "note": "instruction issue and the shared-memory pipe, not HBM"},
-    "place_tile_kernel": {"issue_slots_busy": 0.525, "shared_memory_pipe": 0.472, "dram_throughput": 0.132,
+    "place_tile_kernel": {"issue_slots_busy": 0.524, "shared_memory_pipe": 0.473, "dram_throughput": 0.131,
                           "note": "dependent-instruction latency at one 1024-thread block per SM"},
 }
 # warp instructions per launch from the same capture (smsp__inst_executed.sum): with the live launch duration and
 # SM clock they give the share of the issue slots the kernel fills (148 SMs x 4 schedulers x 1 warp instruction per
 # cycle, B300_MICROARCH.md / DESIGN.md section 7) -- the bound the two kernels actually run into
 NCU_WARP_INSTRUCTIONS: dict = {
-    "bin_sort_search_kernel": 94_840_309,
+    "bin_sort_search_kernel": 93_573_124,
     "place_tile_kernel": 35_762_284,
 }
 N_SMS, SCHEDULERS_PER_SM = 148, 4
