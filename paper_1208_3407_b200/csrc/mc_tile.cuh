@@ -212,8 +212,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
         }
       }
     }
-    __syncthreads();
-    fence_proxy_async_smem();   // the staged pairs are about to be read by the bulk-copy engine
+    fence_proxy_async_smem();   // this thread's staged pairs are about to be read by the bulk-copy engine
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < kPer / 4; ++j) reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + j] = make_uint4(0, 0, 0, 0);
