@@ -299,6 +299,34 @@ def test_enumerate_config2_is_valid_and_complete():
     assert np.unique(pa * (1 << 32) + pb).size == n
 
 
+def test_enumerate_with_too_small_a_capacity_writes_a_prefix_only():
+    """include/bits.h: pairs at positions >= capacity are not written, *total_out is the full count either way."""
+    w = W.make_config(2, scale=0.05)
+    d = [dev(x) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    pa, pb, n = bits.enumerate_pairs(*d)
+    sync()
+    assert n > 1000
+    cap = n // 3
+    guard = 0x7fffffff
+    qa = torch.full((n,), guard, dtype=torch.int32, device=DEV)
+    qb = torch.full((n,), guard, dtype=torch.int32, device=DEV)
+    total = torch.zeros(1, dtype=torch.int64, device=DEV)
+    ws = torch.empty(bits.workspace_bytes(bits.FN_ENUMERATE, w.n_a, w.n_b), dtype=torch.uint8, device=DEV)
+    st = bits.lib().bits_enumerate(d[0].data_ptr(), d[1].data_ptr(), w.n_a, d[2].data_ptr(), d[3].data_ptr(), w.n_b, 0,
+                                   ws.data_ptr(), ws.numel(), qa.data_ptr(), qb.data_ptr(), cap, total.data_ptr(),
+                                   torch.cuda.current_stream().cuda_stream)
+    sync()
+    assert st == 0 and int(total.item()) == n
+    assert torch.equal(qa[:cap], pa[:cap])                 # A-major slices: the same positions hold the same a_i
+    got = torch.stack([qa[:cap], qb[:cap]], 1).cpu().numpy().astype(np.int64)
+    full = torch.stack([pa, pb], 1).cpu().numpy().astype(np.int64)
+    # inside one a_i the order of the b_j is unspecified: compare as sets per a_i over the a_i that fit entirely
+    last_a = int(got[-1, 0])
+    keep_g, keep_f = got[got[:, 0] < last_a], full[full[:, 0] < last_a]
+    assert np.array_equal(keep_g[np.lexsort((keep_g[:, 1], keep_g[:, 0]))], keep_f[np.lexsort((keep_f[:, 1], keep_f[:, 0]))])
+    assert bool((qa[cap:] == guard).all()) and bool((qb[cap:] == guard).all())
+
+
 def test_results_do_not_depend_on_programmatic_launch():
     """The kernels of a call are chained by programmatic dependent launch (option mc_pdl, on by default):
     with it off every launch is fully serialised.  Counts, pairs, decisions and Monte Carlo rounds must be
