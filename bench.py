@@ -131,6 +131,24 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def golden_round_counts(config: int, mc_seed: int):
+    """(header, uint64 counts) from tests/golden/cfg<k>_seed<s>_rounds.txt (the oracle's per-round counts, written by
+    tests/golden/make_golden.py), or (None, None) if there is no such file.  Reads the file only: no oracle code runs."""
+    path = os.path.join(ROOT, "tests", "golden", f"cfg{config}_seed{mc_seed}_rounds.txt")
+    if not os.path.exists(path):
+        return None, None
+    header, vals = None, []
+    with open(path) as f:
+        for ln in f:
+            ln = ln.strip()
+            if ln.startswith("#"):
+                if ln[1:].strip().startswith("{"):
+                    header = json.loads(ln[1:].strip())
+            elif ln:
+                vals.append(int(ln))
+    return header, np.array(vals, dtype=np.uint64)
+
+
 def workload_name(k: int) -> str:
     from paper_1208_3407_b200 import workloads as W
     return W.CONFIG_NAMES[k]
@@ -242,6 +260,53 @@ def l2_yardsticks(device):
             "l2_random_sector_gather_gbs_80MB": gather * 32}
 
 
+def library_yardsticks(device, w4, d4):
+    """SURVEY 8(d) "Yardsticks": cub::DeviceRadixSort::SortKeys and thrust upper_bound / lower_bound on the same
+    arrays on this box (bench-only code in probe/yardsticks.cu, never linked into libbits_b200.so).
+    w4, d4: config 4 and its device arrays (a_start, a_end, b_start, b_end)."""
+    import ctypes as C
+    import torch
+    from paper_1208_3407_b200 import bits
+    from paper_1208_3407_b200 import build as B
+    from paper_1208_3407_b200 import workloads as W
+    lib = C.CDLL(B.build_yardsticks())
+    lib.yard_cub_sort_temp_bytes.restype = C.c_size_t
+    lib.yard_cub_sort_temp_bytes.argtypes = [C.c_uint64]
+    lib.yard_cub_sort_keys_ms.restype = C.c_double
+    lib.yard_cub_sort_keys_ms.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_size_t, C.c_int, C.c_int, C.c_int, C.c_void_p]
+    lib.yard_thrust_bounds_ms.restype = C.c_double
+    lib.yard_thrust_bounds_ms.argtypes = [C.c_void_p] * 2 + [C.c_uint64] + [C.c_void_p] * 2 + [C.c_uint64] + [C.c_void_p] * 2 + [C.c_int, C.c_void_p]
+    st = torch.cuda.current_stream().cuda_stream
+    n = w4.n_b
+    tmp = torch.empty(max(int(lib.yard_cub_sort_temp_bytes(n)), 256), dtype=torch.uint8, device=device)
+    srt = [torch.empty(n, dtype=torch.int32, device=device) for _ in range(2)]
+    out = {}
+    # config 4: B's starts and B's ends (what bits_count* sorts once per call)
+    ms = [lib.yard_cub_sort_keys_ms(d4[2 + k].data_ptr(), srt[k].data_ptr(), n, tmp.data_ptr(), tmp.numel(), 0, 32, 5, st) for k in range(2)]
+    out["cub_sort_cfg4_B_2x1e7_keys"] = {"ms_both_arrays": sum(ms), "sort_keys_per_s": 2 * n / (sum(ms) * 1e-3)}
+    # the same two searches per query as count_kernel, as two vectorised library calls on the arrays cub just sorted
+    first = torch.empty(w4.n_a, dtype=torch.int32, device=device)
+    last = torch.empty(w4.n_a, dtype=torch.int32, device=device)
+    tb = lib.yard_thrust_bounds_ms(srt[0].data_ptr(), srt[1].data_ptr(), n, d4[1].data_ptr(), d4[0].data_ptr(), w4.n_a,
+                                   first.data_ptr(), last.data_ptr(), 3, st)
+    out["thrust_bounds_cfg4_1e7_queries"] = {"ms_upper_plus_lower": tb, "intervals_searched_per_s": w4.n_a / (tb * 1e-3),
+                                             "note": "ranks written to two arrays; no subtraction, no reduction"}
+    torch.cuda.synchronize()
+    want = bits.count_per_interval(*d4)[0]
+    torch.cuda.synchronize()
+    out["thrust_bounds_cfg4_1e7_queries"]["same_counts_as_library"] = bool(torch.equal(first - last, want))
+    del first, last, want
+    # config 5: the freshly placed keys of one round (what every PERMUTE_B round sorts)
+    w5 = W.make_config(5)
+    spans = to_dev((w5.b_end - w5.b_start).astype(np.uint32), device)
+    ps, pe = bits.place(spans, w5.chrom_offsets, w5.mc_seed, 0, 1)
+    torch.cuda.synchronize()
+    ms = [lib.yard_cub_sort_keys_ms(x.data_ptr(), srt[k].data_ptr(), w5.n_b, tmp.data_ptr(), tmp.numel(), 0, 32, 5, st)
+          for k, x in enumerate((ps, pe))]
+    out["cub_sort_cfg5_placed_2x1e7_keys"] = {"ms_both_arrays": sum(ms), "sort_keys_per_s": 2 * w5.n_b / (sum(ms) * 1e-3)}
+    return out
+
+
 def secondary_workloads(device, peak_gbs):
     """The other throughputs BASELINE.json's metric names, on their own configs (not the timed headline)."""
     import torch
@@ -271,6 +336,7 @@ def secondary_workloads(device, peak_gbs):
         "hbm_bytes_model": 72 * w.n_b + 12 * w.n_a + 8 * w.n_b,
         "hbm_frac_of_peak": (72 * w.n_b + 12 * w.n_a + 8 * w.n_b) / (med * 1e-3) / 1e9 / peak_gbs,
     }
+    out["yardsticks"] = library_yardsticks(device, w, d)
     del d, ws, counts
     # config 3: 1e4 queries re-placed per round against a fixed 1e6-interval B, 10,000 rounds, fused kernel
     w = W.make_config(3)
@@ -296,22 +362,38 @@ def secondary_workloads(device, peak_gbs):
     out["cfg2_enumerate"] = {"pairs": n_pairs, "pairs_per_s": n_pairs / (med * 1e-3), "ms_median": med, "ms_min": mn}
     med, mn = time_device(lambda: bits.decide(*d, workspace=ws), 5)
     out["cfg2_decide"] = {"ms_median": med, "ms_min": mn}
-    # the paper's screen on synthetic tracks (8 tracks of 1e5 intervals from config 2's recipe,
-    # 64 ordered pairs x 1000 rounds, queries re-placed); wall clock, the enrichment scores are host arithmetic
-    K, n_t, R_s = 8, 100_000, 1000
+    # the paper's screen (159 tracks, 25,281 ordered pairs) on synthetic tracks of 1e5
+    # intervals drawn from config 2's recipe, as ONE bits_screen call (every track sorted and indexed once, all pairs and
+    # rounds in gridded launches); 20 of the paper's 10,000 rounds per pair, device time by CUDA events
+    K, n_t, R_s = 159, 100_000, 20
     rng = np.random.default_rng(8)
-    tracks = []
-    for _ in range(K):
-        idx = rng.choice(w.n_b, n_t, replace=False)
-        tracks.append((to_dev(w.b_start[idx], device), to_dev(w.b_end[idx], device)))
-    bits.screen(tracks[:2], w.chrom_offsets, 1, 10)
-    t0 = time.perf_counter()
-    _, enr, _ = bits.screen(tracks, w.chrom_offsets, 1, R_s)
-    dt = time.perf_counter() - t0
-    out["screen_8_tracks_of_1e5"] = {"pairs": K * K, "rounds_per_pair": R_s, "seconds": dt,
-                                     "pair_rounds_per_s": K * K * R_s / dt, "intervals_searched_per_s": K * K * R_s * n_t / dt,
-                                     "enrichment_diag_mean": float(np.mean(np.diag(enr))),
-                                     "enrichment_offdiag_mean": float(np.mean(enr[~np.eye(K, dtype=bool)]))}
+    idx = [rng.choice(w.n_b, n_t, replace=False) for _ in range(K)]
+    starts = to_dev(np.concatenate([w.b_start[i] for i in idx]), device)
+    ends = to_dev(np.concatenate([w.b_end[i] for i in idx]), device)
+    toff = np.arange(K + 1, dtype=np.uint64) * n_t
+    obs_s = torch.empty((K, K), dtype=torch.int64, device=device)
+    rc_s = torch.empty((K, K, R_s), dtype=torch.int64, device=device)
+    ws = torch.empty(int(bits.lib().bits_screen_workspace_bytes(toff.ctypes.data, K, 24)), dtype=torch.uint8, device=device)
+    run = lambda R: bits.screen_concat(starts, ends, toff, w.chrom_offsets, 1, R, workspace=ws, observed_out=obs_s,
+                                       round_counts_out=rc_s[:, :, :R].contiguous() if R != R_s else rc_s)
+    launches0 = bits.launch_count()
+    med0, _ = time_device(lambda: run(0), 2, warmup=1)               # setup + observed counts only
+    med, mn = time_device(lambda: run(R_s), 2, warmup=1)
+    per_call_launches = (bits.launch_count() - launches0) // 6
+    enr = bits.screen_enrichment(obs_s.cpu().numpy().view(np.uint64), rc_s.cpu().numpy().view(np.uint64))
+    rounds_ms = max(med - med0, 1e-6)
+    sectors_per_interval = 6.0      # two index words + four key sectors per ICOUNT (search.cuh rank_le x 2)
+    out["screen_159_tracks_of_1e5"] = {
+        "tracks": K, "pairs": K * K, "intervals_per_track": n_t, "rounds_per_pair": R_s, "ms_median": med, "ms_min": mn,
+        "setup_and_observed_ms": med0, "launches_per_call": per_call_launches, "synchronisations_per_call": 1,
+        "pair_rounds_per_s": K * K * R_s / (rounds_ms * 1e-3),
+        "intervals_searched_per_s": K * K * R_s * n_t / (rounds_ms * 1e-3),
+        "l2_sectors_per_s_model": K * K * R_s * n_t * sectors_per_interval / (rounds_ms * 1e-3),
+        "paper_scale_estimate_s": {"pairs": K * K, "rounds": 10_000, "seconds": med0 * 1e-3 + rounds_ms * 1e-3 * 10_000 / R_s,
+                                   "paper": "9,069 min on one GPU of 2012 for 25,281 pairs x 10,000 rounds of the ENCODE/UCSC "
+                                            "tracks (PAPER.md:171; other data, other hardware: context only)"},
+        "enrichment_diag_mean": float(np.mean(np.diag(enr))),
+        "enrichment_offdiag_mean": float(np.mean(enr[~np.eye(K, dtype=bool)]))}
     return out
 
 
@@ -449,6 +531,16 @@ def run_b200(args):
         "sort_keys_per_s": (2 * n_sorted * value) if n_sorted else None,
         "profile_events_in_timed_region": False,
     }
+    # the counts of the step that was timed against the oracle's golden per-round counts (full configs only)
+    g_head, g_counts = golden_round_counts(args.config, w.mc_seed) if args.scale == 1.0 else (None, None)
+    if g_head is not None and g_head.get("checksums") == w.checksums() and r0 + R <= g_counts.size:
+        got = rc.cpu().numpy().view(np.uint64)
+        line["golden_match"] = bool(np.array_equal(got, g_counts[r0:r0 + R]) and
+                                    int(obs.cpu().numpy().view(np.uint64)[0]) == g_head["observed"])
+        line["golden"] = {"file": f"tests/golden/cfg{args.config}_seed{w.mc_seed}_rounds.txt", "rounds_compared": R,
+                          "round_begin": r0, "source": "CPU oracle over disjoint round slices (tests/golden/make_golden.py)"}
+    else:
+        line["golden_match"] = None
     if roofline:
         line["roofline"] = roofline
     if clocks is not None:

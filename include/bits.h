@@ -28,6 +28,13 @@
  *   - Sizes: n_a, n_b < 2^32.  Degenerate sizes are legal: n_a == 0 or n_b == 0 gives total 0,
  *     all per-interval counts 0 and all round counts 0.
  *   - All results are integers: per-interval counts uint32, totals and round counts uint64.
+ *   - Threads: the library keeps no state between calls except (a) the tuning knobs of
+ *     bits_set_option and the event timers of bits_profile_read, which are THREAD-LOCAL (a host
+ *     thread sees only the knobs it set itself), (b) the launch counter of bits_launch_count
+ *     (atomic, process-wide) and (c) a per-device "kernel attributes are set" flag (atomic).
+ *     Calls from different host threads are independent as long as their workspaces and streams are.
+ *   - Devices: every call runs on the CUDA device that is current in the calling thread; pointers
+ *     and stream must belong to it.  Any number of devices may be used from one process.
  */
 #ifndef BITS_B200_H_
 #define BITS_B200_H_
@@ -146,8 +153,13 @@ int bits_count_per_interval(const uint32_t* a_start, const uint32_t* a_end, uint
  * chrom_offsets: HOST uint32[n_chrom + 1], off[0] = 0, strictly ascending, off[n_chrom] = G <= 2^32-1
  * (read before the call returns).  Every interval of the permuted set must satisfy end < G.
  * observed_out: dev uint64[1]; round_counts_out: dev uint64[n_rounds].
- * Synchronises `stream` once (the longest span of the permuted set is checked against the
- * longest chromosome: BITS_ERR_NO_PLACEMENT). */
+ * BITS_B_SORTED together with BITS_PERMUTE_B is rejected (BITS_ERR_FLAGS): arrays sorted each on its
+ * own no longer pair a start with its end, so the lengths the re-placement must keep are lost.
+ * Synchronisation: `stream` is synchronised once before the first round (the longest span of the
+ * permuted set is checked against the longest chromosome: BITS_ERR_NO_PLACEMENT) and, with
+ * BITS_PERMUTE_B, once more per 4,096 rounds (overflow flags of the fused rounds are read back; a
+ * flagged round is redone by the general path).  After such a redo the "sorted arrays of the last
+ * round" (bits_workspace_sorted_offset) are those of the round that was redone last. */
 int bits_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
                    const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
                    const uint32_t* chrom_offsets, uint32_t n_chrom, int which, uint64_t seed,
@@ -200,6 +212,33 @@ double bits_pvalue(uint64_t observed, const uint64_t* round_counts, uint32_t n_r
  * observed 0 with a positive median: -inf.  NaN for n_rounds == 0 or a NULL array. */
 double bits_enrichment(uint64_t observed, const uint64_t* round_counts, uint32_t n_rounds);
 
+/* The many-pair screen as one device job (Sec. 3.3: every pairwise comparison of K interval
+ * sets by the Monte Carlo simulation; Fig. 3 caption :224: score = log2(observed / median of the simulated counts)).
+ * The K tracks are passed concatenated: track t = starts/ends[track_offsets[t] .. track_offsets[t+1]) (dev uint32;
+ * track_offsets: HOST uint64[n_tracks + 1], [0] = 0, non-decreasing, last < 2^32; n_tracks <= 65535).
+ * For every ORDERED pair (i, j), p = i * n_tracks + j:
+ *   observed_out[p] = |I(T_i, T_j)|                                            (dev uint64[n_tracks^2])
+ *   round_counts_out[p * n_rounds + k] = total(T_i', T_j), k in [0, n_rounds)     (dev uint64[n_tracks^2 * n_rounds])
+ * where T_i' is track i re-placed for round r = round_begin + k exactly as in bits_mc_rounds with
+ * BITS_PERMUTE_A, except that the fourth Philox counter word is the pair id p: interval q of track i draws
+ * counter (q >> 1, r, 0, p).  Every pair therefore has its own null draws, and pair (0, 0) reproduces
+ * bits_mc_rounds(T_0, T_0, BITS_PERMUTE_A) (reading R24).
+ * Every track is sorted and indexed once; all (pair, round) work runs in gridded launches with no host
+ * round trip in between.  flags: BITS_VALIDATE only.  Synchronises `stream` once (longest span of any track
+ * against the longest chromosome: BITS_ERR_NO_PLACEMENT, only if n_rounds > 0).  Empty tracks are legal (counts 0).
+ * Workspace: bits_screen_workspace_bytes(track_offsets, n_tracks, n_chrom) (0 for a bad offset table). */
+size_t bits_screen_workspace_bytes(const uint64_t* track_offsets, uint32_t n_tracks, uint32_t n_chrom);
+int bits_screen(const uint32_t* starts, const uint32_t* ends, const uint64_t* track_offsets, uint32_t n_tracks,
+                const uint32_t* chrom_offsets, uint32_t n_chrom, uint64_t seed,
+                uint32_t round_begin, uint32_t n_rounds, uint32_t flags,
+                void* workspace, size_t workspace_bytes,
+                uint64_t* observed_out, uint64_t* round_counts_out, void* stream);
+
+/* bits_enrichment for every pair of a screen (all HOST pointers): enrichment_out[p] =
+ * bits_enrichment(observed[p], round_counts + p * n_rounds, n_rounds), p in [0, n_pairs). */
+int bits_screen_enrichment(const uint64_t* observed, const uint64_t* round_counts, uint64_t n_pairs,
+                           uint32_t n_rounds, double* enrichment_out);
+
 /* Kernels launched by this library in this process since load (for bench.py's gpu_launches). */
 uint64_t bits_launch_count(void);
 
@@ -212,8 +251,9 @@ uint64_t bits_launch_count(void);
  * events.  ms_out / launches_out: host pointers, may be NULL. */
 int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out);
 
-/* Tuning knobs for design studies (bench.py --study); returns BITS_ERR_FLAGS for an unknown
- * name.  They never change results.  Names are listed in DESIGN.md "Knobs". */
+/* Tuning knobs for design studies (bench.py --opt NAME=VALUE); returns BITS_ERR_FLAGS for an unknown
+ * name or a value out of range.  They never change results.  Thread-local (see "Threads" above).
+ * Names are listed in DESIGN.md "Knobs". */
 int bits_set_option(const char* name, int64_t value);
 
 const char* bits_strerror(int status);

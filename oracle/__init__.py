@@ -43,8 +43,12 @@ def lib():
         L.oracle_place_from_bits.argtypes = [C.c_uint64, C.c_uint32, _u32p, C.c_uint32, _u32p]
         L.oracle_place_round.argtypes = [_u32p, C.c_uint64, _u32p, C.c_uint32, C.c_uint64, C.c_uint32,
                                          C.c_uint32, _u32p, _u32p]
+        L.oracle_place_round_stream.argtypes = [_u32p, C.c_uint64, _u32p, C.c_uint32, C.c_uint64, C.c_uint32,
+                                                C.c_uint32, C.c_uint32, _u32p, _u32p]
         L.oracle_mc_rounds.argtypes = [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, _u32p, C.c_uint32,
                                        C.c_int, C.c_uint64, C.c_uint32, C.c_uint32, _u64p, _u64p]
+        L.oracle_mc_rounds_stream.argtypes = [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, _u32p, C.c_uint32,
+                                              C.c_int, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _u64p, _u64p]
         L.oracle_pvalue.argtypes = [C.c_uint64, _u64p, C.c_uint32, C.c_int]
         L.oracle_pvalue.restype = C.c_double
         L.oracle_enrichment.argtypes = [C.c_uint64, _u64p, C.c_uint32]
@@ -131,19 +135,21 @@ def place_from_bits(x: int, d: int, chrom_offsets) -> int:
     return int(s.value)
 
 
-def place_round(spans, chrom_offsets, seed: int, rnd: int, tag: int):
+def place_round(spans, chrom_offsets, seed: int, rnd: int, tag: int, stream: int = 0):
+    """One round's placement; `stream` is the fourth Philox counter word (0 = a single job, pair id in the screen)."""
     sp, spp = _a32(spans)
     off, offp = _a32(chrom_offsets)
     s = np.zeros(sp.size, dtype=np.uint32)
     e = np.zeros(sp.size, dtype=np.uint32)
-    _chk(lib().oracle_place_round(spp, sp.size, offp, off.size - 1, C.c_uint64(seed), C.c_uint32(rnd),
-                                  C.c_uint32(tag), s.ctypes.data_as(_u32p), e.ctypes.data_as(_u32p)))
+    _chk(lib().oracle_place_round_stream(spp, sp.size, offp, off.size - 1, C.c_uint64(seed), C.c_uint32(rnd),
+                                         C.c_uint32(tag), C.c_uint32(stream), s.ctypes.data_as(_u32p),
+                                         e.ctypes.data_as(_u32p)))
     return s, e
 
 
 def mc_rounds(a_start, a_end, b_start, b_end, chrom_offsets, which: int, seed: int,
-              round_begin: int, n_rounds: int):
-    """-> (observed:int, round_counts:uint64[n_rounds])."""
+              round_begin: int, n_rounds: int, stream: int = 0):
+    """-> (observed:int, round_counts:uint64[n_rounds]).  stream: fourth Philox counter word of every draw."""
     a_s, asp = _a32(a_start)
     a_e, aep = _a32(a_end)
     b_s, bsp = _a32(b_start)
@@ -151,10 +157,31 @@ def mc_rounds(a_start, a_end, b_start, b_end, chrom_offsets, which: int, seed: i
     off, offp = _a32(chrom_offsets)
     obs = C.c_uint64(0)
     rc = np.zeros(max(n_rounds, 1), dtype=np.uint64)
-    _chk(lib().oracle_mc_rounds(asp, aep, a_s.size, bsp, bep, b_s.size, offp, off.size - 1, which,
-                                C.c_uint64(seed), C.c_uint32(round_begin), C.c_uint32(n_rounds),
-                                C.byref(obs), rc.ctypes.data_as(_u64p)))
+    _chk(lib().oracle_mc_rounds_stream(asp, aep, a_s.size, bsp, bep, b_s.size, offp, off.size - 1, which,
+                                       C.c_uint64(seed), C.c_uint32(stream), C.c_uint32(round_begin),
+                                       C.c_uint32(n_rounds), C.byref(obs), rc.ctypes.data_as(_u64p)))
     return int(obs.value), rc[:n_rounds]
+
+
+def screen(tracks, chrom_offsets, seed: int, round_begin: int, n_rounds: int):
+    """The paper's co-localisation screen (Sec. 3.3: every pairwise comparison of K interval
+    sets by the Monte Carlo simulation; Fig. 3 caption :224: score = log2(observed / median of the simulated
+    counts)).  For every ORDERED pair (i, j), in row-major order: observed = |I(T_i, T_j)|; per round track i
+    is re-placed (lengths kept, chromosome ends respected) and counted against the fixed track j; the draws of
+    pair (i, j) come from Philox stream (fourth counter word) i * K + j, so every pair has its own null
+    (reading R24).  `tracks` = [(start, end), ...].
+    -> (observed uint64[K, K], round_counts uint64[K, K, n_rounds], enrichment float64[K, K])."""
+    K = len(tracks)
+    obs = np.zeros((K, K), dtype=np.uint64)
+    rc = np.zeros((K, K, n_rounds), dtype=np.uint64)
+    enr = np.full((K, K), np.nan, dtype=np.float64)
+    for i in range(K):
+        for j in range(K):
+            o, r = mc_rounds(tracks[i][0], tracks[i][1], tracks[j][0], tracks[j][1], chrom_offsets, 0, seed,
+                             round_begin, n_rounds, stream=i * K + j)
+            obs[i, j], rc[i, j] = o, r
+            enr[i, j] = enrichment(o, r)
+    return obs, rc, enr
 
 
 def enrichment(observed: int, round_counts) -> float:

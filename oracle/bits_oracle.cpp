@@ -24,6 +24,9 @@
 //                              kept and chromosome ends respected (DESIGN.md readings
 //                              R10-R12).
 //   oracle_mc_rounds           the Monte Carlo loop of PAPER.md:157-159.
+//   oracle_mc_rounds_stream    the same with the fourth Philox counter word given (the pair id of
+//                              the many-pair screen; the screen itself is the
+//                              loop over ordered pairs in oracle/__init__.py).
 //   oracle_pvalue              add-one empirical p (reading R13; the paper gives
 //                              no formula).
 //
@@ -86,12 +89,14 @@ inline int place_from_bits(uint64_t x, uint32_t d, const uint32_t* off, uint32_t
   return 1;  // unreachable: u < V
 }
 
+// `stream` is the fourth counter word: 0 for a single Monte Carlo job, the pair id inside the many-pair
+// screen (SURVEY.md section 8(f).3 reserves it; readings R11, R24).
 inline int place_round(const uint32_t* spans, uint64_t n, const uint32_t* off, uint32_t n_chrom,
-                       uint64_t seed, uint32_t round, uint32_t tag,
+                       uint64_t seed, uint32_t round, uint32_t tag, uint32_t stream,
                        uint32_t* start_out, uint32_t* end_out) {
   const uint32_t key[2] = {static_cast<uint32_t>(seed & 0xffffffffu), static_cast<uint32_t>(seed >> 32)};
   for (uint64_t i = 0; i < n; ++i) {
-    const uint32_t ctr[4] = {static_cast<uint32_t>(i >> 1), round, tag, 0u};
+    const uint32_t ctr[4] = {static_cast<uint32_t>(i >> 1), round, tag, stream};
     uint32_t o[4];
     philox4x32_10(ctr, key, o);
     const uint32_t h = static_cast<uint32_t>(i & 1);
@@ -157,19 +162,26 @@ int oracle_place_from_bits(uint64_t x, uint32_t d, const uint32_t* off, uint32_t
   return place_from_bits(x, d, off, n_chrom, start_out) ? ORACLE_ERR_NO_PLACEMENT : ORACLE_OK;
 }
 
-int oracle_place_round(const uint32_t* spans, uint64_t n, const uint32_t* off, uint32_t n_chrom,
-                       uint64_t seed, uint32_t round, uint32_t tag,
-                       uint32_t* start_out, uint32_t* end_out) {
-  return place_round(spans, n, off, n_chrom, seed, round, tag, start_out, end_out)
+int oracle_place_round_stream(const uint32_t* spans, uint64_t n, const uint32_t* off, uint32_t n_chrom,
+                              uint64_t seed, uint32_t round, uint32_t tag, uint32_t stream,
+                              uint32_t* start_out, uint32_t* end_out) {
+  return place_round(spans, n, off, n_chrom, seed, round, tag, stream, start_out, end_out)
              ? ORACLE_ERR_NO_PLACEMENT : ORACLE_OK;
 }
 
+int oracle_place_round(const uint32_t* spans, uint64_t n, const uint32_t* off, uint32_t n_chrom,
+                       uint64_t seed, uint32_t round, uint32_t tag,
+                       uint32_t* start_out, uint32_t* end_out) {
+  return oracle_place_round_stream(spans, n, off, n_chrom, seed, round, tag, 0u, start_out, end_out);
+}
+
 // which: 0 = re-place A (queries; B sorted once), 1 = re-place B (searched set; re-sorted every round).
-int oracle_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
-                     const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
-                     const uint32_t* off, uint32_t n_chrom, int which, uint64_t seed,
-                     uint32_t round_begin, uint32_t n_rounds,
-                     uint64_t* observed_out, uint64_t* round_counts_out) {
+// stream: the fourth Philox counter word of every draw (0 = a single job; pair id in the screen).
+int oracle_mc_rounds_stream(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                            const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                            const uint32_t* off, uint32_t n_chrom, int which, uint64_t seed, uint32_t stream,
+                            uint32_t round_begin, uint32_t n_rounds,
+                            uint64_t* observed_out, uint64_t* round_counts_out) {
   if (which != 0 && which != 1) return ORACLE_ERR_ARG;
   if (!well_formed(a_start, a_end, n_a) || !well_formed(b_start, b_end, n_b)) return ORACLE_ERR_MALFORMED;
   // 1. observed = total(A, B)
@@ -186,7 +198,7 @@ int oracle_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_
   // 3-4. rounds
   for (uint32_t k = 0; k < n_rounds; ++k) {
     const uint32_t r = round_begin + k;
-    if (n_p && place_round(spans.data(), n_p, off, n_chrom, seed, r, static_cast<uint32_t>(which),
+    if (n_p && place_round(spans.data(), n_p, off, n_chrom, seed, r, static_cast<uint32_t>(which), stream,
                            s2.data(), e2.data()))
       return ORACLE_ERR_NO_PLACEMENT;
     if (which == 0) {
@@ -199,6 +211,15 @@ int oracle_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_
     }
   }
   return ORACLE_OK;
+}
+
+int oracle_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                     const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                     const uint32_t* off, uint32_t n_chrom, int which, uint64_t seed,
+                     uint32_t round_begin, uint32_t n_rounds,
+                     uint64_t* observed_out, uint64_t* round_counts_out) {
+  return oracle_mc_rounds_stream(a_start, a_end, n_a, b_start, b_end, n_b, off, n_chrom, which, seed, 0u,
+                                 round_begin, n_rounds, observed_out, round_counts_out);
 }
 
 // tail 0: p_enrich = (#{count_r >= observed} + 1) / (R + 1); tail 1: p_deplete with <=.

@@ -51,6 +51,10 @@ _SIGNATURES = {
                                       _vp]),
     "bits_pvalue": (C.c_double, [C.c_uint64, _u64p, C.c_uint32, C.c_int]),
     "bits_enrichment": (C.c_double, [C.c_uint64, _u64p, C.c_uint32]),
+    "bits_screen_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_uint32, C.c_uint32]),
+    "bits_screen": (C.c_int, [_u32p, _u32p, C.c_void_p, C.c_uint32, _u32p, C.c_uint32, C.c_uint64, C.c_uint32, C.c_uint32,
+                              C.c_uint32, _vp, C.c_size_t, _u64p, _u64p, _vp]),
+    "bits_screen_enrichment": (C.c_int, [_u64p, _u64p, C.c_uint64, C.c_uint32, C.c_void_p]),
     "bits_launch_count": (C.c_uint64, []),
     "bits_profile_read": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p]),
     "bits_set_option": (C.c_int, [C.c_char_p, C.c_int64]),
@@ -294,28 +298,51 @@ def enrichment(observed: int, round_counts) -> float:
     return float(lib().bits_enrichment(int(observed), rc.ctypes.data if rc.size else 0, rc.size))
 
 
-def screen(tracks, chrom_offsets, seed: int, n_rounds: int, which: int = PERMUTE_A, round_begin: int = 0):
-    """The paper's co-localisation screen (Fig. 3): for every ordered pair (i, j) of the K
-    interval sets in `tracks` (each a (start, end) pair of device tensors) the observed count, `n_rounds`
-    Monte Carlo rounds and log2(observed / median).  Returns (observed int64[K, K], enrichment float64[K, K],
-    round_counts uint64[K, K, n_rounds]) as numpy arrays.  Marshalling only: every count comes from
-    bits_mc_rounds; one workspace sized for the largest pair is reused."""
-    K = len(tracks)
+def screen_concat(starts, ends, track_offsets, chrom_offsets, seed: int, n_rounds: int, round_begin: int = 0,
+                  flags: int = 0, workspace=None, observed_out=None, round_counts_out=None):
+    """bits_screen on K tracks passed concatenated (device uint32 tensors + host offsets uint64[K + 1]) ->
+    (observed int64[K, K], round_counts int64[K, K, n_rounds]) device tensors, valid after stream sync."""
+    dev = starts.device
+    toff = np.ascontiguousarray(track_offsets, dtype=np.uint64)
+    K = toff.size - 1
     off = _offsets(chrom_offsets)
-    n_max = max(t[0].numel() for t in tracks)
-    dev = tracks[0][0].device
-    ws = torch.empty(max(workspace_bytes(FN_MC_ROUNDS, n_max, n_max, off.size - 1, which), 256), dtype=torch.uint8, device=dev)
-    obs = torch.empty((K, K), dtype=torch.int64, device=dev)
-    rc = torch.empty((K, K, n_rounds), dtype=torch.int64, device=dev)
-    for i in range(K):
-        for j in range(K):
-            mc_rounds(tracks[i][0], tracks[i][1], tracks[j][0], tracks[j][1], off, which, seed, round_begin, n_rounds,
-                      workspace=ws, observed_out=obs[i, j:j + 1], round_counts_out=rc[i, j])
-    torch.cuda.synchronize(dev)
-    obs_h = obs.cpu().numpy()
+    nbytes = int(lib().bits_screen_workspace_bytes(toff.ctypes.data, K, off.size - 1))
+    if nbytes == 0:
+        raise BitsError(2, "bad track offset table")
+    ws = _workspace(nbytes, workspace, dev)
+    obs = observed_out if observed_out is not None else torch.empty((K, K), dtype=torch.int64, device=dev)
+    rc = round_counts_out if round_counts_out is not None else torch.empty((K, K, n_rounds), dtype=torch.int64, device=dev)
+    _chk(lib().bits_screen(_dev_u32(starts, "starts"), _dev_u32(ends, "ends"), toff.ctypes.data, K, off.ctypes.data,
+                           off.size - 1, seed, round_begin, n_rounds, flags, ws.data_ptr(), ws.numel(), obs.data_ptr(),
+                           rc.data_ptr() if n_rounds else 0, _stream()))
+    return obs, rc
+
+
+def screen_enrichment(observed, round_counts) -> np.ndarray:
+    """bits_screen_enrichment on host arrays: log2(observed / median of the pair's round counts), shape of `observed`."""
+    o = np.ascontiguousarray(observed, dtype=np.uint64)
+    r = np.ascontiguousarray(round_counts, dtype=np.uint64)
+    n_rounds = r.size // o.size if o.size else 0
+    out = np.empty(o.shape, dtype=np.float64)
+    _chk(lib().bits_screen_enrichment(o.ctypes.data, r.ctypes.data if r.size else 0, o.size, n_rounds, out.ctypes.data))
+    return out
+
+
+def screen(tracks, chrom_offsets, seed: int, n_rounds: int, round_begin: int = 0):
+    """The paper's co-localisation screen (Fig. 3) over K interval sets, `tracks` = [(start, end)
+    device tensors]: one bits_screen call (every track sorted and indexed once, all pairs and rounds in gridded
+    launches, pair id in the Philox counter).  Returns numpy arrays (observed uint64[K, K], enrichment
+    float64[K, K], round_counts uint64[K, K, n_rounds]).  Marshalling only: the tracks are concatenated for the call."""
+    K = len(tracks)
+    toff = np.zeros(K + 1, dtype=np.uint64)
+    toff[1:] = np.cumsum([t[0].numel() for t in tracks])
+    starts = torch.cat([t[0] for t in tracks]) if K > 1 else tracks[0][0]
+    ends = torch.cat([t[1] for t in tracks]) if K > 1 else tracks[0][1]
+    obs, rc = screen_concat(starts, ends, toff, chrom_offsets, seed, n_rounds, round_begin)
+    torch.cuda.synchronize(starts.device)
+    obs_h = obs.cpu().numpy().view(np.uint64)
     rc_h = rc.cpu().numpy().view(np.uint64)
-    enr = np.array([[enrichment(int(obs_h[i, j]), rc_h[i, j]) for j in range(K)] for i in range(K)], dtype=np.float64)
-    return obs_h, enr, rc_h
+    return obs_h, screen_enrichment(obs_h, rc_h), rc_h
 
 
 def host_workspace(fn: int, n_a: int, n_b: int, n_chrom: int = 0, which: int = 0, n_rounds: int = 0,

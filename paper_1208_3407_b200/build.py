@@ -56,6 +56,21 @@ def build_probe(force: bool = False) -> str:
     return PROBE_LIB
 
 
+YARD_SRC = os.path.join(HERE, "probe", "yardsticks.cu")
+YARD_LIB = os.path.join(HERE, "probe", "libyardsticks.so")
+
+
+def build_yardsticks(force: bool = False) -> str:
+    """Compile the bench-only CUB / thrust yardsticks (probe/yardsticks.cu); never linked into libbits_b200.so."""
+    if not force and os.path.exists(YARD_LIB) and os.path.getmtime(YARD_SRC) <= os.path.getmtime(YARD_LIB):
+        return YARD_LIB
+    tmp = YARD_LIB + f".tmp{os.getpid()}"
+    subprocess.check_call([NVCC, *FLAGS, "-o", tmp, YARD_SRC])
+    os.replace(tmp, YARD_LIB)
+    return YARD_LIB
+
+
 if __name__ == "__main__":
     build_probe(force="--force" in sys.argv)
+    build_yardsticks(force="--force" in sys.argv)
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

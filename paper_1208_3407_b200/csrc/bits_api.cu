@@ -15,10 +15,11 @@
 #include "mc_tile.cuh"
 #include "search.cuh"
 #include "enumerate.cuh"
+#include "screen.cuh"
 
 namespace bits {
 
-unsigned long long g_launches = 0;
+std::atomic<unsigned long long> g_launches{0};
 
 struct Options {
   int64_t sort_msd = 1;            // 1 = MSD bucket sort with the LSD sort as device-side fallback, 0 = LSD sort only
@@ -32,9 +33,12 @@ struct Options {
   int64_t mc_tile_variant = 2;     // PERMUTE_B fused rounds: shape of place_tile_kernel (0: 2 x 512 threads, 1: 1 x 1024, 2: 1 x 1024 with longer tiles)
   int64_t mc_bin_variant = 0;      // PERMUTE_B fused rounds: shape of the per-bin sort (0 wide, 1 narrow, 2 small blocks)
   int64_t mc_gather_group = -1;    // PERMUTE_B fused rounds: log2 of the lanes per gathered segment (-1 = from the mean segment length)
+  int64_t mc_shift_bias = 0;       // PERMUTE_B fused rounds: added to the bin width (log2) the host picked; > 0 overflows bins on purpose (tests)
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
 };
-static Options g_opt;
+// Options and the per-kernel event timers belong to the calling host thread (bits.h, "Threads"): two threads
+// driving the library do not see each other's knobs.
+static thread_local Options g_opt;
 
 constexpr int kSMs = 148;
 constexpr size_t kMaxSmemPerBlock = 232448 - 2048;   // 227 KB opt-in limit of shared memory per block on sm_100, less room for static shared memory
@@ -65,7 +69,7 @@ struct Profiler {
   }
   void reset() { collect(); for (int i = 0; i < kNumCls; ++i) { ms[i] = 0; launches[i] = 0; } }
 };
-static Profiler g_prof;
+static thread_local Profiler g_prof;
 
 struct ProfScope {
   cudaStream_t st;
@@ -193,6 +197,7 @@ struct Layout {
   uint32_t* e_tie = nullptr;                     // [n_b + 1]
   uint32_t* e_end_by_start = nullptr;            // [n_b]
   uint32_t* e_idx_by_start = nullptr;            // [n_b]
+  uint32_t* e_max[3] = {nullptr, nullptr, nullptr};   // largest end per run of 32 / 1,024 / 32,768 positions of e_end_by_start
   size_t bytes = 0;
 };
 constexpr uint32_t kFlagChunk = 4096;    // fused rounds are checked for raised flags in chunks of this many
@@ -248,6 +253,9 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
       L.e_tie = c.take<uint32_t>(n_b + 4);
       L.e_end_by_start = c.take<uint32_t>(n_b + 4);
       L.e_idx_by_start = c.take<uint32_t>(n_b + 4);
+      L.e_max[0] = c.take<uint32_t>((n_b >> enu::kSkip1) + 4);
+      L.e_max[1] = c.take<uint32_t>((n_b >> enu::kSkip2) + 4);
+      L.e_max[2] = c.take<uint32_t>((n_b >> enu::kSkip3) + 4);
       break;
     case BITS_FN_PLACE:
       break;
@@ -340,10 +348,15 @@ static SortPlan plan_for(const SortCtx& c, const uint32_t* src0, const uint32_t*
   return p;
 }
 
-// One-time attribute setup for the kernels that use more than 48 KB of shared memory.
+// Attribute setup for the kernels that use more than 48 KB of shared memory: once per DEVICE
+// (cudaFuncSetAttribute applies to the current device only).
 static int msd_configure() {
-  static int done = -1;
-  if (done < 0) {
+  constexpr int kMaxDevices = 64;
+  static std::atomic<int> done_on[kMaxDevices];      // zero-initialised
+  int device = 0;
+  BITS_CUDA_TRY(cudaGetDevice(&device));
+  const bool tracked = device >= 0 && device < kMaxDevices;
+  if (!tracked || done_on[device].load(std::memory_order_acquire) == 0) {
     const cudaError_t e1 = cudaFuncSetAttribute(msd::scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kScSmem);
     const cudaError_t e2 = cudaFuncSetAttribute(msd::bucket_sort_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
     cudaError_t e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgWide>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -363,7 +376,7 @@ static int msd_configure() {
     if (e4 == cudaSuccess)
       e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024L::kSmem);
     if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { (void)cudaGetLastError(); return BITS_ERR_CUDA; }
-    done = 1;
+    if (tracked) done_on[device].store(1, std::memory_order_release);
   }
   return BITS_OK;
 }
@@ -606,6 +619,9 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
                    uint64_t* observed_out, uint64_t* round_counts_out, cudaStream_t st) {
   BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
   if (which != BITS_PERMUTE_A && which != BITS_PERMUTE_B) return BITS_ERR_FLAGS;
+  // independently sorted arrays no longer pair starts with ends: the lengths that re-placement must keep
+  // are gone
+  if (which == BITS_PERMUTE_B && (flags & BITS_B_SORTED)) return BITS_ERR_FLAGS;
   if (!observed_out || (n_rounds && !round_counts_out)) return BITS_ERR_NULL;
   if ((uint64_t)round_begin + n_rounds > (1ull << 32)) return BITS_ERR_SIZE;
   ChromTable chrom;
@@ -774,6 +790,10 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     // a small set: narrower bins (finer sub-buckets, more blocks) as long as there are no more bins than blocks
     while (best > 1 && fits(best - 1) && ((G + (1ull << (best - 1)) - 1) >> (best - 1)) <= 2ull * kSMs) --best;
     fused_ok = best >= 0;
+    if (fused_ok && g_opt.mc_shift_bias > 0) {     // tests: wider bins than the margin allows, so that bins overflow on the device
+      best += (int)g_opt.mc_shift_bias;
+      if (best > mct::kMaxShift) best = mct::kMaxShift;
+    }
     if (fused_ok) {
       pt.spans = L.spans; pt.n = (uint32_t)n_b; pt.tag = 1u; pt.key = key; pt.chrom = chrom;
       pt.shift = (uint32_t)best; pt.n_bins = (uint32_t)((G + (1ull << best) - 1) >> best);
@@ -847,6 +867,144 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out + done + j, 0, sizeof(uint64_t), st));
       BITS_TRY(general_round(done + j));
     }
+    done += chunk;
+  }
+  return BITS_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// The many-pair screen (screen.cuh).
+struct ScreenLayout {
+  Small small;
+  SortCtx scratch;                    // sort bookkeeping and the temp buffers, sized for the largest track
+  std::vector<uint32_t*> keys[2];     // per track: B_S, B_E
+  std::vector<uint32_t*> idx[2];      // per track: their bucket indices
+  std::vector<uint32_t*> spans;       // per track
+  scr::Track* tracks = nullptr;       // dev [K]
+  uint32_t* tile_track = nullptr;     // dev [n_tiles]
+  uint32_t* tile_first = nullptr;     // dev [K]
+  uint64_t n_tiles = 0;
+  size_t bytes = 0;
+};
+
+static ScreenLayout make_screen_layout(void* ws, const uint64_t* toff, uint32_t K, uint32_t n_chrom) {
+  ScreenLayout L;
+  Carver c(ws);
+  L.small.carve(c, n_chrom);
+  uint64_t n_max = 0;
+  for (uint32_t t = 0; t < K; ++t) {
+    const uint64_t n = toff[t + 1] - toff[t];
+    n_max = n > n_max ? n : n_max;
+    L.n_tiles += ceil_div(n, (uint64_t)scr::kTile);
+  }
+  L.scratch.carve(c, n_max, false);
+  for (int a = 0; a < 2; ++a) { L.keys[a].resize(K); L.idx[a].resize(K); }
+  L.spans.resize(K);
+  for (uint32_t t = 0; t < K; ++t) {
+    const uint64_t n = toff[t + 1] - toff[t];
+    const uint32_t shift = index_shift_for(n);
+    for (int a = 0; a < 2; ++a) L.keys[a][t] = c.take<uint32_t>(align_up(n + kPad, 64));
+    for (int a = 0; a < 2; ++a) L.idx[a][t] = c.take<uint32_t>(index_entries(shift));
+    L.spans[t] = c.take<uint32_t>(align_up(n, 4) + 4);
+  }
+  L.tracks = c.take<scr::Track>(K);
+  L.tile_track = c.take<uint32_t>(L.n_tiles + 1);
+  L.tile_first = c.take<uint32_t>((uint64_t)K + 1);
+  L.bytes = align_up(c.used, 256);
+  return L;
+}
+
+static int check_tracks(const uint64_t* toff, uint32_t K) {
+  if (!toff) return BITS_ERR_NULL;
+  if (K == 0 || K > 65535u) return BITS_ERR_SIZE;             // pair ids i * K + j are 32-bit Philox counter words
+  if (toff[0] != 0) return BITS_ERR_SIZE;
+  for (uint32_t t = 0; t < K; ++t)
+    if (toff[t + 1] < toff[t]) return BITS_ERR_SIZE;
+  if (toff[K] >= (1ull << 32)) return BITS_ERR_SIZE;
+  return BITS_OK;
+}
+
+static int screen_impl(const uint32_t* starts, const uint32_t* ends, const uint64_t* toff, uint32_t K, const uint32_t* off,
+                       uint32_t n_chrom, uint64_t seed, uint32_t round_begin, uint32_t n_rounds, uint32_t flags, void* ws,
+                       size_t ws_bytes, uint64_t* observed_out, uint64_t* round_counts_out, cudaStream_t st) {
+  BITS_TRY(check_tracks(toff, K));
+  if (flags & ~(uint32_t)BITS_VALIDATE) return BITS_ERR_FLAGS;
+  const uint64_t n_total = toff[K];
+  if (n_total && (!starts || !ends)) return BITS_ERR_NULL;
+  if (!observed_out || (n_rounds && !round_counts_out)) return BITS_ERR_NULL;
+  if ((uint64_t)round_begin + n_rounds > (1ull << 32)) return BITS_ERR_SIZE;
+  ChromTable chrom;
+  uint32_t l_max = 0;
+  BITS_TRY(check_genome(off, n_chrom, &chrom, &l_max));
+  const ScreenLayout L = make_screen_layout(ws, toff, K, n_chrom);
+  if (!ws_ok(ws, ws_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
+  if ((flags & BITS_VALIDATE) && n_total)
+    BITS_TRY(validate_inputs(starts, ends, (uint32_t)n_total, nullptr, nullptr, 0, L.small.bad, st));
+  BITS_TRY(upload_genome(off, n_chrom, L.small, &chrom, st));
+  const uint64_t n_pairs = (uint64_t)K * K;
+  BITS_CUDA_TRY(cudaMemsetAsync(observed_out, 0, sizeof(uint64_t) * n_pairs, st));
+  if (n_rounds) BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out, 0, sizeof(uint64_t) * n_pairs * n_rounds, st));
+  if (n_total == 0) return BITS_OK;
+
+  // spans of every track + the NO_PLACEMENT check over all of them (the call's one synchronisation)
+  BITS_CUDA_TRY(cudaMemsetAsync(L.small.max_span, 0, 4 * sizeof(uint32_t), st));
+  for (uint32_t t = 0; t < K; ++t) {
+    const uint32_t n = (uint32_t)(toff[t + 1] - toff[t]);
+    if (!n) continue;
+    spans_kernel<<<grid_for(n, 256), 256, 0, st>>>(starts + toff[t], ends + toff[t], n, L.spans[t], L.small.max_span, L.small.span_sum);
+    BITS_LAUNCH_CHECK();
+  }
+  uint32_t h_small[4] = {0, 0, 0, 0};
+  BITS_CUDA_TRY(cudaMemcpyAsync(h_small, L.small.max_span, sizeof(h_small), cudaMemcpyDeviceToHost, st));
+  BITS_CUDA_TRY(cudaStreamSynchronize(st));
+  if (n_rounds && h_small[0] >= l_max) return BITS_ERR_NO_PLACEMENT;
+
+  // every track sorted and indexed once
+  std::vector<scr::Track> h_tracks(K);
+  std::vector<uint32_t> h_tile_track((size_t)L.n_tiles + 1, 0u), h_tile_first((size_t)K + 1, 0u);
+  uint32_t epoch = 1, tile = 0;
+  BITS_TRY(reset_sort_ctx(L.scratch, st));
+  for (uint32_t t = 0; t < K; ++t) {
+    const uint64_t n = toff[t + 1] - toff[t];
+    SortCtx c = L.scratch;
+    c.n = (uint32_t)n; c.n_tiles = rs::num_tiles(n); c.shift = index_shift_for(n);
+    for (int a = 0; a < 2; ++a) { c.buf[a][0] = L.keys[a][t]; c.idx[a] = L.idx[a][t]; }
+    scr::Track& T = h_tracks[t];
+    T.start = starts + toff[t]; T.end = ends + toff[t]; T.spans = L.spans[t];
+    for (int a = 0; a < 2; ++a) { T.keys[a] = L.keys[a][t]; T.idx[a] = L.idx[a][t]; }
+    T.n = (uint32_t)n; T.shift = c.shift;
+    h_tile_first[t] = tile;
+    for (uint64_t k = 0; k < ceil_div(n, (uint64_t)scr::kTile); ++k) h_tile_track[tile++] = t;
+    if (!n) continue;
+    if (epoch > (1u << 30) - 16u) {       // epochs (30 bits) must not wrap
+      BITS_CUDA_TRY(cudaMemsetAsync(L.scratch.status[0], 0, sizeof(uint64_t) * (uint64_t)L.scratch.n_tiles * rs::kRadix, st));
+      BITS_CUDA_TRY(cudaMemsetAsync(L.scratch.status[1], 0, sizeof(uint64_t) * (uint64_t)L.scratch.n_tiles * rs::kRadix, st));
+      epoch = 1;
+    }
+    BITS_TRY(sort_arrays(c, T.start, T.end, 2, nullptr, false, &epoch, st));
+    BITS_TRY(launch_build_index(c, st));
+  }
+  BITS_CUDA_TRY(cudaMemcpyAsync(L.tracks, h_tracks.data(), sizeof(scr::Track) * K, cudaMemcpyHostToDevice, st));   // pageable: staged before return
+  BITS_CUDA_TRY(cudaMemcpyAsync(L.tile_track, h_tile_track.data(), sizeof(uint32_t) * (L.n_tiles + 1), cudaMemcpyHostToDevice, st));
+  BITS_CUDA_TRY(cudaMemcpyAsync(L.tile_first, h_tile_first.data(), sizeof(uint32_t) * ((size_t)K + 1), cudaMemcpyHostToDevice, st));
+
+  scr::ScreenArgs a;
+  a.tracks = L.tracks; a.tile_track = L.tile_track; a.tile_first = L.tile_first; a.n_tracks = K;
+  a.round0 = round_begin; a.out0 = 0; a.n_rounds = n_rounds; a.key = make_philox_keys(seed); a.chrom = chrom;
+  a.observed = reinterpret_cast<unsigned long long*>(observed_out);
+  a.round_counts = reinterpret_cast<unsigned long long*>(round_counts_out);
+  {
+    ProfScope prof(kClsCount, st);
+    scr::screen_kernel<true><<<dim3((unsigned)L.n_tiles, K, 1), scr::kThreads, 0, st>>>(a);
+    BITS_LAUNCH_CHECK();
+  }
+  for (uint32_t done = 0; done < n_rounds;) {
+    const uint32_t chunk = n_rounds - done < 4096u ? n_rounds - done : 4096u;
+    a.round0 = round_begin + done; a.out0 = done;
+    ProfScope prof(kClsMcA, st);
+    scr::screen_kernel<false><<<dim3((unsigned)L.n_tiles, K, chunk), scr::kThreads, 0, st>>>(a);
+    BITS_LAUNCH_CHECK();
     done += chunk;
   }
   return BITS_OK;
@@ -974,8 +1132,11 @@ int bits_enumerate(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   launch_pdl(enu::start_order_kernel, grid_for(n_b, 256), 256, 0, st, b_start, b_end, (uint32_t)n_b, sorted_set(L.b, 0), L.e_tie,
              L.e_end_by_start, L.e_idx_by_start);
   BITS_LAUNCH_CHECK();
+  BITS_CUDA_TRY(cudaMemsetAsync(L.e_max[2], 0, sizeof(uint32_t) * (((size_t)n_b >> enu::kSkip3) + 4), st));
+  launch_pdl(enu::end_maxima_kernel, (unsigned)ceil_div(n_b, 1024), 1024, 0, st, L.e_end_by_start, (uint32_t)n_b, L.e_max[0], L.e_max[1], L.e_max[2]);
+  BITS_LAUNCH_CHECK();
   launch_pdl(enu::emit_pairs_kernel, grid_for(n_a, 256), 256, 0, st, a_start, a_end, (uint32_t)n_a, sorted_set(L.b, 0), L.e_counts, L.e_offsets,
-             L.e_end_by_start, L.e_idx_by_start, pair_a_out, pair_b_out, capacity);
+             L.e_end_by_start, L.e_idx_by_start, L.e_max[0], L.e_max[1], L.e_max[2], pair_a_out, pair_b_out, capacity);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -1107,7 +1268,28 @@ double bits_enrichment(uint64_t observed, const uint64_t* round_counts, uint32_t
   return log2((double)observed / median);
 }
 
-uint64_t bits_launch_count(void) { return g_launches; }
+size_t bits_screen_workspace_bytes(const uint64_t* track_offsets, uint32_t n_tracks, uint32_t n_chrom) {
+  if (check_tracks(track_offsets, n_tracks) != BITS_OK) return 0;
+  return make_screen_layout(nullptr, track_offsets, n_tracks, n_chrom).bytes;
+}
+
+int bits_screen(const uint32_t* starts, const uint32_t* ends, const uint64_t* track_offsets, uint32_t n_tracks,
+                const uint32_t* chrom_offsets, uint32_t n_chrom, uint64_t seed, uint32_t round_begin, uint32_t n_rounds,
+                uint32_t flags, void* workspace, size_t workspace_bytes, uint64_t* observed_out,
+                uint64_t* round_counts_out, void* stream) {
+  return screen_impl(starts, ends, track_offsets, n_tracks, chrom_offsets, n_chrom, seed, round_begin, n_rounds, flags,
+                     workspace, workspace_bytes, observed_out, round_counts_out, static_cast<cudaStream_t>(stream));
+}
+
+int bits_screen_enrichment(const uint64_t* observed, const uint64_t* round_counts, uint64_t n_pairs, uint32_t n_rounds,
+                           double* enrichment_out) {
+  if (n_pairs && (!observed || !enrichment_out || (n_rounds && !round_counts))) return BITS_ERR_NULL;
+  for (uint64_t p = 0; p < n_pairs; ++p)
+    enrichment_out[p] = bits_enrichment(observed[p], n_rounds ? round_counts + p * n_rounds : nullptr, n_rounds);
+  return BITS_OK;
+}
+
+uint64_t bits_launch_count(void) { return g_launches.load(); }
 
 int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out) {
   if (cls < 0 || cls >= kNumCls) return BITS_ERR_FLAGS;
@@ -1127,6 +1309,7 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "mc_tile_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_tile_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 3) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_gather_group")) { if (value < -1 || value > 5) return BITS_ERR_FLAGS; g_opt.mc_gather_group = value; return BITS_OK; }
+  if (!strcmp(name, "mc_shift_bias")) { if (value < 0 || value > 8) return BITS_ERR_FLAGS; g_opt.mc_shift_bias = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }
   if (!strcmp(name, "place_fused_hist")) { g_opt.place_fused_hist = value; return BITS_OK; }

@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "../../include/bits.h"
 
 namespace bits {
@@ -11,7 +13,7 @@ constexpr int kWarp = 32;
 constexpr uint32_t kFullMask = 0xffffffffu;
 
 // Number of kernel launches made by the library (bits_launch_count()).
-extern unsigned long long g_launches;
+extern std::atomic<unsigned long long> g_launches;
 
 #define BITS_CUDA_TRY(expr)                              \
   do {                                                   \

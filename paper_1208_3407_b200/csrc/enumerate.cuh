@@ -111,12 +111,38 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(const uint32_t
   }
 }
 
-// One query per thread: walk B in start order downwards from `first`, emit until c(a) pairs are out.
+// Largest end of every run of 32 / 1,024 / 32,768 consecutive positions of end_by_start (three levels of
+// fan-out 32).  They bound the walk below: a run whose largest end lies before a.start holds no
+// intersection and is skipped whole.  Without them ONE long interval with a small start (a
+// chromosome-wide feature) would make every query that meets it scan all of B below its `first` --
+// the linear scan PAPER.md:63-67 warns about.  max3 is zero on entry.  1,024 threads per block.
+constexpr int kSkip1 = 5, kSkip2 = 10, kSkip3 = 15;
+__global__ void __launch_bounds__(1024) end_maxima_kernel(const uint32_t* __restrict__ end_by_start, uint32_t n_b,
+                                                          uint32_t* __restrict__ max1, uint32_t* __restrict__ max2, uint32_t* max3) {
+  __shared__ uint32_t s_m[32];
+  grid_dependency_wait();
+  const uint64_t i = (uint64_t)blockIdx.x * 1024 + threadIdx.x;
+  uint32_t m = i < n_b ? end_by_start[i] : 0u;
+  m = __reduce_max_sync(kFullMask, m);
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0) { s_m[w] = m; if (i < n_b) max1[i >> kSkip1] = m; }
+  __syncthreads();
+  if (w == 0) {
+    m = __reduce_max_sync(kFullMask, s_m[lane]);
+    if (lane == 0) { max2[blockIdx.x] = m; atomicMax(&max3[blockIdx.x >> (kSkip3 - kSkip2)], m); }
+  }
+}
+
+// One query per thread: walk B in start order downwards from `first`, emit until c(a) pairs are out; runs of 32,
+// 1,024 and 32,768 positions none of whose ends reaches a.start are stepped over through the maxima above, so
+// the walk costs O(32 * 3 + n_b / 32,768) steps per emitted pair at worst instead of O(n_b).
 __global__ void __launch_bounds__(256) emit_pairs_kernel(const uint32_t* __restrict__ a_start, const uint32_t* __restrict__ a_end,
                                                          uint32_t n_a, SortedSet bs, const uint32_t* __restrict__ counts,
                                                          const unsigned long long* __restrict__ offsets,
                                                          const uint32_t* __restrict__ end_by_start,
                                                          const uint32_t* __restrict__ idx_by_start,
+                                                         const uint32_t* __restrict__ max1, const uint32_t* __restrict__ max2,
+                                                         const uint32_t* __restrict__ max3,
                                                          uint32_t* __restrict__ pair_a, uint32_t* __restrict__ pair_b,
                                                          unsigned long long capacity) {
   grid_dependency_wait();
@@ -127,6 +153,13 @@ __global__ void __launch_bounds__(256) emit_pairs_kernel(const uint32_t* __restr
     unsigned long long out = offsets[i];
     uint32_t p = rank_le(bs, a_end[i]);            // = first: every b below it starts at or before a.end
     while (left && p) {
+      if ((p & 31u) == 0) {                        // at a run boundary: may the run(s) just below be skipped?
+        if ((p & 1023u) == 0) {
+          if ((p & 32767u) == 0 && max3[(p >> kSkip3) - 1u] < s) { p -= 32768u; continue; }
+          if (max2[(p >> kSkip2) - 1u] < s) { p -= 1024u; continue; }
+        }
+        if (max1[(p >> kSkip1) - 1u] < s) { p -= 32u; continue; }
+      }
       --p;
       if (end_by_start[p] >= s) {                  // ... and this one also ends at or after a.start: <a, b> is in I(A, B)
         if (out < capacity) { pair_a[out] = (uint32_t)i; pair_b[out] = idx_by_start[p]; }

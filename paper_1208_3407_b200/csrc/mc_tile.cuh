@@ -76,7 +76,9 @@ constexpr uint32_t kFlagBinTooBig = 1u, kFlagCrossFull = 4u;
 
 // Bulk asynchronous copy shared -> global (the TMA engine moves the bytes, no LDS / STG issued).
 // dst, src 16-byte aligned, bytes a multiple of 16.
-__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// (unqualified: orders this thread's earlier generic-proxy accesses to shared AND global memory before later
+// async-proxy ones -- the tile's slice of `pairs` is used as scratch through ordinary stores first)
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void bulk_store_smem_to_global(void* gdst, const void* ssrc, uint32_t bytes) {
   const uint32_t s = (uint32_t)__cvta_generic_to_shared(ssrc);
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes) : "memory");
@@ -212,7 +214,8 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kerne
         }
       }
     }
-    fence_proxy_async_smem();   // this thread's staged pairs are about to be read by the bulk-copy engine
+    fence_proxy_async_all();    // this thread's staged pairs are about to be read, and its scratch stores to the tile's
+                                // slice of `pairs` overwritten, by the bulk-copy engine
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < kPer / 4; ++j) reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + j] = make_uint4(0, 0, 0, 0);
@@ -459,6 +462,7 @@ __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_
     if (np + n_in + 4u > (uint32_t)C::kCap) {                              // block-uniform (4: room for the sentinels)
       if (tid == 0) atomicOr(a.flag, kFlagBinTooBig);
       d = d_next;
+      __syncthreads();       // every thread has read s_next before thread 0 takes the next ticket at the loop top
       continue;
     }
     // where each tile's segment of this bin sits in the tile (lo) and goes in the bin's buffers (pos)

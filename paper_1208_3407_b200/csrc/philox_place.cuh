@@ -139,12 +139,13 @@ __device__ __forceinline__ ChromView stage_chrom_table(const ChromTable& t, uint
 }
 
 // Four consecutive intervals i0..i0+3 (i0 % 4 == 0) of round `round`: two Philox calls.
-// Interval i uses counter (i >> 1, round, tag, 0) and output words 2h, 2h+1 with h = i & 1.
+// Interval i uses counter (i >> 1, round, tag, stream) and output words 2h, 2h+1 with h = i & 1;
+// stream = 0 for a single Monte Carlo job, the pair id inside the many-pair screen (R11, R24).
 __device__ __forceinline__ void place4(uint32_t i0, uint32_t round, uint32_t tag, const PhiloxKeys& key,
                                        const uint32_t d[4], const ChromView& off, const ChromTable& t,
-                                       uint32_t start[4]) {
-  const uint4 r0 = philox4x32_10(i0 >> 1, round, tag, 0u, key);
-  const uint4 r1 = philox4x32_10((i0 >> 1) + 1u, round, tag, 0u, key);
+                                       uint32_t start[4], uint32_t stream = 0u) {
+  const uint4 r0 = philox4x32_10(i0 >> 1, round, tag, stream, key);
+  const uint4 r1 = philox4x32_10((i0 >> 1) + 1u, round, tag, stream, key);
   start[0] = place_start(r0.x, r0.y, d[0], off, t);
   start[1] = place_start(r0.z, r0.w, d[1], off, t);
   start[2] = place_start(r1.x, r1.y, d[2], off, t);

@@ -105,6 +105,9 @@ def test_host_side_argument_checks_return_before_cuda():
     assert mc(None, 1, 0, 0, 1) == 1
     assert mc(off.ctypes.data, 0, 0, 0, 1) == 3                                            # n_chrom == 0
     assert mc(off.ctypes.data, 1, 0, 2**32 - 1, 2) == 2                                    # round overflow
+    # independently sorted B has lost the pairing of starts and ends, so its lengths cannot be kept
+    assert L.bits_mc_rounds(fake, fake, 1, fake, fake, 1, off.ctypes.data, 1, bits.PERMUTE_B, 1, 0, 1, bits.B_SORTED,
+                            ws, 1 << 40, fake, fake, None) == 6
     bad1 = np.array([1, 100], dtype=np.uint32)
     bad2 = np.array([0, 100, 100], dtype=np.uint32)
     assert mc(bad1.ctypes.data, 1, 0, 0, 1) == 3
@@ -137,3 +140,56 @@ def test_new_entry_points_reject_bad_arguments_on_the_host():
     assert L.bits_workspace_sorted_offset(bits.FN_COUNT, 10, 1000, 0, 0, 1, C.addressof(off)) == 0 and off.value > 0
     assert L.bits_workspace_sorted_offset(bits.FN_SORT, 10, 1000, 0, 0, 0, C.addressof(off)) == 6
     assert L.bits_workspace_sorted_offset(bits.FN_COUNT, 10, 1000, 0, 0, 2, C.addressof(off)) == 6
+
+
+def test_options_are_thread_local():
+    """bits_set_option state belongs to the calling host thread (bits.h, "Threads")."""
+    import threading
+    L = bits.lib()
+    assert L.bits_set_option(b"grid_mult", 3) == 0
+    seen = {}
+    def other():
+        seen["rc"] = L.bits_set_option(b"grid_mult", 99)          # out of range: this thread's value stays at its default
+        seen["bad"] = L.bits_set_option(b"no_such_knob", 1)
+    t = threading.Thread(target=other); t.start(); t.join()
+    assert seen == {"rc": 6, "bad": 6}
+    assert L.bits_set_option(b"grid_mult", 8) == 0
+    assert L.bits_set_option(b"mc_shift_bias", 9) == 6 and L.bits_set_option(b"mc_shift_bias", 0) == 0
+
+
+def test_screen_rejects_bad_arguments_on_the_host():
+    """bits_screen / bits_screen_workspace_bytes / bits_screen_enrichment: argument errors before any CUDA call."""
+    L = bits.lib()
+    one = (C.c_uint32 * 4)(1, 2, 3, 4)
+    p = C.addressof(one)
+    off = np.array([0, 100], dtype=np.uint32)
+    good = np.array([0, 2, 4], dtype=np.uint64)
+    wsb = lambda t, k: L.bits_screen_workspace_bytes(t.ctypes.data if t is not None else None, k, 1)
+    assert wsb(good, 2) > 0 and wsb(good, 2) % 256 == 0
+    assert wsb(None, 2) == 0 and wsb(good, 0) == 0 and wsb(good[:2], 65536) == 0
+    assert wsb(np.array([1, 2, 4], dtype=np.uint64), 2) == 0                      # [0] != 0
+    assert wsb(np.array([0, 3, 2], dtype=np.uint64), 2) == 0                      # decreasing
+    assert wsb(np.array([0, 2, 2**32], dtype=np.uint64), 2) == 0                  # too many intervals
+    assert wsb(np.array([0, 0, 0], dtype=np.uint64), 2) > 0                       # empty tracks are legal
+    big = wsb(np.array([0, 100_000, 200_000, 300_000], dtype=np.uint64), 3)
+    assert big > 3 * 100_000 * 4 * 2
+    scr = lambda t, k, o, nch, rb, nr, fl, obs, rc: L.bits_screen(p, p, t.ctypes.data if t is not None else None, k,
+                                                                  o.ctypes.data if o is not None else None, nch, 1, rb, nr, fl,
+                                                                  0, 0, obs, rc, None)
+    assert scr(None, 2, off, 1, 0, 1, 0, p, p) == 1
+    assert scr(good, 0, off, 1, 0, 1, 0, p, p) == 2
+    assert scr(good, 2, off, 1, 0, 1, 1, p, p) == 6                               # BITS_B_SORTED means nothing here
+    assert scr(good, 2, off, 1, 0, 1, 0, None, p) == 1
+    assert scr(good, 2, off, 1, 0, 1, 0, p, None) == 1
+    assert scr(good, 2, off, 1, 2**32 - 1, 2, 0, p, p) == 2
+    assert scr(good, 2, None, 1, 0, 1, 0, p, p) == 1
+    assert scr(good, 2, off, 0, 0, 1, 0, p, p) == 3
+    assert scr(good, 2, off, 1, 0, 1, 0, p, p) == 5                               # no workspace
+    # enrichment of every pair on the host
+    obs = np.array([8, 0, 5], dtype=np.uint64)
+    rc = np.array([[2, 2, 4], [0, 0, 0], [0, 0, 1]], dtype=np.uint64)
+    out = np.zeros(3)
+    assert L.bits_screen_enrichment(obs.ctypes.data, rc.ctypes.data, 3, 3, out.ctypes.data) == 0
+    assert out[0] == 2.0 and math.isnan(out[1]) and out[2] == math.inf
+    assert L.bits_screen_enrichment(None, rc.ctypes.data, 3, 3, out.ctypes.data) == 1
+    assert np.array_equal(bits.screen_enrichment(obs, rc), out, equal_nan=True)

@@ -395,3 +395,82 @@ def test_enrichment_score_closed_cases():
     rng = np.random.default_rng(1)
     x = rng.integers(1, 10**9, 1001)
     assert oracle.enrichment(12345, x) == math.log2(12345 / float(np.median(x)))
+
+
+# ------------------------------------------------------------------------------------- screen
+def test_place_round_stream_is_the_fourth_counter_word(curand_philox):
+    # counter = (i >> 1, round, tag, stream): rebuilt from cuRAND's routine + big ints, as for stream 0 above
+    rng = np.random.default_rng(40)
+    spans = rng.integers(0, 50_000, 23).astype(np.uint32)
+    seed, rnd, tag, stream = 0xCAFE_F00D_0BAD_BEEF, 9, 0, 25_280
+    s, e = oracle.place_round(spans, GEN, seed, rnd, tag, stream)
+    for i in range(spans.size):
+        o = curand_philox([i >> 1, rnd, tag, stream], [seed & 0xFFFFFFFF, seed >> 32])
+        h = i & 1
+        want = py_place(int(o[2 * h]) | (int(o[2 * h + 1]) << 32), int(spans[i]), GEN)
+        assert int(s[i]) == want and int(e[i]) == want + int(spans[i])
+    s0, _ = oracle.place_round(spans, GEN, seed, rnd, tag)
+    assert np.array_equal(s0, oracle.place_round(spans, GEN, seed, rnd, tag, 0)[0]) and (s0 != s).mean() > 0.9
+
+
+def test_screen_brute_forced():
+    """oracle.screen on K = 3 small tracks: every observed count and every round count by
+    O(N*M) brute force on placements rebuilt with the pair's own stream id i*K + j; the score from numpy's median."""
+    rng = np.random.default_rng(41)
+    off = np.array([0, 30_000, 50_000, 90_000], dtype=np.uint32)
+    tracks = []
+    for n, max_len in ((120, 900), (200, 300), (75, 2500)):
+        c = rng.integers(0, 3, n)
+        ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        st = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        tracks.append((st.astype(np.uint32), (st + ln - 1).astype(np.uint32)))
+    K, R, r0, seed = 3, 7, 100, 12
+    obs, rc, enr = oracle.screen(tracks, off, seed, r0, R)
+    for i in range(K):
+        for j in range(K):
+            assert int(obs[i, j]) == int(brute_counts(*tracks[i], *tracks[j]).sum())
+            spans = tracks[i][1] - tracks[i][0]
+            for k in range(R):
+                s, e = oracle.place_round(spans, off, seed, r0 + k, 0, i * K + j)
+                assert int(rc[i, j, k]) == int(brute_counts(s, e, *tracks[j]).sum())
+            med = float(np.median(rc[i, j].astype(np.float64)))
+            want = np.log2(float(obs[i, j]) / med) if med > 0 else (np.inf if obs[i, j] else np.nan)
+            assert enr[i, j] == want or (np.isnan(enr[i, j]) and np.isnan(want))
+    # pair (0, 0) draws from stream 0: the plain Monte Carlo job on (T_0, T_0)
+    _, plain = oracle.mc_rounds(*tracks[0], *tracks[0], off, 0, seed, r0, R)
+    assert np.array_equal(rc[0, 0], plain)
+    # the other pairs have their own null: track 0's draws differ between partners
+    assert not np.array_equal(oracle.place_round(tracks[0][1] - tracks[0][0], off, seed, r0, 0, 1)[0],
+                              oracle.place_round(tracks[0][1] - tracks[0][0], off, seed, r0, 0, 2)[0])
+
+
+# ------------------------------------------------------------------------------------- golden round counts
+def _golden():
+    import importlib.util
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "make_golden.py")
+    spec = importlib.util.spec_from_file_location("make_golden", path)
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod
+
+
+@pytest.mark.parametrize("config,slices", [(3, ((0, 40), (3333, 25), (9983, 17))), (5, ((0, 1), (437, 1), (999, 1)))])
+def test_golden_round_counts_are_the_oracles(config, slices):
+    """tests/golden/cfg{3,5}_seed1_rounds.txt (written by tests/golden/make_golden.py from the oracle over disjoint
+    round slices): the inputs are the ones workloads.make_config builds today (checksums), a few slices re-derived
+    here from the oracle -- at other slice boundaries than the file was written with -- give the same counts, and
+    the stored p-values follow from the stored integers."""
+    g = _golden()
+    header, counts = g.load(config)
+    w = W.make_config(config)
+    assert header["checksums"] == w.checksums() and header["chrom_offsets_checksum"] == W.array_checksum(w.chrom_offsets)
+    assert header["n_rounds"] == w.n_rounds == counts.size and header["which"] == w.which and header["mc_seed"] == w.mc_seed
+    for r0, n in slices:
+        obs, rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, w.which, w.mc_seed, r0, n)
+        assert obs == header["observed"]
+        assert np.array_equal(rc, counts[r0:r0 + n])
+    assert header["p_enrich"] == oracle.pvalue(header["observed"], counts, 0)
+    assert header["p_deplete"] == oracle.pvalue(header["observed"], counts, 1)
+    ge = int((counts >= header["observed"]).sum())
+    assert header["p_enrich"] == (ge + 1) / (counts.size + 1)

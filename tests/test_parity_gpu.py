@@ -481,6 +481,72 @@ def _mc_b_case(a_s, a_e, b_s, b_e, off, seed, r0, n, expect_fused=None):
     assert np.array_equal(host_u64(rc), o_rc)
 
 
+def _golden(config):
+    import importlib.util
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "make_golden.py")
+    spec = importlib.util.spec_from_file_location("make_golden", path)
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod.load(config)
+
+
+@pytest.mark.parametrize("config,split", [(3, 3333), (5, 437)])
+def test_mc_full_length_golden(config, split):
+    """EVERY per-round count of the full-size Monte Carlo configs (10,000 rounds of config 3, 1,000 rounds of
+    config 5, in the launch configuration bench.py times) against the oracle's golden counts
+    (tests/golden/cfg{3,5}_seed1_rounds.txt, written by tests/golden/make_golden.py from the oracle alone), the
+    p-values derived from them, and the same rounds by two calls split at an odd round_begin."""
+    header, golden = _golden(config)
+    w = W.make_config(config)
+    assert header["checksums"] == w.checksums()
+    R = w.n_rounds
+    obs, rc = run_mc(w, w.which, w.mc_seed, 0, R)
+    assert obs == header["observed"]
+    bad = np.nonzero(rc != golden)[0]
+    assert bad.size == 0, f"{bad.size} rounds differ, first {bad[:5]}"
+    assert bits.pvalue(obs, rc, 0) == header["p_enrich"] and bits.pvalue(obs, rc, 1) == header["p_deplete"]
+    _, lo = run_mc(w, w.which, w.mc_seed, 0, split)
+    _, hi = run_mc(w, w.which, w.mc_seed, split, R - split)
+    assert np.array_equal(np.concatenate([lo, hi]), golden)
+    if config == 5:                                  # and through the host-buffer entry point bench.py's e2e leg times
+        r = bits.mc_rounds_host(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, w.which, w.mc_seed, 900, 100)
+        assert r.observed == header["observed"] and np.array_equal(r.round_counts, golden[900:])
+
+
+def test_mc_permute_b_bins_overflow_on_the_device():
+    """Bins wider than the host's margin allows (mc_shift_bias): about half of the bins of every round hold more
+    than kCap keys, so bin_sort_search_kernel takes its overflow branch on the device, raises the round's flag and
+    moves on to its next ticket; the flagged rounds are redone by the general path.  The kernel must terminate
+    cleanly and every count must be the oracle's."""
+    off = W.genome_offsets(W.GENOME24_LENGTHS)
+    G = int(off[-1])
+    n_b = int(4090 * G / 2**21)                      # ~4,090 keys per 2^21-wide bin: the host picks shift 21; bias + 1 -> ~8,180
+    rng = np.random.default_rng(77)
+    def draw(n, max_len):
+        c = rng.integers(0, 24, n)
+        ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        s = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        return s.astype(np.uint32), (s + ln - 1).astype(np.uint32)
+    b_s, b_e = draw(n_b, 500)
+    a_s, a_e = draw(100_000, 2000)
+    bits.set_option("mc_shift_bias", 1)
+    try:
+        # (programmatic dependent launch is on here; the event timers of _mc_b_case switch it off)
+        obs, rc = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, 1, 21, 5, 3)
+        sync()
+        o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, 1, 21, 5, 3)
+        assert int(host_u64(obs)[0]) == o_obs and np.array_equal(host_u64(rc), o_rc)
+        for _ in range(2):                           # twice: tickets, flags and hand-over counters restart correctly
+            _mc_b_case(a_s, a_e, b_s, b_e, off, 21, 5, 3, expect_fused=True)
+            assert bits.profile_read()["sorted_query"][1] == 3          # every round was flagged and redone
+    finally:
+        bits.set_option("mc_shift_bias", 0)
+    _mc_b_case(a_s, a_e, b_s, b_e, off, 21, 5, 3, expect_fused=True)
+    assert bits.profile_read()["sorted_query"][1] == 0                  # without the bias nothing overflows
+
+
 @pytest.mark.parametrize("tile_variant", [0, 1, 2])
 @pytest.mark.parametrize("bin_variant", [0, 1, 2, 3])
 def test_mc_permute_b_kernel_shapes(tile_variant, bin_variant):
@@ -621,26 +687,67 @@ def test_mc_permute_b_leaves_sorted_arrays_of_last_round(k, scale, rounds):
     assert np.array_equal(host_u32(b_e), oracle.sort_u32(o_e))
 
 
-def test_screen_of_tracks_matches_oracle():
-    """The co-localisation screen: K x K observed counts, round counts and log2(observed / median)."""
-    rng = np.random.default_rng(31)
-    off = W.genome_offsets([3_000_000, 2_000_000, 1_200_000])
-    G = int(off[-1])
+def _screen_tracks(rng, off, shapes):
+    n_chrom = off.size - 1
     tracks = []
-    for n, max_len in ((4000, 400), (2500, 2000), (6000, 120)):
-        c = rng.integers(0, 3, n)
+    for n, max_len in shapes:
+        c = rng.integers(0, n_chrom, n)
         ln = rng.integers(1, max_len, n)
         lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
         s = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
         tracks.append((s.astype(np.uint32), (s + ln - 1).astype(np.uint32)))
-    R = 21
-    obs, enr, rc = bits.screen([(dev(s), dev(e)) for s, e in tracks], off, 4, R)
-    for i in range(3):
-        for j in range(3):
-            o_obs, o_rc = oracle.mc_rounds(tracks[i][0], tracks[i][1], tracks[j][0], tracks[j][1], off, 0, 4, 0, R)
-            assert int(obs[i, j]) == o_obs and np.array_equal(rc[i, j], o_rc)
-            want = oracle.enrichment(o_obs, o_rc)
-            assert enr[i, j] == want or (np.isnan(enr[i, j]) and np.isnan(want))
+    return tracks
+
+
+def test_screen_of_tracks_matches_oracle():
+    """bits_screen: K x K observed counts, every round count (pair id in the Philox counter) and
+    log2(observed / median), against oracle.screen; tracks of very different sizes, one of them empty; round slicing."""
+    rng = np.random.default_rng(31)
+    off = W.genome_offsets([3_000_000, 2_000_000, 1_200_000])
+    tracks = _screen_tracks(rng, off, ((4000, 400), (2500, 2000), (0, 10), (6000, 120), (1, 50), (1025, 300)))
+    K, R, seed = len(tracks), 21, 4
+    dtracks = [(dev(s), dev(e)) for s, e in tracks]
+    before = bits.launch_count()
+    obs, enr, rc = bits.screen(dtracks, off, seed, R)
+    n_launches = bits.launch_count() - before
+    o_obs, o_rc, o_enr = oracle.screen(tracks, off, seed, 0, R)
+    assert np.array_equal(obs, o_obs) and np.array_equal(rc, o_rc)
+    assert np.array_equal(enr, o_enr, equal_nan=True)
+    assert n_launches < 40 * K                                # setup per track + two gridded launches, not per pair
+    # pair (0, 0) is the plain Monte Carlo job (stream 0); other pairs draw from their own stream
+    _, plain = run_mc(W.Workload("t", *tracks[0], *tracks[0], off), 0, seed, 0, R)
+    assert np.array_equal(rc[0, 0], plain)
+    _, plain01 = run_mc(W.Workload("t", *tracks[0], *tracks[1], off), 0, seed, 0, R)
+    assert not np.array_equal(rc[0, 1], plain01)
+    # rounds are addressed by (seed, round, pair): slices of the round range are bit-identical
+    _, _, hi = bits.screen(dtracks, off, seed, R - 8, round_begin=8)
+    assert np.array_equal(hi, o_rc[:, :, 8:])
+    # a single track, and no rounds
+    obs1, _, rc1 = bits.screen(dtracks[:1], off, seed, 0)
+    assert obs1.shape == (1, 1) and int(obs1[0, 0]) == int(o_obs[0, 0]) and rc1.shape == (1, 1, 0)
+
+
+def test_screen_genome_scale_tracks():
+    """A screen on the 24-chromosome genome with tracks large enough for several query tiles and the MSD sort."""
+    rng = np.random.default_rng(32)
+    off = W.genome_offsets(W.GENOME24_LENGTHS)
+    tracks = _screen_tracks(rng, off, ((30_000, 3000), (70_001, 800), (12_345, 20_000)))
+    obs, enr, rc = bits.screen([(dev(s), dev(e)) for s, e in tracks], off, 9, 5, round_begin=4_000_000_000)
+    o_obs, o_rc, o_enr = oracle.screen(tracks, off, 9, 4_000_000_000, 5)
+    assert np.array_equal(obs, o_obs) and np.array_equal(rc, o_rc) and np.array_equal(enr, o_enr, equal_nan=True)
+
+
+def test_screen_errors():
+    off = np.array([0, 1000, 3000], dtype=np.uint32)
+    s, e = dev([1, 5, 0]), dev([3, 9, 2000])                  # the third interval is as long as the longest chromosome
+    with pytest.raises(bits.BitsError) as ei:
+        bits.screen_concat(s, e, [0, 2, 3], off, 1, 4)
+    assert ei.value.status == 4
+    obs, rc = bits.screen_concat(s, e, [0, 2, 3], off, 1, 0)  # no rounds: nothing is placed, the observed counts are fine
+    sync()
+    assert host_u64(obs).reshape(2, 2)[0, 1] == 2
+    with pytest.raises(bits.BitsError):
+        bits.screen_concat(s, e, [0, 3, 2], off, 1, 4)        # offsets must not decrease
 
 
 def test_cli_on_bed_files(tmp_path, capsys):
