@@ -69,6 +69,11 @@ def parse_args():
     p.add_argument("--rounds", type=int, default=0, help="rounds per step (0 = the configuration's own count)")
     p.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                    help="bits_set_option knob for design studies (DESIGN.md section 10); results never change")
+    p.add_argument("--study", default=None, choices=["search", "count"],
+                   help="design studies instead of the bench line: 'search' = config 4 with every search design of the count "
+                        "path + 100 rounds of config 3; 'count' = config 4's bits_count_per_interval only (the command the "
+                        "ncu captures under profiles/ run); with --once every call runs once, without warm-up")
+    p.add_argument("--once", action="store_true", help="--study: one call per design, no warm-up (for captures under ncu)")
     p.add_argument("--no-extras", action="store_true", help="skip the secondary workloads, e2e and cpu_baseline legs")
     p.add_argument("--no-profile-events", action="store_true", help="do not bracket kernels with events in the timed region")
     return p.parse_args()
@@ -623,8 +628,71 @@ def run_b200(args):
     return 0
 
 
+def run_study(args):
+    """Design studies of the count path (north_star subsystem 3: try several search designs and keep what ncu
+    supports).  Prints one JSON line; per-kernel device times come from the library's event timers."""
+    import torch
+    from paper_1208_3407_b200 import bits
+    from paper_1208_3407_b200 import workloads as W
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    for kv in args.opt:
+        name, _, val = kv.partition("=")
+        bits.set_option(name, int(val))
+    reps = 1 if args.once else 8
+    w = W.make_config(4, scale=args.scale)
+    d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    ws = torch.empty(bits.workspace_bytes(bits.FN_COUNT_PER_INTERVAL, w.n_a, w.n_b), dtype=torch.uint8, device=device)
+    counts = torch.empty(w.n_a, dtype=torch.int32, device=device)
+    total = torch.empty(1, dtype=torch.int64, device=device)
+    out = {"study": args.study, "workload": w.name, "n_a": w.n_a, "n_b": w.n_b, "calls_per_design": reps, "designs": {}}
+
+    def one_design(label):
+        if not args.once:
+            for _ in range(2):
+                bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total)
+            med, mn = time_device(lambda: bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total), reps, warmup=0)
+        bits.set_option("profile", 2); bits.set_option("profile", 1)
+        for _ in range(reps):
+            bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total)
+        torch.cuda.synchronize()
+        prof = bits.profile_read(); bits.set_option("profile", 0)
+        r = {"kernel_us": {k: 1e3 * v[0] / reps for k, v in prof.items() if v[1]},
+             "total": int(total.cpu().numpy().view(np.uint64)[0])}
+        if not args.once:
+            r["call_ms_median"], r["call_ms_min"] = med, mn
+            r["intervals_searched_per_s"] = w.n_a / (med * 1e-3)
+        out["designs"][label] = r
+
+    if args.study == "count":
+        one_design("default")
+    else:
+        for v, name in SEARCH_DESIGNS:
+            bits.set_option("search_variant", v)
+            one_design(f"{v}: {name}")
+        bits.set_option("search_variant", 0)
+        w3 = W.make_config(3, scale=args.scale)
+        d3 = [to_dev(x, device) for x in (w3.a_start, w3.a_end, w3.b_start, w3.b_end)]
+        R = 100
+        bits.set_option("profile", 2); bits.set_option("profile", 1)
+        for _ in range(reps):
+            bits.mc_rounds(*d3, w3.chrom_offsets, 0, 1, 0, R)
+        torch.cuda.synchronize()
+        prof = bits.profile_read(); bits.set_option("profile", 0)
+        us = 1e3 * prof["mc_permute_a"][0] / prof["mc_permute_a"][1]
+        out["cfg3_mc_permute_a_100_rounds_per_launch"] = {"kernel_us": us, "intervals_searched_per_s": R * w3.n_a / (us * 1e-6)}
+    print(json.dumps(out))
+    return 0
+
+
+# search designs of the count path (bits_set_option "search_variant"; DESIGN.md section 5)
+SEARCH_DESIGNS = ((0, "bucket index"), (1, "plain binary search (the paper's design)"), (2, "top 11 levels in shared memory"))
+
+
 def main():
     args = parse_args()
+    if args.study:
+        return run_study(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_b200(args)

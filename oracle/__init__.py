@@ -14,7 +14,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "bits_oracle.cpp")
-_LIB = os.path.join(_HERE, "libbits_oracle.so")
+# BITS_ORACLE_SANITIZE=1: the same source under AddressSanitizer + UndefinedBehaviorSanitizer (run the pins with
+# LD_PRELOAD="$(gcc -print-file-name=libasan.so) $(gcc -print-file-name=libubsan.so)")
+_SANITIZE = bool(os.environ.get("BITS_ORACLE_SANITIZE"))
+_LIB = os.path.join(_HERE, "libbits_oracle_san.so" if _SANITIZE else "libbits_oracle.so")
 _lib = None
 
 
@@ -22,8 +25,9 @@ def build(force: bool = False) -> str:
     """Compile the oracle with g++ -O3 -march=native (single-threaded C++17)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["g++", "-std=c++17", "-O3", "-march=native", "-fPIC", "-shared",
-                               "-o", tmp, _SRC])
+        opt = (["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+               if _SANITIZE else ["-O3", "-march=native"])
+        subprocess.check_call(["g++", "-std=c++17", *opt, "-fPIC", "-shared", "-o", tmp, _SRC])
         os.replace(tmp, _LIB)
     return _LIB
 

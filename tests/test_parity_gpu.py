@@ -299,6 +299,45 @@ def test_enumerate_config2_is_valid_and_complete():
     assert np.unique(pa * (1 << 32) + pb).size == n
 
 
+def test_enumerate_walk_is_bounded_when_one_interval_spans_everything():
+    """a scan back from the binary-search position is what BITS replaces.  With one genome-wide
+    interval in B (a tiny start, the largest end) every query must reach position 0 of the start order; the
+    walk steps over runs of 32 / 1,024 / 32,768 positions whose largest end lies before a.start, so that case
+    costs about what the uniform one does instead of O(|B|) per query.  Set equality on a sample + validity and
+    completeness on the whole + a timing bound against the same sets without the long interval."""
+    w = W.make_config(2, scale=0.4)
+    G = int(w.chrom_offsets[-1])
+    b_s = np.concatenate([w.b_start, [0, 5]]).astype(np.uint32)
+    b_e = np.concatenate([w.b_end, [G - 1, 4_000_000]]).astype(np.uint32)     # one genome-wide, one long interval
+    d_long = [dev(x) for x in (w.a_start, w.a_end, b_s, b_e)]
+    d_base = [dev(x) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    pa, pb, n = bits.enumerate_pairs(*d_long)
+    sync()
+    pa, pb = host_u32(pa).astype(np.int64), host_u32(pb).astype(np.int64)
+    o_total, o_counts = oracle.count_per_interval(w.a_start, w.a_end, b_s, b_e)
+    assert n == o_total and o_counts.min() >= 1
+    assert np.all((w.a_start.astype(np.int64)[pa] <= b_e.astype(np.int64)[pb]) & (w.a_end.astype(np.int64)[pa] >= b_s.astype(np.int64)[pb]))
+    assert np.array_equal(np.bincount(pa, minlength=w.n_a), o_counts)
+    assert np.unique(pa * (1 << 32) + pb).size == n
+    assert int(np.bincount(pb, minlength=b_s.size)[-2]) == w.n_a                 # the genome-wide interval meets every query
+    sample = np.arange(0, w.n_a, 997)[:300]                                   # set equality with the definition on a sample of A
+    want = oracle.enumerate_pairs(w.a_start[sample], w.a_end[sample], b_s, b_e)
+    sel = np.isin(pa, sample)
+    got = np.stack([np.searchsorted(sample, pa[sel]), pb[sel]], 1)
+    assert np.array_equal(got[np.lexsort((got[:, 1], got[:, 0]))], want)
+    def timed(d):
+        ws = torch.empty(bits.workspace_bytes(bits.FN_ENUMERATE, d[0].numel(), d[2].numel()), dtype=torch.uint8, device=DEV)
+        bits.enumerate_pairs(*d, workspace=ws); sync()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(3):
+            bits.enumerate_pairs(*d, workspace=ws)
+        e1.record(); sync()
+        return e0.elapsed_time(e1) / 3
+    t_long, t_base = timed(d_long), timed(d_base)
+    assert t_long < 5.0 * t_base + 1.0, (t_long, t_base)      # (an unbounded walk takes seconds here: 4e5 queries x 4e5 steps)
+
+
 def test_enumerate_with_too_small_a_capacity_writes_a_prefix_only():
     """include/bits.h: pairs at positions >= capacity are not written, *total_out is the full count either way."""
     w = W.make_config(2, scale=0.05)
