@@ -246,7 +246,8 @@ uint64_t bits_launch_count(void);
  * bits_set_option("profile", 1) is on (2 resets the totals).  cls: 0 place, 1 histogram,
  * 2 LSD sort pass, 3 index build, 4 count (search + reduce), 5 sorted-query search + reduce,
  * 6 fused Monte Carlo kernel (place + search + reduce), 7 other, 8 MSD sort plan, 9 MSD sort
- * scatter, 10 MSD per-bucket sort, 11 fused place + scatter, 12 fused per-bucket sort + search + reduce.
+ * scatter, 10 MSD per-bucket sort, 11 fused place + scatter, 12 fused per-bucket sort + search + reduce,
+ * 13 scatter of the queries into bucket order, 14 per-bucket search + reduce out of shared memory.
  * Synchronises the recorded
  * events.  ms_out / launches_out: host pointers, may be NULL. */
 int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out);

@@ -109,7 +109,7 @@ def set_option(name: str, value: int) -> None:
 
 
 PROFILE_CLASSES = ("place", "histogram", "sort_pass", "index_build", "count", "sorted_query", "mc_permute_a", "other",
-                   "plan", "scatter", "bucket_sort", "place_scatter", "bucket_sort_search")
+                   "plan", "scatter", "bucket_sort", "place_scatter", "bucket_sort_search", "query_scatter", "bucket_search")
 
 
 def profile_read() -> dict:

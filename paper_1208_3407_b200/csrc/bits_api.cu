@@ -16,6 +16,7 @@
 #include "search.cuh"
 #include "enumerate.cuh"
 #include "screen.cuh"
+#include "binned_count.cuh"
 
 namespace bits {
 
@@ -33,6 +34,8 @@ struct Options {
   int64_t mc_tile_variant = 2;     // PERMUTE_B fused rounds: shape of place_tile_kernel (0: 2 x 512 threads, 1: 1 x 1024, 2: 1 x 1024 with longer tiles)
   int64_t mc_bin_variant = 0;      // PERMUTE_B fused rounds: shape of the per-bin sort (0 wide, 1 narrow, 2 small blocks)
   int64_t mc_gather_group = -1;    // PERMUTE_B fused rounds: log2 of the lanes per gathered segment (-1 = from the mean segment length)
+  int64_t msd_pack = 7168;         // MSD sort plan: 0 = buckets by the prefix / target rule, n = consecutive bins packed greedily up to n keys (measured on config 4: 0 -> 146 us, 8192 -> 134, 7168 -> 124 for the bucket sort)
+  int64_t count_binned = -1;       // count path: 1 = queries binned by B's buckets and searched out of shared memory (binned_count.cuh), 0 = bucket index + count_kernel, -1 = by size
   int64_t mc_shift_bias = 0;       // PERMUTE_B fused rounds: added to the bin width (log2) the host picked; > 0 overflows bins on purpose (tests)
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
 };
@@ -47,7 +50,7 @@ constexpr size_t kMaxSmemPerBlock = 232448 - 2048;   // 227 KB opt-in limit of s
 // Optional per-kernel-class timing with CUDA events on the launching stream (bits_set_option
 // "profile" = 1; read with bits_profile_read).  Used by bench.py for the roofline figures.
 enum { kClsPlace = 0, kClsHist, kClsSortPass, kClsIndex, kClsCount, kClsSortedQuery, kClsMcA, kClsOther,
-       kClsPlan, kClsScatter, kClsBucketSort, kClsPlaceScatter, kClsBucketSortSearch, kNumCls };
+       kClsPlan, kClsScatter, kClsBucketSort, kClsPlaceScatter, kClsBucketSortSearch, kClsQueryScatter, kClsBucketSearch, kNumCls };
 struct Profiler {
   bool on = false;
   std::vector<cudaEvent_t> ev;     // pairs: 2k = start, 2k+1 = stop
@@ -135,6 +138,8 @@ struct SortCtx {
   uint32_t* bucket_start[2] = {nullptr, nullptr};   // uint32[kBins + 1]
   uint32_t* n_buckets = nullptr;                    // uint32[2]
   uint32_t* msd_flag = nullptr;                     // uint32[2]
+  uint16_t* bucket_of_bin = nullptr;                // uint16[kBins] bucket of array 0 that holds each bin (binned_count.cuh)
+  uint32_t* bucket_lo = nullptr;                    // uint32[kBins + 1] first bin of each bucket of array 0
   size_t zero_bytes = 0;                            // from hist[0][0]: digit histograms, tickets, bin histograms, bucket counts, flags, status words
   void carve(Carver& c, uint64_t n_keys, bool with_index) {
     n = (uint32_t)n_keys;
@@ -156,6 +161,8 @@ struct SortCtx {
       bin_cursor[a] = c.take<uint32_t>(msd::kBins);
       bucket_start[a] = c.take<uint32_t>(msd::kBins + 4);
     }
+    bucket_of_bin = c.take<uint16_t>(msd::kBins);
+    bucket_lo = c.take<uint32_t>(msd::kBins + 4);
     shift = index_shift_for(n_keys);
     if (with_index)
       for (int a = 0; a < 2; ++a) idx[a] = c.take<uint32_t>(index_entries(shift));
@@ -190,6 +197,8 @@ struct Layout {
   uint32_t* cross_keys = nullptr;        // [kMaxBins * kCrossCap]
   uint32_t* qb[2] = {nullptr, nullptr};
   uint32_t* round_flags = nullptr;       // uint32[kFlagChunk]
+  // count path with binned queries (binned_count.cuh)
+  qb::Lists ql = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // (eight pointers)
   // enumeration (enumerate.cuh)
   uint32_t* e_counts = nullptr;                  // [n_a]
   unsigned long long* e_offsets = nullptr;       // [n_a]
@@ -223,6 +232,14 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
     case BITS_FN_COUNT:
     case BITS_FN_COUNT_PER_INTERVAL:
       L.b.carve(c, n_b, true);
+      L.ql.q_end = c.take<uint32_t>(n_a + 4);
+      L.ql.q_start = c.take<uint32_t>(n_a + 4);
+      L.ql.q_idx = c.take<uint32_t>(fn == BITS_FN_COUNT_PER_INTERVAL ? n_a + 4 : 4);
+      L.ql.hist = c.take<uint32_t>(msd::kBins + 64);
+      L.ql.item_bucket = c.take<uint16_t>(ceil_div(n_a, (uint64_t)qb::kChunk) + msd::kBins + 8);
+      L.ql.off = c.take<uint32_t>(msd::kBins + 4);
+      L.ql.cursor = c.take<uint32_t>(msd::kBins + 4);
+      L.ql.item_off = c.take<uint32_t>(msd::kBins + 4);
       break;
     case BITS_FN_MC_ROUNDS:
       L.b.carve(c, n_b, true);
@@ -412,7 +429,9 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     for (int a = 0; a < 2; ++a) {
       pa.p[a].hist = c.bin_hist[a]; pa.p[a].bin_cursor = c.bin_cursor[a]; pa.p[a].bucket_start = c.bucket_start[a];
       pa.p[a].n_buckets = c.n_buckets + a; pa.p[a].flag = c.msd_flag + a; pa.p[a].lsd_hist = c.hist[0][a]; pa.p[a].lsd_ticket = c.ticket + 4 * a;
+      pa.p[a].bucket_of_bin = a == 0 ? c.bucket_of_bin : nullptr; pa.p[a].bucket_lo = a == 0 ? c.bucket_lo : nullptr;
     }
+    pa.pack_cap = (uint32_t)g_opt.msd_pack;
     ProfScope prof(kClsPlan, st);
     launch_pdl(msd::plan_kernel, n_arrays, 1024, 0, st, pa);
     BITS_LAUNCH_CHECK();
@@ -450,15 +469,19 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
   return launch_sort_passes(p, epoch, st);
 }
 
-static int launch_build_index(const SortCtx& c, cudaStream_t st) {
+static int launch_build_index(const SortCtx& c, cudaStream_t st, const uint32_t* run_if = nullptr) {
   IndexArgs ia;
+  ia.run_if = run_if;
   ia.keys[0] = c.buf[0][0]; ia.keys[1] = c.buf[1][0];
   ia.idx[0] = c.idx[0]; ia.idx[1] = c.idx[1];
   ia.n = c.n; ia.shift = c.shift;
   const uint64_t need = ceil_div((uint64_t)c.n, 4) + 1;   // four positions per thread
   const uint64_t threads = need > (uint64_t)kPad ? need : (uint64_t)kPad;
+  const uint64_t blocks = ceil_div(threads, 256);
+  ia.total = blocks * 256;
   ProfScope prof(kClsIndex, st);
-  launch_pdl(build_index_kernel, dim3((unsigned)ceil_div(threads, 256), 2), 256, 0, st, ia);
+  // (a gated launch is almost always skipped: fewer blocks to start and retire)
+  launch_pdl(build_index_kernel, dim3((unsigned)(run_if && blocks > 2u * kSMs ? 2u * kSMs : blocks), 2), 256, 0, st, ia);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -482,14 +505,14 @@ static inline SortedSet sorted_set(const SortCtx& c, int a) {
 }
 
 static int launch_count(const uint32_t* a_start, const uint32_t* a_end, uint32_t n_a, const SortCtx& b,
-                        uint32_t* counts, uint64_t* total, cudaStream_t st) {
+                        uint32_t* counts, uint64_t* total, cudaStream_t st, const uint32_t* run_if = nullptr) {
   const bool vec = (((uintptr_t)a_start | (uintptr_t)a_end | (uintptr_t)counts) & 15) == 0;
   const int grid = grid_for(ceil_div(n_a, 4), 256);
   ProfScope prof(kClsCount, st);
   const SortedSet s0 = sorted_set(b, 0), s1 = sorted_set(b, 1);
   unsigned long long* tot = reinterpret_cast<unsigned long long*>(total);
   const int sv = (int)g_opt.search_variant;
-#define BITS_COUNT_LAUNCH(V, S) launch_pdl(count_kernel<V, S>, grid, 256, 0, st, a_start, a_end, n_a, s0, s1, counts, tot)
+#define BITS_COUNT_LAUNCH(V, S) launch_pdl(count_kernel<V, S>, run_if && grid > 2 * kSMs ? 2 * kSMs : grid, 256, 0, st, a_start, a_end, n_a, s0, s1, counts, tot, run_if)
   if (vec) {
     if (sv == kSearchPlain) BITS_COUNT_LAUNCH(true, kSearchPlain);
     else if (sv == kSearchStaged) BITS_COUNT_LAUNCH(true, kSearchStaged);
@@ -524,6 +547,55 @@ static int check_common(const void* a_start, const void* a_end, uint64_t n_a, co
   return BITS_OK;
 }
 
+// Search + reduce with the queries binned by B's buckets (binned_count.cuh).  L.b has just been sorted by the MSD sort.
+static int launch_binned_count(const uint32_t* a_start, const uint32_t* a_end, uint32_t n_a, const Layout& L,
+                               uint32_t* counts, uint64_t* total, cudaStream_t st) {
+  static std::atomic<int> configured[64];
+  int device = 0;
+  BITS_CUDA_TRY(cudaGetDevice(&device));
+  if (device < 0 || device >= 64 || configured[device].load(std::memory_order_acquire) == 0) {
+    BITS_CUDA_TRY(cudaFuncSetAttribute(qb::query_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)qb::kScSmem));
+    BITS_CUDA_TRY(cudaFuncSetAttribute(qb::query_scatter_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)qb::kScSmem));
+    BITS_CUDA_TRY(cudaFuncSetAttribute(qb::bucket_search_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)qb::kSrSmem));
+    BITS_CUDA_TRY(cudaFuncSetAttribute(qb::bucket_search_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)qb::kSrSmem));
+    if (device >= 0 && device < 64) configured[device].store(1, std::memory_order_release);
+  }
+  qb::Plan p;
+  p.flag = L.b.msd_flag; p.bucket_of_bin = L.b.bucket_of_bin; p.bucket_lo = L.b.bucket_lo; p.bucket_start = L.b.bucket_start[0];
+  p.n_buckets = L.b.n_buckets; p.end_cursor = L.b.bin_cursor[1];
+  const uint32_t n_tiles = (uint32_t)ceil_div(n_a, (uint64_t)qb::kScTile);
+  {
+    ProfScope prof(kClsHist, st);
+    const uint32_t blocks = (uint32_t)ceil_div(ceil_div(n_a, 4), 1024 * 4);
+    launch_pdl(qb::query_hist_kernel, blocks < (uint32_t)kSMs ? (blocks ? blocks : 1u) : (uint32_t)kSMs, 1024, 0, st, a_end, n_a, p, L.ql);
+    BITS_LAUNCH_CHECK();
+  }
+  {
+    ProfScope prof(kClsPlan, st);
+    launch_pdl(qb::query_plan_kernel, 1, 1024, 0, st, p, L.ql);
+    BITS_LAUNCH_CHECK();
+  }
+  {
+    ProfScope prof(kClsQueryScatter, st);
+    const uint32_t blocks = n_tiles < (uint32_t)kSMs ? n_tiles : (uint32_t)kSMs;
+    if (counts) launch_pdl(qb::query_scatter_kernel<true>, blocks, qb::kScThreads, qb::kScSmem, st, a_start, a_end, n_a, p, L.ql);
+    else launch_pdl(qb::query_scatter_kernel<false>, blocks, qb::kScThreads, qb::kScSmem, st, a_start, a_end, n_a, p, L.ql);
+    BITS_LAUNCH_CHECK();
+  }
+  {
+    qb::SearchArgs sa;
+    sa.p = p; sa.l = L.ql; sa.b_s = L.b.buf[0][0]; sa.b_e = L.b.buf[1][0]; sa.n_b = L.b.n; sa.counts = counts;
+    sa.total = reinterpret_cast<unsigned long long*>(total);
+    ProfScope prof(kClsBucketSearch, st);
+    const uint32_t want = (uint32_t)ceil_div(n_a, (uint64_t)qb::kChunk) + 1u;
+    const uint32_t blocks = want < 2u * kSMs ? want : 2u * (uint32_t)kSMs;
+    if (counts) launch_pdl(qb::bucket_search_kernel<true>, blocks, qb::kSrThreads, qb::kSrSmem, st, sa);
+    else launch_pdl(qb::bucket_search_kernel<false>, blocks, qb::kSrThreads, qb::kSrSmem, st, sa);
+    BITS_LAUNCH_CHECK();
+  }
+  return BITS_OK;
+}
+
 static int count_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
                       const uint32_t* b_end, uint64_t n_b, uint32_t flags, void* ws, size_t ws_bytes, int fn,
                       uint32_t* counts_out, uint64_t* total_out, cudaStream_t st) {
@@ -542,8 +614,19 @@ static int count_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n
   }
   uint32_t epoch = 1;
   BITS_TRY(reset_sort_ctx(L.b, st));
-  BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
-  return launch_count(a_start, a_end, (uint32_t)n_a, L.b, counts_out, total_out, st);
+  // Large query sets against a large B: queries binned by B's buckets, every bucket searched out of shared
+  // memory (binned_count.cuh); needs the MSD sort's plan.  The index path behind it runs only if the sort fell back.
+  const bool can_bin = g_opt.sort_msd != 0 && !(flags & BITS_B_SORTED);
+  const bool binned = can_bin && (g_opt.count_binned > 0 || (g_opt.count_binned < 0 && n_a >= (1u << 20) && n_b >= (3u << 20)));
+  if (!binned) {
+    BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
+    return launch_count(a_start, a_end, (uint32_t)n_a, L.b, counts_out, total_out, st);
+  }
+  BITS_CUDA_TRY(cudaMemsetAsync(L.ql.hist, 0, sizeof(uint32_t) * (msd::kBins + 64), st));
+  BITS_TRY(sort_arrays(L.b, b_start, b_end, 2, nullptr, false, &epoch, st));
+  BITS_TRY(launch_binned_count(a_start, a_end, (uint32_t)n_a, L, counts_out, total_out, st));
+  BITS_TRY(launch_build_index(L.b, st, L.b.msd_flag));
+  return launch_count(a_start, a_end, (uint32_t)n_a, L.b, counts_out, total_out, st, L.b.msd_flag);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1309,6 +1392,8 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "mc_tile_variant")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_tile_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 3) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_gather_group")) { if (value < -1 || value > 5) return BITS_ERR_FLAGS; g_opt.mc_gather_group = value; return BITS_OK; }
+  if (!strcmp(name, "msd_pack")) { if (value < 0 || value > msd::kBucketCap) return BITS_ERR_FLAGS; g_opt.msd_pack = value; return BITS_OK; }
+  if (!strcmp(name, "count_binned")) { if (value < -1 || value > 1) return BITS_ERR_FLAGS; g_opt.count_binned = value; return BITS_OK; }
   if (!strcmp(name, "mc_shift_bias")) { if (value < 0 || value > 8) return BITS_ERR_FLAGS; g_opt.mc_shift_bias = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }

@@ -139,8 +139,13 @@ struct PlanArr {
   uint32_t* flag;           // [1] out: kFlagBucketTooBig or 0 (plain store: this also resets it)
   uint32_t* lsd_hist;       // [1024] cleared here for the fallback sort's digit histograms (may be null)
   uint32_t* lsd_ticket;     // [4] cleared here: the fallback sort's tile tickets, one per pass (may be null)
+  uint16_t* bucket_of_bin;  // [kBins] out (may be null): the bucket every bin belongs to (binned_count.cuh)
+  uint32_t* bucket_lo;      // [kBins + 1] out (may be null): first bin of bucket d; bucket_lo[n_buckets] = kBins
 };
-struct PlanArgs { PlanArr p[2]; };
+struct PlanArgs {
+  PlanArr p[2];
+  uint32_t pack_cap;        // 0: buckets by the prefix / target rule; else consecutive bins are packed greedily up to this many keys
+};
 
 __global__ void __launch_bounds__(1024) plan_kernel(PlanArgs a) {
   static_assert(kBins == 4096, "4 bins per thread");
@@ -169,19 +174,47 @@ __global__ void __launch_bounds__(1024) plan_kernel(PlanArgs a) {
   __syncthreads();
   const uint32_t target = big < (uint32_t)kBucketCap ? (uint32_t)kBucketCap - big + 1u : 1u;
 #pragma unroll
-  for (int j = 0; j < 4; ++j) { ex[j] += before; s_raw[4 * t + j + 1] = ex[j] / target; }
+  for (int j = 0; j < 4; ++j) ex[j] += before;
   reinterpret_cast<uint4*>(P.bin_cursor)[t] = make_uint4(ex[0], ex[1], ex[2], ex[3]);
-  if (t == 0) s_raw[0] = 0xffffffffu;
-  __syncthreads();
   uint32_t first[4], nf = 0, fex[4];
+  if (a.pack_cap) {
+    // greedy packing: a bucket takes consecutive bins while it stays within pack_cap keys (fuller buckets than the
+    // rule below: fewer of them, fewer fixed costs per bucket).  Sequential inside chunks of 64 bins, one thread per
+    // chunk; a chunk boundary always starts a bucket.
+    __shared__ uint8_t s_first[kBins];
 #pragma unroll
-  for (int j = 0; j < 4; ++j) { first[j] = s_raw[4 * t + j + 1] != s_raw[4 * t + j]; fex[j] = nf; nf += first[j]; }
+    for (int j = 0; j < 4; ++j) s_raw[4 * t + j] = ex[j];
+    if (t == 0) s_raw[kBins] = total;
+    __syncthreads();
+    if (t < kBins / 64) {
+      uint32_t from = s_raw[64 * t];
+      s_first[64 * t] = 1;
+      for (int b = 64 * t + 1; b < 64 * t + 64; ++b) {
+        const bool brk = s_raw[b + 1] - from > a.pack_cap;
+        if (brk) from = s_raw[b];
+        s_first[b] = brk ? 1 : 0;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { first[j] = s_first[4 * t + j]; fex[j] = nf; nf += first[j]; }
+  } else {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) s_raw[4 * t + j + 1] = ex[j] / target;
+    if (t == 0) s_raw[0] = 0xffffffffu;
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { first[j] = s_raw[4 * t + j + 1] != s_raw[4 * t + j]; fex[j] = nf; nf += first[j]; }
+  }
   uint32_t nb;
   const uint32_t fbefore = block_excl_scan<1024>(nf, s_w, &nb);
 #pragma unroll
-  for (int j = 0; j < 4; ++j)
-    if (first[j]) { const uint32_t d = fbefore + fex[j]; P.bucket_start[d] = ex[j]; s_start[d] = ex[j]; }
-  if (t == 0) { P.bucket_start[nb] = total; s_start[nb] = total; *P.n_buckets = nb; }
+  for (int j = 0; j < 4; ++j) {
+    const uint32_t d = fbefore + fex[j] + first[j] - 1u;       // bucket of bin 4t + j (bin 0 always starts one)
+    if (first[j]) { P.bucket_start[d] = ex[j]; s_start[d] = ex[j]; if (P.bucket_lo) P.bucket_lo[d] = 4u * t + j; }
+    if (P.bucket_of_bin) P.bucket_of_bin[4 * t + j] = (uint16_t)d;
+  }
+  if (t == 0) { P.bucket_start[nb] = total; s_start[nb] = total; *P.n_buckets = nb; if (P.bucket_lo) P.bucket_lo[nb] = (uint32_t)kBins; }
   __syncthreads();
   bool bad = false;
   for (uint32_t d = t; d < nb; d += 1024) bad |= (s_start[d + 1] - s_start[d]) > (uint32_t)kBucketCap;

@@ -79,6 +79,8 @@ struct IndexArgs {
   uint32_t* idx[2];
   uint32_t n;
   uint32_t shift;
+  uint64_t total;           // threads' worth of work: four positions each, a multiple of the block size
+  const uint32_t* run_if;   // null: always; else dev uint32[2]: run only if one of them is non-zero (fallback behind binned_count.cuh)
 };
 
 __global__ void __launch_bounds__(256) build_index_kernel(IndexArgs a) {
@@ -87,49 +89,54 @@ __global__ void __launch_bounds__(256) build_index_kernel(IndexArgs a) {
   const uint32_t n = a.n, s = a.shift;
   const uint32_t H = 1u << (32 - s);
   grid_dependency_wait();
-  const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;   // warps are never partly out of range
+  if (a.run_if && (a.run_if[0] | a.run_if[1]) == 0u) return;
+  const uint64_t gid0 = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   const uint32_t lane = threadIdx.x & 31;
-  if (gid < kPad) keys[(uint64_t)n + gid] = 0xffffffffu;
   {
     // idx[(key[n-1] >> s) + 1 .. H] = n: the entries above the largest key (for a genome that ends well
     // below 2^32 that is a long run) are filled by the whole grid, not by one thread
     const uint64_t tail_lo = n ? (uint64_t)(keys[n - 1] >> s) + 1u : 0u;
-    for (uint64_t h = tail_lo + gid; h <= H; h += (uint64_t)gridDim.x * blockDim.x) idx[h] = n;
+    for (uint64_t h = tail_lo + gid0; h <= H; h += stride) idx[h] = n;
   }
-  // four consecutive positions per thread (one 16-byte load; the arrays are 32-byte aligned and padded)
-  const uint64_t i0 = gid << 2;
-  uint32_t k[4] = {0, 0, 0, 0};
-  uint32_t prev = 0;
-  if (i0 < n) {
-    if (i0 + 3 < n) {
-      const uint4 v = *reinterpret_cast<const uint4*>(keys + i0);
-      k[0] = v.x; k[1] = v.y; k[2] = v.z; k[3] = v.w;
-    } else {
+  // four consecutive positions per thread (one 16-byte load; the arrays are 32-byte aligned and padded);
+  // a.total is a multiple of the block size, so warps are never partly out of range
+  for (uint64_t gid = gid0; gid < a.total; gid += stride) {
+    if (gid < kPad) keys[(uint64_t)n + gid] = 0xffffffffu;
+    const uint64_t i0 = gid << 2;
+    uint32_t k[4] = {0, 0, 0, 0};
+    uint32_t prev = 0;
+    if (i0 < n) {
+      if (i0 + 3 < n) {
+        const uint4 v = *reinterpret_cast<const uint4*>(keys + i0);
+        k[0] = v.x; k[1] = v.y; k[2] = v.z; k[3] = v.w;
+      } else {
 #pragma unroll
-      for (int j = 0; j < 4; ++j) k[j] = i0 + j < n ? keys[i0 + j] : 0u;
+        for (int j = 0; j < 4; ++j) k[j] = i0 + j < n ? keys[i0 + j] : 0u;
+      }
+      if (i0) prev = keys[i0 - 1];
     }
-    if (i0) prev = keys[i0 - 1];
-  }
 #pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    const uint32_t i = (uint32_t)i0 + j;
-    uint32_t lo = 1, hi = 0;   // fill idx[lo..hi] = i  (empty by default)
-    if (i0 + j < n) {
-      lo = (i == 0) ? 0u : (prev >> s) + 1u;
-      hi = k[j] >> s;
-    }
-    prev = k[j];
-    const bool some = lo <= hi;
-    const uint32_t len = some ? hi - lo + 1u : 0u;
-    if (some && len <= 4)
-      for (uint32_t h = lo; h <= hi; ++h) idx[h] = i;
-    uint32_t big = __ballot_sync(kFullMask, len > 4);
-    while (big) {
-      const int src = __ffs(big) - 1;
-      big &= big - 1;
-      const uint32_t l = __shfl_sync(kFullMask, lo, src), hh = __shfl_sync(kFullMask, hi, src);
-      const uint32_t v = __shfl_sync(kFullMask, i, src);
-      for (uint64_t h = (uint64_t)l + lane; h <= hh; h += 32) idx[h] = v;
+    for (int j = 0; j < 4; ++j) {
+      const uint32_t i = (uint32_t)i0 + j;
+      uint32_t lo = 1, hi = 0;   // fill idx[lo..hi] = i  (empty by default)
+      if (i0 + j < n) {
+        lo = (i == 0) ? 0u : (prev >> s) + 1u;
+        hi = k[j] >> s;
+      }
+      prev = k[j];
+      const bool some = lo <= hi;
+      const uint32_t len = some ? hi - lo + 1u : 0u;
+      if (some && len <= 4)
+        for (uint32_t h = lo; h <= hi; ++h) idx[h] = i;
+      uint32_t big = __ballot_sync(kFullMask, len > 4);
+      while (big) {
+        const int src = __ffs(big) - 1;
+        big &= big - 1;
+        const uint32_t l = __shfl_sync(kFullMask, lo, src), hh = __shfl_sync(kFullMask, hi, src);
+        const uint32_t v = __shfl_sync(kFullMask, i, src);
+        for (uint64_t h = (uint64_t)l + lane; h <= hh; h += 32) idx[h] = v;
+      }
     }
   }
 }
@@ -179,10 +186,12 @@ template <bool kVec, int kSearch>
 __global__ void __launch_bounds__(256) count_kernel(const uint32_t* __restrict__ a_start,
                                                     const uint32_t* __restrict__ a_end, uint32_t n_a,
                                                     SortedSet bs, SortedSet be,
-                                                    uint32_t* __restrict__ counts, unsigned long long* total) {
+                                                    uint32_t* __restrict__ counts, unsigned long long* total,
+                                                    const uint32_t* run_if) {
   __shared__ uint64_t s_red[8];
   __shared__ uint32_t s_top[kSearch == kSearchStaged ? 2 * kStaged : 1];
   grid_dependency_wait();
+  if (run_if && (run_if[0] | run_if[1]) == 0u) return;   // (fallback behind binned_count.cuh: runs only if the MSD sort fell back)
   if (kSearch == kSearchStaged) {
     stage_top_levels(bs, s_top);
     stage_top_levels(be, s_top + kStaged);

@@ -127,16 +127,58 @@ def test_place_many_chromosomes_and_unaligned_pointers():
 
 # ------------------------------------------------------------------------------------- count
 def check_counts(a_s, a_e, b_s, b_e, flags=0, b_for_gpu=None):
+    """Per-interval counts and totals against the oracle, by both designs of the search step: queries binned by B's
+    buckets and searched out of shared memory (count_binned = 1, the default for large sets) and the bucket index
+    (count_binned = 0); -1 = the library's own choice by size."""
     want_total, want_counts = oracle.count_per_interval(a_s, a_e, b_s, b_e)
     gb_s, gb_e = b_for_gpu if b_for_gpu is not None else (b_s, b_e)
     d = [dev(x) for x in (a_s, a_e, gb_s, gb_e)]
-    counts, total = bits.count_per_interval(*d, flags=flags)
-    total_only = bits.count(*d, flags=flags)
-    sync()
-    assert np.array_equal(host_u32(counts), want_counts)
-    assert int(host_u64(total)[0]) == want_total
-    assert int(host_u64(total_only)[0]) == want_total
+    try:
+        for binned in (1, 0, -1):
+            bits.set_option("count_binned", binned)
+            counts, total = bits.count_per_interval(*d, flags=flags)
+            total_only = bits.count(*d, flags=flags)
+            sync()
+            bad = np.nonzero(host_u32(counts) != want_counts)[0]
+            assert bad.size == 0, (binned, bad.size, bad[:5])
+            assert int(host_u64(total)[0]) == want_total, binned
+            assert int(host_u64(total_only)[0]) == want_total, binned
+    finally:
+        bits.set_option("count_binned", -1)
     return want_total
+
+
+def test_count_binned_queries_special_cases():
+    """binned_count.cuh: queries longer than a bucket (their start lies before the bucket's coordinate range: `last`
+    by a global search), a bucket range holding more ends than the staging buffer, buckets with several work items
+    (more than 4,096 queries), and a searched set whose MSD sort falls back to the LSD sort (the binned kernels
+    exit, the index path behind them answers)."""
+    rng = np.random.default_rng(90)
+    G = 3_000_000_000
+    b_s = rng.integers(0, G, 400_000)
+    b_e = b_s + rng.integers(0, 5000, 400_000)
+    # (1) long queries: spans up to 2^23, far beyond the 2^20-wide bins
+    a_s = rng.integers(0, G, 60_000)
+    a_e = a_s + rng.integers(0, 2**23, 60_000)
+    check_counts(a_s, a_e, b_s, b_e)
+    # (2) 30,000 long intervals of B end inside one 2^20-wide bin: more ends in that bucket's range than kCapE
+    ls = rng.integers(0, 2_000_000_000, 30_000)
+    le = 2_500_000_000 + rng.integers(0, 900_000, 30_000)
+    b2_s, b2_e = np.concatenate([b_s, ls]), np.concatenate([b_e, le])
+    qs = 2_500_000_000 + rng.integers(-500_000, 1_200_000, 50_000)
+    check_counts(np.concatenate([a_s, qs]), np.concatenate([a_e, qs + rng.integers(0, 3000, 50_000)]), b2_s, b2_e)
+    # (3) 40,000 queries inside one bucket (ten work items), the rest spread out
+    qs = 1_000_000_000 + rng.integers(0, 500_000, 40_000)
+    check_counts(np.concatenate([qs, a_s[:5000]]), np.concatenate([qs + rng.integers(0, 300, 40_000), a_e[:5000]]), b_s, b_e)
+    # (4) 60,000 starts inside one bin: the MSD sort raises its flag, the LSD sort and the index path take over
+    cs = 123_456_789 + rng.integers(0, 200_000, 60_000)
+    b4_s, b4_e = np.concatenate([b_s[:50_000], cs]), np.concatenate([b_e[:50_000], cs + rng.integers(0, 100, 60_000)])
+    bits.set_option("count_binned", 1)
+    try:
+        check_counts(a_s[:20_000], a_e[:20_000], b4_s, b4_e)
+    finally:
+        bits.set_option("count_binned", -1)
+
 
 
 def test_count_config1_tiny():
