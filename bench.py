@@ -34,26 +34,26 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
-NCU_TRAFFIC_BYTES: dict = {
-    # profiles/r1b_fused_ncu_full_summary.txt (config 5, one launch)
-    "bin_sort_search_kernel": 128_459_264,     # 91.32 MB read + 37.14 MB written
-    "place_tile_kernel": 70_430_464,           # 40.11 MB read + 30.32 MB written
-}
-# what the same capture says bounds each kernel (neither is near its HBM roofline)
-NCU_LIMITER: dict = {
-    "bin_sort_search_kernel": {"issue_slots_busy": 0.707, "shared_memory_pipe": 0.654, "dram_throughput": 0.124,
-                               "note": "instruction issue and the shared-memory pipe, not HBM"},
-    "place_tile_kernel": {"issue_slots_busy": 0.524, "shared_memory_pipe": 0.473, "dram_throughput": 0.131,
-                          "note": "dependent-instruction latency at one 1024-thread block per SM"},
-}
-# warp instructions per launch from the same capture (smsp__inst_executed.sum): with the live launch duration and
-# SM clock they give the share of the issue slots the kernel fills (148 SMs x 4 schedulers x 1 warp instruction per
-# cycle, B300_MICROARCH.md / DESIGN.md section 7) -- the bound the two kernels actually run into
-NCU_WARP_INSTRUCTIONS: dict = {
-    "bin_sort_search_kernel": 93_573_124,
-    "place_tile_kernel": 35_762_284,
-}
+# Counters of the dominant kernels that only ncu can give (DRAM bytes, warp instructions, what bounds the kernel) live
+# in profiles/r2b_fused_ncu_counters.json, written from the committed `ncu --set full` capture together with the hash
+# of the kernel sources it was taken of (paper_1208_3407_b200.build.csrc_hash()).  They are reported only while that
+# hash is the one of the sources this run was built from; otherwise the line says "stale_capture".
+NCU_COUNTERS_FILE = os.path.join(ROOT, "profiles", "r2b_fused_ncu_counters.json")
+
+
+def ncu_counters():
+    """(counters by kernel, note) -- counters are {} when the capture is missing or belongs to other kernel sources."""
+    from paper_1208_3407_b200 import build as B
+    if not os.path.exists(NCU_COUNTERS_FILE):
+        return {}, "no capture file"
+    with open(NCU_COUNTERS_FILE) as f:
+        d = json.load(f)
+    have = B.csrc_hash()
+    if d.get("csrc_hash") != have:
+        return {}, f"stale_capture: {os.path.basename(NCU_COUNTERS_FILE)} was taken of csrc {d.get('csrc_hash')}, this build is {have}"
+    return d.get("kernels", {}), f"from {os.path.basename(NCU_COUNTERS_FILE)} (csrc {have}, workload {d.get('workload')})"
+
+
 N_SMS, SCHEDULERS_PER_SM = 148, 4
 HBM_FALLBACK_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
@@ -332,15 +332,31 @@ def secondary_workloads(device, peak_gbs):
     torch.cuda.synchronize()
     prof = bits.profile_read(); bits.set_option("profile", 0)
     ms = {k: v[0] / calls for k, v in prof.items()}     # device ms per call and kernel class
-    sort_ms = ms["histogram"] + ms["plan"] + ms["scatter"] + ms["bucket_sort"]   # MSD bucket sort of B's starts and ends
+    n, q = w.n_b, w.n_a
+    # (the histogram and plan classes now hold two launches each: B's bins + plan, the queries' buckets + plan)
+    sort_ms = ms["scatter"] + ms["bucket_sort"] + (ms["histogram"] + ms["plan"]) * (8 * n) / (8 * n + 4 * q)
+    # algorithmic HBM bytes per call of every kernel class of this path and what that is of the peak
+    alg = {"histogram": 8 * n + 4 * q, "scatter": 16 * n, "bucket_sort": 16 * n, "query_scatter": 20 * q, "bucket_search": 16 * q + 8 * n}
     out["cfg4_large_count_10M"] = {
         "intervals_searched_per_s": w.n_a / (med * 1e-3), "ms_median": med, "ms_min": mn,
         "sort_keys_per_s": 2 * w.n_b / (sort_ms * 1e-3) if sort_ms else None,
-        "kernel_ms": {"histogram": ms["histogram"], "plan": ms["plan"], "scatter": ms["scatter"], "bucket_sort": ms["bucket_sort"],
-                      "lsd_fallback_pass": ms["sort_pass"], "index_build": ms["index_build"], "count": ms["count"]},
+        "search_design": "queries binned by B's buckets, buckets searched out of shared memory (binned_count.cuh)" if ms.get("bucket_search") else "bucket index (search.cuh)",
+        "kernel_ms": {k: v for k, v in ms.items() if v},
+        "kernel_roofline": {k: {"algorithmic_bytes": b, "ms": ms[k], "achieved_gbs": b / (ms[k] * 1e-3) / 1e9,
+                                "frac_of_hbm_peak": b / (ms[k] * 1e-3) / 1e9 / peak_gbs} for k, b in alg.items() if ms.get(k)},
         "hbm_bytes_model": 72 * w.n_b + 12 * w.n_a + 8 * w.n_b,
         "hbm_frac_of_peak": (72 * w.n_b + 12 * w.n_a + 8 * w.n_b) / (med * 1e-3) / 1e9 / peak_gbs,
+        "hbm_bytes_this_design": sum(alg.values()),
+        "hbm_frac_of_peak_this_design": sum(alg.values()) / (med * 1e-3) / 1e9 / peak_gbs,
+        "note": "hbm_bytes_model is SURVEY 8(d)'s model of the unfused LSD path (920 MB); hbm_bytes_this_design is what this path must move",
     }
+    # the same call with the round-1 search design (bucket index + count_kernel), beside it
+    bits.set_option("count_binned", 0)
+    try:
+        med0, mn0 = time_device(lambda: bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total), 10)
+    finally:
+        bits.set_option("count_binned", -1)
+    out["cfg4_large_count_10M"]["bucket_index_design"] = {"ms_median": med0, "ms_min": mn0, "intervals_searched_per_s": w.n_a / (med0 * 1e-3)}
     out["yardsticks"] = library_yardsticks(device, w, d)
     del d, ws, counts
     # config 3: 1e4 queries re-placed per round against a fixed 1e6-interval B, 10,000 rounds, fused kernel
@@ -504,28 +520,37 @@ def run_b200(args):
             kname, alg_bytes = alg[dom]
             launch_ms = timed[dom][0] / timed[dom][1]
             achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+            counters, counters_note = ncu_counters() if (args.config == 5 and args.scale == 1.0 and not args.opt) else ({}, "not the captured workload")
+            kc = counters.get(kname, {})
             roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                         "frac": achieved / peak,
-                        "traffic": NCU_TRAFFIC_BYTES.get(kname) if (args.config == 5 and args.scale == 1.0) else None,
-                        "ncu_limiter": NCU_LIMITER.get(kname) if (args.config == 5 and args.scale == 1.0) else None,
+                        "traffic": kc.get("dram_bytes"), "ncu_limiter": kc.get("limiter"), "ncu_counters": counters_note,
                         "peak_source": peak_src,
                         "avg_launch_ms": launch_ms, "launches_timed": timed[dom][1],
                         "algorithmic_bytes_per_launch": alg_bytes,
                         "kernel_ms_per_round": {k: v[0] / (R * prof_steps) for k, v in timed.items()},
                         "timed_in": f"{prof_steps} extra step(s) right behind the timed region, one event pair per launch",
                         "kernel_share_of_step": {k: v[0] / tot for k, v in timed.items()}}
-            if kname in NCU_WARP_INSTRUCTIONS and args.config == 5 and args.scale == 1.0:
-                roofline["issue_slots"] = {"warp_instructions_per_launch": NCU_WARP_INSTRUCTIONS[kname],
+            if kc.get("warp_instructions"):
+                roofline["issue_slots"] = {"warp_instructions_per_launch": kc["warp_instructions"],
                                            "peak_per_s_formula": "148 SMs x 4 schedulers x sm_mhz (filled in below)"}
             if n_sorted:
-                # SURVEY 8(d) per-round model: place 12 M + sort 72 M (histogram fused: - 8 M) + search 8 N_q
-                model = 12 * n_sorted + 72 * n_sorted - 8 * n_sorted + 8 * w.n_a
-                roofline["round_hbm_bytes_model"] = model
-                roofline["round_frac_of_peak"] = model * value / world / 1e9 / peak
-                # what the two-launch design itself must move per round
+                # what the two-launch design itself moves per round: the measured fraction of the round
                 own = 12 * n_sorted + 16 * n_sorted + 8 * w.n_a
                 roofline["round_hbm_bytes_this_design"] = own
                 roofline["round_frac_of_peak_this_design"] = own * value / world / 1e9 / peak
+                # SURVEY 8(d)'s per-round byte model of the UNFUSED path (place 12 M + one histogram read and four 8-bit
+                # radix passes 72 M + search 8 N_q = 848 MB on config 5; 768 MB with the histogram fused into placement):
+                # rounds/s times these bytes is a speed-up against that modelled design expressed in bandwidth units,
+                # NOT bytes this implementation moves -- its kernels are bound by instruction issue, not by HBM
+                survey = 12 * n_sorted + 72 * n_sorted + 8 * w.n_a
+                roofline["round_hbm_bytes_model_survey"] = survey
+                roofline["round_frac_of_peak_model_survey"] = survey * value / world / 1e9 / peak
+                roofline["round_hbm_bytes_model_survey_hist_fused"] = survey - 8 * n_sorted
+                roofline["round_frac_of_peak_model_survey_hist_fused"] = (survey - 8 * n_sorted) * value / world / 1e9 / peak
+                roofline["round_frac_note"] = ("round_frac_of_peak_this_design is the measured fraction; the *_model_survey figures credit "
+                                               "the passes the fused design does not make (SURVEY 8d: 'credit taken as >100 % of this model, "
+                                               "model unchanged')")
 
     line = {
         "metric": "mc_rounds_per_s", "value": value, "unit": "rounds/s", "n_gpus": world, "steps": args.steps,
@@ -611,6 +636,20 @@ def run_b200(args):
                                                              observed_out=obs, round_counts_out=rc2), 3, warmup=1)
             finally:
                 bits.set_option("mc_symmetric", 0)
+            # the literal path (general placement kernel -> MSD sort of both arrays -> bucket index -> one ICOUNT per query),
+            # beside the headline: same integers, no fused kernels, no sorted queries
+            Rl = min(R, 20)
+            rc3 = torch.empty(Rl, dtype=torch.int64, device=device)
+            bits.set_option("mc_fused", 0); bits.set_option("mc_sorted_queries", 0)
+            try:
+                medl, _ = time_device(lambda: bits.mc_rounds(*d, w.chrom_offsets, w.which, w.mc_seed, r0, Rl, workspace=ws2,
+                                                             observed_out=obs, round_counts_out=rc3), 3, warmup=1)
+            finally:
+                bits.set_option("mc_fused", 1); bits.set_option("mc_sorted_queries", 1)
+            line["other_workloads"]["cfg5_literal_path"] = {
+                "mc_rounds_per_s": Rl / (medl * 1e-3), "rounds_per_call": Rl, "ms_median": medl,
+                "path": "place_kernel -> MSD sort of B_S and B_E -> bucket index -> count_kernel (one ICOUNT per query), per round",
+                "same_counts_as_headline_path": bool(torch.equal(rc3, rc[:Rl]))}
             line["other_workloads"]["cfg5_symmetric_sort_free"] = {
                 "mc_rounds_per_s": Rs / (med * 1e-3), "rounds_per_call": Rs, "ms_median": med,
                 "intervals_searched_per_s": Rs * w.n_b / (med * 1e-3),

@@ -21,6 +21,17 @@ FLAGS = [
 ]
 
 
+def csrc_hash() -> str:
+    """sha256 over the kernel sources (csrc/*.cu, *.cuh, sorted by name): identifies the build a profile was taken of."""
+    import hashlib
+    h = hashlib.sha256()
+    for path in sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))):
+        h.update(os.path.basename(path).encode())
+        with open(path, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def sources() -> list[str]:
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
