@@ -205,15 +205,23 @@ def decide(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None) -> to
     return out
 
 
-def enumerate_pairs(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None):
+def enumerate_pairs(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None, capacity: int | None = None):
     """bits_enumerate -> (pair_a, pair_b, total): every intersecting pair as indices into A and B (device int32-typed
-    uint32 tensors of `total` elements).  Two calls: the first (capacity 0) sizes the outputs; synchronises once."""
+    uint32 tensors).  capacity = None: two calls, the first (capacity 0) sizes the outputs, `total` elements come
+    back; synchronises once.  capacity = n: ONE call into arrays of n elements (no sort + count twice); pairs beyond n
+    are not written, `total` is the full count either way."""
     dev = a_start.device
     n_a, n_b = a_start.numel(), b_start.numel()
     ws = _workspace(workspace_bytes(FN_ENUMERATE, n_a, n_b, 0, 0, flags), workspace, dev)
     total = torch.zeros(1, dtype=torch.int64, device=dev)
     args = (_dev_u32(a_start, "a_start"), _dev_u32(a_end, "a_end"), n_a, _dev_u32(b_start, "b_start"), _dev_u32(b_end, "b_end"), n_b,
             flags, ws.data_ptr(), ws.numel())
+    if capacity is not None:
+        pa = torch.empty(capacity, dtype=torch.int32, device=dev)
+        pb = torch.empty(capacity, dtype=torch.int32, device=dev)
+        _chk(lib().bits_enumerate(*args, pa.data_ptr() if capacity else 0, pb.data_ptr() if capacity else 0, capacity,
+                                  total.data_ptr(), _stream()))
+        return pa, pb, int(total.item())
     _chk(lib().bits_enumerate(*args, 0, 0, 0, total.data_ptr(), _stream()))
     n = int(total.item())
     pa = torch.empty(n, dtype=torch.int32, device=dev)

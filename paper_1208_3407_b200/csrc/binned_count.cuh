@@ -9,10 +9,10 @@
 // of queries and counts stream (profiles/r2a_cfg4_launches.md: 770 MB read for 200 MB of
 // algorithmic traffic).  Here the random accesses become streams:
 //
-//   query_hist_kernel     bucket of every query (bucket = the MSD sort's bucket of B_S that holds
-//                         a.end's bin, msd_sort.cuh plan_kernel) -> queries per bucket.
-//   query_plan_kernel     exclusive scan: where each bucket's queries go; work items of at most
-//                         kChunk queries of one bucket.
+//   (msd::bin_hist_kernel, msd::plan_kernel)  the queries' ends are histogrammed by bin in the sort's own
+//                         histogram launch; the block that plans B_S turns that into queries per bucket
+//                         (bucket = the MSD sort's bucket of B_S that holds a.end's bin), where each
+//                         bucket's queries go, and work items of at most kChunk queries of one bucket.
 //   query_scatter_kernel  one pass over the queries: (a.end, a.start, input index) leave in bucket
 //                         order (tile-local ranks by shared-memory atomics, one global reservation
 //                         per tile and bucket, staged so that a bucket's writes are contiguous).
@@ -55,7 +55,7 @@ struct Lists {                       // the queries in bucket order (workspace)
   uint32_t* q_end;                   // [n_a]
   uint32_t* q_start;                 // [n_a]
   uint32_t* q_idx;                   // [n_a] input index (used only when per-interval counts are wanted)
-  uint32_t* hist;                    // [kBins] queries per bucket (zero on entry)
+  uint32_t* hist;                    // [kBins] queries per BIN (zero on entry; filled by the sort's histogram launch, read and cleared by its plan)
   uint32_t* off;                     // [kBins + 1] exclusive prefix of hist
   uint32_t* cursor;                  // [kBins] reservation cursors of the scatter pass
   uint32_t* item_off;                // [kBins + 1] exclusive prefix of the work items per bucket
@@ -63,59 +63,6 @@ struct Lists {                       // the queries in bucket order (workspace)
 };
 
 __device__ __forceinline__ bool sort_fell_back(const uint32_t* flag) { return (flag[0] | flag[1]) != 0u; }
-
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) query_hist_kernel(const uint32_t* __restrict__ a_end, uint32_t n_a, Plan p, Lists l) {
-  __shared__ uint32_t s_h[msd::kBins];
-  __shared__ uint16_t s_tbl[msd::kBins];
-  grid_dependency_wait();
-  if (sort_fell_back(p.flag)) return;
-  for (int i = threadIdx.x; i < msd::kBins; i += blockDim.x) { s_h[i] = 0; s_tbl[i] = p.bucket_of_bin[i]; }
-  __syncthreads();
-  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-  if (((uintptr_t)a_end & 15) == 0) {
-    const uint32_t n4 = n_a >> 2;
-    const uint4* k4 = reinterpret_cast<const uint4*>(a_end);
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
-      const uint4 k = __ldg(k4 + i);
-      atomicAdd(&s_h[s_tbl[k.x >> msd::kBinShift]], 1u); atomicAdd(&s_h[s_tbl[k.y >> msd::kBinShift]], 1u);
-      atomicAdd(&s_h[s_tbl[k.z >> msd::kBinShift]], 1u); atomicAdd(&s_h[s_tbl[k.w >> msd::kBinShift]], 1u);
-    }
-    if (blockIdx.x == 0 && threadIdx.x < (n_a & 3u)) atomicAdd(&s_h[s_tbl[a_end[(n_a & ~3u) + threadIdx.x] >> msd::kBinShift]], 1u);
-  } else {
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_a; i += stride)
-      atomicAdd(&s_h[s_tbl[a_end[i] >> msd::kBinShift]], 1u);
-  }
-  __syncthreads();
-  for (int i = threadIdx.x; i < msd::kBins; i += blockDim.x) if (s_h[i]) atomicAdd(&l.hist[i], s_h[i]);
-}
-
-// one block of 1,024 threads, four buckets per thread
-__global__ void __launch_bounds__(1024) query_plan_kernel(Plan p, Lists l) {
-  __shared__ uint32_t s_w[32];
-  grid_dependency_wait();
-  if (sort_fell_back(p.flag)) return;
-  const int t = threadIdx.x;
-  const uint4 v = reinterpret_cast<const uint4*>(l.hist)[t];
-  const uint32_t h[4] = {v.x, v.y, v.z, v.w};
-  uint32_t items[4], sum = 0, isum = 0;
-#pragma unroll
-  for (int j = 0; j < 4; ++j) { items[j] = (h[j] + kChunk - 1) / kChunk; sum += h[j]; isum += items[j]; }
-  uint32_t total, itotal;
-  uint32_t run = msd::block_excl_scan<1024>(sum, s_w, &total);
-  __syncthreads();
-  uint32_t irun = msd::block_excl_scan<1024>(isum, s_w, &itotal);
-  uint32_t o[4], io[4];
-#pragma unroll
-  for (int j = 0; j < 4; ++j) { o[j] = run; run += h[j]; io[j] = irun; irun += items[j]; }
-  reinterpret_cast<uint4*>(l.off)[t] = make_uint4(o[0], o[1], o[2], o[3]);
-  reinterpret_cast<uint4*>(l.cursor)[t] = make_uint4(o[0], o[1], o[2], o[3]);
-  reinterpret_cast<uint4*>(l.item_off)[t] = make_uint4(io[0], io[1], io[2], io[3]);
-  if (t == 0) { l.off[msd::kBins] = total; l.item_off[msd::kBins] = itotal; }
-#pragma unroll
-  for (int j = 0; j < 4; ++j)
-    for (uint32_t k = 0; k < items[j]; ++k) l.item_bucket[io[j] + k] = (uint16_t)(4 * t + j);
-}
 
 // ---------------------------------------------------------------------------------------------
 // Scatter of the queries into bucket order.  Persistent blocks of 1,024 threads, tiles of 16,384 queries

@@ -402,8 +402,15 @@ static int msd_configure() {
 // MSD bucket sort (plan -> scatter -> bucket sort) with the LSD sort as device-side fallback.
 // bin_hist_ready: c.bin_hist already holds the top-bits histogram of the sources (made by the
 // placement kernel).  The stage is complete once the stream reaches the end of what is enqueued.
+// `queries` (optional): a query set to be planned into the order of array 0's buckets in the same launches
+// (binned_count.cuh): its ends are histogrammed beside the keys, its plan is made by the block that plans array 0.
+struct QueryBinning {
+  const uint32_t* a_end;
+  uint32_t n_a;
+  msd::QueryPlan plan;
+};
 static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* src1, int n_arrays, uint32_t* y_override,
-                       bool bin_hist_ready, uint32_t* epoch, cudaStream_t st) {
+                       bool bin_hist_ready, uint32_t* epoch, cudaStream_t st, const QueryBinning* queries = nullptr) {
   SortPlan p = plan_for(c, src0, n_arrays > 1 ? src1 : src0, 0);
   p.n_arrays = n_arrays;
   if (y_override) p.y[0] = y_override;
@@ -419,15 +426,18 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     msd::BinHistArgs h;
     h.keys[0] = src0; h.keys[1] = n_arrays > 1 ? src1 : src0;
     h.hist[0] = c.bin_hist[0]; h.hist[1] = c.bin_hist[1];
-    h.n = c.n;
+    h.n[0] = h.n[1] = c.n;
+    h.keys[2] = queries ? queries->a_end : src0; h.hist[2] = queries ? queries->plan.bin_hist : c.bin_hist[0]; h.n[2] = queries ? queries->n_a : 0u;
     ProfScope prof(kClsHist, st);
     // (every block ends with up to 4,096 global reductions: a few resident blocks per SM, not one per 2,048 keys)
-    const int hb = grid_for(ceil_div(c.n, 4), 512);
-    launch_pdl(msd::bin_hist_kernel, dim3(hb < 2 * kSMs ? hb : 2 * kSMs, n_arrays), 512, 0, st, h);
+    const uint32_t n_big = queries && queries->n_a > c.n ? queries->n_a : c.n;
+    const int hb = grid_for(ceil_div(n_big, 4), 512);
+    launch_pdl(msd::bin_hist_kernel, dim3(hb < 2 * kSMs ? hb : 2 * kSMs, queries && n_arrays == 2 ? 3 : n_arrays), 512, 0, st, h);
     BITS_LAUNCH_CHECK();
   }
   {
     msd::PlanArgs pa;
+    if (queries && n_arrays == 2 && !bin_hist_ready) pa.q = queries->plan; else pa.q.bin_hist = nullptr;
     for (int a = 0; a < 2; ++a) {
       pa.p[a].hist = c.bin_hist[a]; pa.p[a].bin_cursor = c.bin_cursor[a]; pa.p[a].bucket_start = c.bucket_start[a];
       pa.p[a].n_buckets = c.n_buckets + a; pa.p[a].flag = c.msd_flag + a; pa.p[a].lsd_hist = c.hist[0][a]; pa.p[a].lsd_ticket = c.ticket + 4 * a;
@@ -569,17 +579,6 @@ static int launch_binned_count(const uint32_t* a_start, const uint32_t* a_end, u
   p.n_buckets = L.b.n_buckets; p.end_cursor = L.b.bin_cursor[1];
   const uint32_t n_tiles = (uint32_t)ceil_div(n_a, (uint64_t)qb::kScTile);
   {
-    ProfScope prof(kClsHist, st);
-    const uint32_t blocks = (uint32_t)ceil_div(ceil_div(n_a, 4), 1024 * 4);
-    launch_pdl(qb::query_hist_kernel, blocks < 2u * kSMs ? (blocks ? blocks : 1u) : 2u * (uint32_t)kSMs, 1024, 0, st, a_end, n_a, p, L.ql);
-    BITS_LAUNCH_CHECK();
-  }
-  {
-    ProfScope prof(kClsPlan, st);
-    launch_pdl(qb::query_plan_kernel, 1, 1024, 0, st, p, L.ql);
-    BITS_LAUNCH_CHECK();
-  }
-  {
     ProfScope prof(kClsQueryScatter, st);
     const uint32_t blocks = n_tiles < (uint32_t)kSMs ? n_tiles : (uint32_t)kSMs;
     if (counts) launch_pdl(qb::query_scatter_kernel<true>, blocks, qb::kScThreads, qb::kScSmem, st, a_start, a_end, n_a, p, L.ql);
@@ -627,7 +626,12 @@ static int count_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n
     return launch_count(a_start, a_end, (uint32_t)n_a, L.b, counts_out, total_out, st);
   }
   BITS_CUDA_TRY(cudaMemsetAsync(L.ql.hist, 0, sizeof(uint32_t) * (msd::kBins + 64), st));
-  BITS_TRY(sort_arrays(L.b, b_start, b_end, 2, nullptr, false, &epoch, st));
+  // (the queries' bin histogram and their plan ride in the sort's own histogram and plan launches)
+  QueryBinning qbin;
+  qbin.a_end = a_end; qbin.n_a = (uint32_t)n_a;
+  qbin.plan.bin_hist = L.ql.hist; qbin.plan.off = L.ql.off; qbin.plan.cursor = L.ql.cursor; qbin.plan.item_off = L.ql.item_off;
+  qbin.plan.item_bucket = L.ql.item_bucket; qbin.plan.chunk = (uint32_t)qb::kChunk;
+  BITS_TRY(sort_arrays(L.b, b_start, b_end, 2, nullptr, false, &epoch, st, &qbin));
   BITS_TRY(launch_binned_count(a_start, a_end, (uint32_t)n_a, L, counts_out, total_out, st));
   BITS_TRY(launch_build_index(L.b, st, L.b.msd_flag));
   return launch_count(a_start, a_end, (uint32_t)n_a, L.b, counts_out, total_out, st, L.b.msd_flag);

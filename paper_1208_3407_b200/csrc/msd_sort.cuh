@@ -95,9 +95,9 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* s_w, u
 // ---------------------------------------------------------------------------------------------
 // 1. histogram of the top kBinBits bits (stand-alone version).  gridDim.y = arrays.
 struct BinHistArgs {
-  const uint32_t* keys[2];
-  uint32_t* hist[2];     // uint32[kBins] each, zero on entry (plan_kernel leaves them zero)
-  uint32_t n;
+  const uint32_t* keys[3];   // [2]: an extra key array histogrammed in the same launch (the query ends of binned_count.cuh)
+  uint32_t* hist[3];         // uint32[kBins] each, zero on entry (plan_kernel leaves them zero)
+  uint32_t n[3];
 };
 
 __global__ void __launch_bounds__(512) bin_hist_kernel(BinHistArgs a) {
@@ -105,8 +105,8 @@ __global__ void __launch_bounds__(512) bin_hist_kernel(BinHistArgs a) {
   grid_dependency_wait();
   for (int i = threadIdx.x; i < kBins; i += blockDim.x) s_h[i] = 0;
   __syncthreads();
-  const uint32_t* __restrict__ keys = blockIdx.y ? a.keys[1] : a.keys[0];
-  const uint32_t n = a.n;
+  const uint32_t* __restrict__ keys = blockIdx.y == 0 ? a.keys[0] : (blockIdx.y == 1 ? a.keys[1] : a.keys[2]);
+  const uint32_t n = blockIdx.y == 0 ? a.n[0] : (blockIdx.y == 1 ? a.n[1] : a.n[2]);
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   if (((uintptr_t)keys & 15) == 0) {
     const uint32_t n4 = n >> 2;
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(512) bin_hist_kernel(BinHistArgs a) {
       atomicAdd(&s_h[keys[i] >> kBinShift], 1u);
   }
   __syncthreads();
-  uint32_t* g = blockIdx.y ? a.hist[1] : a.hist[0];
+  uint32_t* g = blockIdx.y == 0 ? a.hist[0] : (blockIdx.y == 1 ? a.hist[1] : a.hist[2]);
   for (int i = threadIdx.x; i < kBins; i += blockDim.x) if (s_h[i]) atomicAdd(&g[i], s_h[i]);
 }
 
@@ -142,8 +142,19 @@ struct PlanArr {
   uint16_t* bucket_of_bin;  // [kBins] out (may be null): the bucket every bin belongs to (binned_count.cuh)
   uint32_t* bucket_lo;      // [kBins + 1] out (may be null): first bin of bucket d; bucket_lo[n_buckets] = kBins
 };
+// Plan of a query set that is to be brought into the order of array 0's buckets (binned_count.cuh), made by the
+// block that plans array 0: queries per bucket from the queries' own bin histogram.
+struct QueryPlan {
+  uint32_t* bin_hist;       // [kBins] in: histogram of the queries' bins (null: no queries); cleared for the next use
+  uint32_t* off;            // [kBins + 1] out: where each bucket's queries start; off[n_buckets] = number of queries
+  uint32_t* cursor;         // [kBins] out: = off (advanced by the scatter pass)
+  uint32_t* item_off;       // [kBins + 1] out: exclusive prefix of the work items per bucket; [kBins] = their number
+  uint16_t* item_bucket;    // out: the bucket of every work item
+  uint32_t chunk;           // queries per work item
+};
 struct PlanArgs {
   PlanArr p[2];
+  QueryPlan q;
   uint32_t pack_cap;        // 0: buckets by the prefix / target rule; else consecutive bins are packed greedily up to this many keys
 };
 
@@ -215,6 +226,39 @@ __global__ void __launch_bounds__(1024) plan_kernel(PlanArgs a) {
     if (P.bucket_of_bin) P.bucket_of_bin[4 * t + j] = (uint16_t)d;
   }
   if (t == 0) { P.bucket_start[nb] = total; s_start[nb] = total; *P.n_buckets = nb; if (P.bucket_lo) P.bucket_lo[nb] = (uint32_t)kBins; }
+  if (blockIdx.x == 0 && a.q.bin_hist) {
+    // queries per bucket: the exclusive prefix of the queries' bin histogram, read at the buckets' first bins
+    uint32_t* s_qoff = s_raw;                             // (s_raw is free: the barrier of the scan above lies behind its last use)
+    const uint4 qv = reinterpret_cast<const uint4*>(a.q.bin_hist)[t];
+    reinterpret_cast<uint4*>(a.q.bin_hist)[t] = make_uint4(0, 0, 0, 0);
+    const uint32_t qh[4] = {qv.x, qv.y, qv.z, qv.w};
+    uint32_t qtotal;
+    __syncthreads();
+    uint32_t qrun = block_excl_scan<1024>(qh[0] + qh[1] + qh[2] + qh[3], s_w, &qtotal);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      if (first[j]) { const uint32_t d = fbefore + fex[j]; s_qoff[d] = qrun; a.q.off[d] = qrun; a.q.cursor[d] = qrun; }
+      qrun += qh[j];
+    }
+    if (t == 0) { s_qoff[nb] = qtotal; a.q.off[nb] = qtotal; }
+    __syncthreads();
+    uint32_t items[4], isum = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint32_t d = 4u * t + j;
+      items[j] = d < nb ? (s_qoff[d + 1] - s_qoff[d] + a.q.chunk - 1u) / a.q.chunk : 0u;
+      isum += items[j];
+    }
+    uint32_t itotal;
+    uint32_t irun = block_excl_scan<1024>(isum, s_w, &itotal);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      a.q.item_off[4 * t + j] = irun;
+      for (uint32_t k = 0; k < items[j]; ++k) a.q.item_bucket[irun + k] = (uint16_t)(4 * t + j);
+      irun += items[j];
+    }
+    if (t == 0) a.q.item_off[kBins] = itotal;
+  }
   __syncthreads();
   bool bad = false;
   for (uint32_t d = t; d < nb; d += 1024) bad |= (s_start[d + 1] - s_start[d]) > (uint32_t)kBucketCap;

@@ -339,6 +339,11 @@ def test_enumerate_config2_is_valid_and_complete():
     assert np.array_equal(np.bincount(pa, minlength=w.n_a), o_counts)
     assert np.all(np.diff(pa) >= 0)                        # A-major order: slices by exclusive prefix of the counts
     assert np.unique(pa * (1 << 32) + pb).size == n
+    # one call with a known capacity (no sizing call): the same pairs in the same slices
+    qa, qb, n2 = bits.enumerate_pairs(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), capacity=n + 7)
+    sync()
+    assert n2 == n and np.array_equal(host_u32(qa)[:n].astype(np.int64), pa)
+    assert np.array_equal(np.sort(pa * (1 << 32) + host_u32(qb)[:n].astype(np.int64)), np.sort(pa * (1 << 32) + pb))
 
 
 def test_enumerate_walk_is_bounded_when_one_interval_spans_everything():
