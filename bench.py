@@ -706,10 +706,14 @@ def run_study(args):
     if args.study == "count":
         one_design("default")
     else:
+        bits.set_option("count_binned", 0)                 # the three designs of count_kernel over the sorted arrays in global memory ...
         for v, name in SEARCH_DESIGNS:
             bits.set_option("search_variant", v)
             one_design(f"{v}: {name}")
         bits.set_option("search_variant", 0)
+        bits.set_option("count_binned", 1)                 # ... and the queries binned by B's buckets, buckets searched out of shared memory
+        one_design("3: queries binned by B's buckets, shared-memory search (binned_count.cuh) [default at this size]")
+        bits.set_option("count_binned", -1)
         w3 = W.make_config(3, scale=args.scale)
         d3 = [to_dev(x, device) for x in (w3.a_start, w3.a_end, w3.b_start, w3.b_end)]
         R = 100

@@ -35,6 +35,7 @@ struct Options {
   int64_t mc_bin_variant = 0;      // PERMUTE_B fused rounds: shape of the per-bin sort (0 wide, 1 narrow, 2 small blocks)
   int64_t mc_gather_group = -1;    // PERMUTE_B fused rounds: log2 of the lanes per gathered segment (-1 = from the mean segment length)
   int64_t msd_pack = 7168;         // MSD sort plan: 0 = buckets by the prefix / target rule, n = consecutive bins packed greedily up to n keys (measured on config 4: 0 -> 146 us, 8192 -> 134, 7168 -> 124 for the bucket sort)
+  int64_t msd_scatter_shape = 0;   // MSD scatter pass: 0 = one 1,024-thread block per SM and 16,384-key tiles, 1 = two 512-thread blocks and 8,192-key tiles
   int64_t count_binned = -1;       // count path: 1 = queries binned by B's buckets and searched out of shared memory (binned_count.cuh), 0 = bucket index + count_kernel, -1 = by size
   int64_t mc_shift_bias = 0;       // PERMUTE_B fused rounds: added to the bin width (log2) the host picked; > 0 overflows bins on purpose (tests)
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
@@ -374,7 +375,9 @@ static int msd_configure() {
   BITS_CUDA_TRY(cudaGetDevice(&device));
   const bool tracked = device >= 0 && device < kMaxDevices;
   if (!tracked || done_on[device].load(std::memory_order_acquire) == 0) {
-    const cudaError_t e1 = cudaFuncSetAttribute(msd::scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kScSmem);
+    cudaError_t e1 = cudaFuncSetAttribute(msd::scatter_kernel<msd::ScatterCfg1x1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::ScatterCfg1x1024::kSmem);
+    if (e1 == cudaSuccess)
+      e1 = cudaFuncSetAttribute(msd::scatter_kernel<msd::ScatterCfg2x512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::ScatterCfg2x512::kSmem);
     const cudaError_t e2 = cudaFuncSetAttribute(msd::bucket_sort_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
     cudaError_t e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgWide>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)mct::BinCfgWide::smem_bytes(mct::kMaxTiles));
@@ -456,10 +459,19 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
       const int aa = a < n_arrays ? a : 0;
       sa.arr[a].src = p.src[aa]; sa.arr[a].dst = p.x[aa]; sa.arr[a].bin_cursor = c.bin_cursor[aa]; sa.arr[a].flag = c.msd_flag + aa;
     }
-    sa.n = c.n; sa.n_tiles = (uint32_t)ceil_div(c.n, msd::kScTile);
-    const uint32_t per = (uint32_t)kSMs / (uint32_t)n_arrays;
+    sa.n = c.n;
     ProfScope prof(kClsScatter, st);
-    launch_pdl(msd::scatter_kernel, dim3(sa.n_tiles < per ? sa.n_tiles : per, n_arrays), msd::kScThreads, msd::kScSmem, st, sa);
+    if (g_opt.msd_scatter_shape == 0) {
+      using C = msd::ScatterCfg1x1024;
+      sa.n_tiles = (uint32_t)ceil_div(c.n, C::kTile);
+      const uint32_t per = (uint32_t)kSMs / (uint32_t)n_arrays;
+      launch_pdl(msd::scatter_kernel<C>, dim3(sa.n_tiles < per ? sa.n_tiles : per, n_arrays), C::kThreads, C::kSmem, st, sa);
+    } else {
+      using C = msd::ScatterCfg2x512;
+      sa.n_tiles = (uint32_t)ceil_div(c.n, C::kTile);
+      const uint32_t per = 2u * (uint32_t)kSMs / (uint32_t)n_arrays;
+      launch_pdl(msd::scatter_kernel<C>, dim3(sa.n_tiles < per ? sa.n_tiles : per, n_arrays), C::kThreads, C::kSmem, st, sa);
+    }
     BITS_LAUNCH_CHECK();
   }
   {
@@ -1401,6 +1413,7 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "mc_bin_variant")) { if (value < 0 || value > 3) return BITS_ERR_FLAGS; g_opt.mc_bin_variant = value; return BITS_OK; }
   if (!strcmp(name, "mc_gather_group")) { if (value < -1 || value > 5) return BITS_ERR_FLAGS; g_opt.mc_gather_group = value; return BITS_OK; }
   if (!strcmp(name, "msd_pack")) { if (value < 0 || value > msd::kBucketCap) return BITS_ERR_FLAGS; g_opt.msd_pack = value; return BITS_OK; }
+  if (!strcmp(name, "msd_scatter_shape")) { if (value < 0 || value > 1) return BITS_ERR_FLAGS; g_opt.msd_scatter_shape = value; return BITS_OK; }
   if (!strcmp(name, "count_binned")) { if (value < -1 || value > 1) return BITS_ERR_FLAGS; g_opt.count_binned = value; return BITS_OK; }
   if (!strcmp(name, "mc_shift_bias")) { if (value < 0 || value > 8) return BITS_ERR_FLAGS; g_opt.mc_shift_bias = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }

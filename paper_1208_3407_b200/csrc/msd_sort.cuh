@@ -33,11 +33,8 @@ constexpr int kBinBits = 12;
 constexpr int kBins = 1 << kBinBits;          // 4096
 constexpr int kBinShift = 32 - kBinBits;
 
-// scatter: 1024 threads x 16 keys, one block per SM (two 64 KB key buffers + 32 KB of counters)
-constexpr int kScThreads = 1024;
+// scatter: 16 keys per thread; the block shape is a template configuration (ScatterCfg below)
 constexpr int kScKpt = 16;
-constexpr int kScTile = kScThreads * kScKpt;  // 16384 keys
-constexpr size_t kScSmem = (size_t)(2 * (kScTile + 4) + 2 * kBins) * sizeof(uint32_t);
 
 // bucket sort: 512 threads x 16 keys, two blocks per SM
 constexpr int kBkThreads = 512;
@@ -277,72 +274,97 @@ struct ScatterArr {
 };
 struct ScatterArgs { ScatterArr arr[2]; uint32_t n; uint32_t n_tiles; };
 
-__global__ void __launch_bounds__(kScThreads, 1) scatter_kernel(ScatterArgs a) {
-  constexpr int kPer = kBins / kScThreads;
-  static_assert(kScTile <= 65536 && kPer == 4, "");
+// Shape: kT threads x kScKpt keys per tile, kB resident blocks per SM (1,024 x 1: 16,384-key tiles, longer runs per bin;
+// 512 x 2: 8,192-key tiles, two blocks hide each other's barriers).
+template <int kT, int kB>
+struct ScatterCfg {
+  static constexpr int kThreads = kT, kBlocksPerSm = kB;
+  static constexpr int kTile = kT * kScKpt;
+  static constexpr size_t kSmem = (size_t)(2 * (kTile + 4) + 2 * kBins) * sizeof(uint32_t);
+};
+
+template <class C>
+__global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) scatter_kernel(ScatterArgs a) {
+  constexpr int kThreads = C::kThreads, kTile = C::kTile;
+  constexpr int kPer = kBins / kThreads;        // bins per thread: 4 or 8
+  static_assert(kTile <= 65536 && kPer % 4 == 0, "");
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  uint32_t* s_buf = reinterpret_cast<uint32_t*>(smem_raw);              // [2][kScTile + 4]
-  uint32_t* s_cnt = s_buf + 2 * (kScTile + 4);                          // [kBins] counts, then local bases
+  uint32_t* s_buf = reinterpret_cast<uint32_t*>(smem_raw);              // [2][kTile + 4]
+  uint32_t* s_cnt = s_buf + 2 * (kTile + 4);                            // [kBins] counts, then local bases
   uint32_t* s_delta = s_cnt + kBins;                                    // [kBins] global dst - local base
   __shared__ uint32_t s_w[32];
   const ScatterArr A = blockIdx.y ? a.arr[1] : a.arr[0];
   grid_dependency_wait();
   if (*A.flag) return;
   const int tid = threadIdx.x;
-  const uint32_t mis = misalign_words(A.src);   // tiles start at multiples of kScTile keys: same misalignment
-  reinterpret_cast<uint4*>(s_cnt)[tid] = make_uint4(0, 0, 0, 0);
+  const uint32_t mis = misalign_words(A.src);   // tiles start at multiples of kTile keys: same misalignment
+#pragma unroll
+  for (int q = 0; q < kPer / 4; ++q) reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + q] = make_uint4(0, 0, 0, 0);
   uint32_t tile = blockIdx.x;
   if (tile < a.n_tiles)
-    prefetch_keys<kScThreads>(s_buf + mis, A.src + (size_t)tile * kScTile, min((uint32_t)kScTile, a.n - tile * (uint32_t)kScTile));
+    prefetch_keys<kThreads>(s_buf + mis, A.src + (size_t)tile * kTile, min((uint32_t)kTile, a.n - tile * (uint32_t)kTile));
   for (int it = 0; tile < a.n_tiles; tile += gridDim.x, ++it) {
-    uint32_t* buf = s_buf + (it & 1) * (kScTile + 4) + mis;
+    uint32_t* buf = s_buf + (it & 1) * (kTile + 4) + mis;
     cp_async_wait_all();
     __syncthreads();          // this tile's keys are here; everyone is done with the other buffer
     const uint32_t next = tile + gridDim.x;
     if (next < a.n_tiles)
-      prefetch_keys<kScThreads>(s_buf + ((it + 1) & 1) * (kScTile + 4) + mis, A.src + (size_t)next * kScTile,
-                                min((uint32_t)kScTile, a.n - next * (uint32_t)kScTile));
-    const uint32_t count = min((uint32_t)kScTile, a.n - tile * (uint32_t)kScTile);
-    const bool full = count == (uint32_t)kScTile;
+      prefetch_keys<kThreads>(s_buf + ((it + 1) & 1) * (kTile + 4) + mis, A.src + (size_t)next * kTile,
+                              min((uint32_t)kTile, a.n - next * (uint32_t)kTile));
+    const uint32_t count = min((uint32_t)kTile, a.n - tile * (uint32_t)kTile);
+    const bool full = count == (uint32_t)kTile;
     uint32_t key[kScKpt], r[kScKpt];
 #pragma unroll
     for (int j = 0; j < kScKpt; ++j) {
-      const uint32_t i = tid + j * kScThreads;
+      const uint32_t i = tid + j * kThreads;
       if (full || i < count) { key[j] = buf[i]; r[j] = atomicAdd(&s_cnt[key[j] >> kBinShift], 1u); }
     }
     __syncthreads();
     // exclusive scan of the bin counts; one global reservation per non-empty (tile, bin)
     uint32_t c[kPer], ga[kPer], lb[kPer];
     {
-      const uint4 v4 = reinterpret_cast<const uint4*>(s_cnt)[tid];
-      c[0] = v4.x; c[1] = v4.y; c[2] = v4.z; c[3] = v4.w;
-      uint32_t run = block_excl_scan<kScThreads>(c[0] + c[1] + c[2] + c[3], s_w);
+      uint32_t sum = 0;
+#pragma unroll
+      for (int q = 0; q < kPer / 4; ++q) {
+        const uint4 v4 = reinterpret_cast<const uint4*>(s_cnt)[(kPer / 4) * tid + q];
+        c[4 * q] = v4.x; c[4 * q + 1] = v4.y; c[4 * q + 2] = v4.z; c[4 * q + 3] = v4.w;
+        sum += v4.x + v4.y + v4.z + v4.w;
+      }
+      uint32_t run = block_excl_scan<kThreads>(sum, s_w);
 #pragma unroll
       for (int j = 0; j < kPer; ++j) {
         lb[j] = run;
         ga[j] = c[j] ? atomicAdd(&A.bin_cursor[tid * kPer + j], c[j]) : 0u;
         run += c[j];
       }
-      reinterpret_cast<uint4*>(s_cnt)[tid] = make_uint4(lb[0], lb[1], lb[2], lb[3]);
+#pragma unroll
+      for (int q = 0; q < kPer / 4; ++q)
+        reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + q] = make_uint4(lb[4 * q], lb[4 * q + 1], lb[4 * q + 2], lb[4 * q + 3]);
     }
     __syncthreads();
     // stage in bin order, in place (every key of the tile is in a register by now)
 #pragma unroll
     for (int j = 0; j < kScKpt; ++j) {
-      const uint32_t i = tid + j * kScThreads;
+      const uint32_t i = tid + j * kThreads;
       if (full || i < count) buf[s_cnt[key[j] >> kBinShift] + r[j]] = key[j];
     }
-    reinterpret_cast<uint4*>(s_delta)[tid] = make_uint4(ga[0] - lb[0], ga[1] - lb[1], ga[2] - lb[2], ga[3] - lb[3]);
+#pragma unroll
+    for (int q = 0; q < kPer / 4; ++q)
+      reinterpret_cast<uint4*>(s_delta)[(kPer / 4) * tid + q] =
+          make_uint4(ga[4 * q] - lb[4 * q], ga[4 * q + 1] - lb[4 * q + 1], ga[4 * q + 2] - lb[4 * q + 2], ga[4 * q + 3] - lb[4 * q + 3]);
     __syncthreads();
-    reinterpret_cast<uint4*>(s_cnt)[tid] = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int q = 0; q < kPer / 4; ++q) reinterpret_cast<uint4*>(s_cnt)[(kPer / 4) * tid + q] = make_uint4(0, 0, 0, 0);
     uint32_t* __restrict__ dst = A.dst;
 #pragma unroll
     for (int j = 0; j < kScKpt; ++j) {
-      const uint32_t i = tid + j * kScThreads;
+      const uint32_t i = tid + j * kThreads;
       if (full || i < count) { const uint32_t k = buf[i]; dst[s_delta[k >> kBinShift] + i] = k; }
     }
   }
 }
+using ScatterCfg1x1024 = ScatterCfg<1024, 1>;
+using ScatterCfg2x512 = ScatterCfg<512, 2>;
 
 // ---------------------------------------------------------------------------------------------
 // 4. per-bucket sort in shared memory.  Persistent blocks: grid = (blocks, arrays); block b takes
