@@ -48,7 +48,7 @@ struct Plan {                        // what the MSD sort of B left behind (devi
   const uint32_t* bucket_lo;         // [n_buckets + 1] first bin of each bucket
   const uint32_t* bucket_start;      // [n_buckets + 1] where each bucket's keys start in B_S
   const uint32_t* n_buckets;         // [1]
-  const uint32_t* end_cursor;        // [kBins] #{ends < (bin + 1) << 20} (the scatter pass leaves its cursors there)
+  const uint32_t* end_prefix;        // [kBins] #{ends < bin << 20} (the exclusive prefix of the ends' bin histogram, from the plan)
 };
 
 struct Lists {                       // the queries in bucket order (workspace)
@@ -259,8 +259,8 @@ __device__ __forceinline__ Bucket load_bucket(const SearchArgs& a, uint32_t item
   const uint32_t lo_bin = a.p.bucket_lo[d], hi_bin = a.p.bucket_lo[d + 1];
   b.base_s = a.p.bucket_start[d];
   b.ns = a.p.bucket_start[d + 1] - b.base_s;           // <= kCapS (else the sort's flag is up)
-  b.e0 = lo_bin ? a.p.end_cursor[lo_bin - 1] : 0u;
-  b.ne = (hi_bin ? a.p.end_cursor[hi_bin - 1] : 0u) - b.e0;
+  b.e0 = a.p.end_prefix[lo_bin];
+  b.ne = (hi_bin < (uint32_t)msd::kBins ? a.p.end_prefix[hi_bin] : a.n_b) - b.e0;
   b.lo = lo_bin << msd::kBinShift;
   const uint32_t span_bins = hi_bin - lo_bin;          // the bucket covers span_bins << 20 coordinates
   const uint32_t bits = msd::kBinShift + (span_bins > 1u ? 32u - __clz(span_bins - 1u) : 0u);

@@ -139,7 +139,8 @@ struct SortCtx {
   uint32_t* bucket_start[2] = {nullptr, nullptr};   // uint32[kBins + 1]
   uint32_t* n_buckets = nullptr;                    // uint32[2]
   uint32_t* msd_flag = nullptr;                     // uint32[2]
-  uint16_t* bucket_of_bin = nullptr;                // uint16[kBins] bucket of array 0 that holds each bin (binned_count.cuh)
+  uint16_t* bucket_of_bin[2] = {nullptr, nullptr};  // uint16[kBins] the bucket that holds each bin
+  uint32_t* bucket_cursor[2] = {nullptr, nullptr};  // uint32[kBins] reservation cursors of the scatter pass
   uint32_t* bucket_lo = nullptr;                    // uint32[kBins + 1] first bin of each bucket of array 0
   size_t zero_bytes = 0;                            // from hist[0][0]: digit histograms, tickets, bin histograms, bucket counts, flags, status words
   void carve(Carver& c, uint64_t n_keys, bool with_index) {
@@ -162,7 +163,10 @@ struct SortCtx {
       bin_cursor[a] = c.take<uint32_t>(msd::kBins);
       bucket_start[a] = c.take<uint32_t>(msd::kBins + 4);
     }
-    bucket_of_bin = c.take<uint16_t>(msd::kBins);
+    for (int a = 0; a < 2; ++a) {
+      bucket_of_bin[a] = c.take<uint16_t>(msd::kBins);
+      bucket_cursor[a] = c.take<uint32_t>(msd::kBins);
+    }
     bucket_lo = c.take<uint32_t>(msd::kBins + 4);
     shift = index_shift_for(n_keys);
     if (with_index)
@@ -444,7 +448,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     for (int a = 0; a < 2; ++a) {
       pa.p[a].hist = c.bin_hist[a]; pa.p[a].bin_cursor = c.bin_cursor[a]; pa.p[a].bucket_start = c.bucket_start[a];
       pa.p[a].n_buckets = c.n_buckets + a; pa.p[a].flag = c.msd_flag + a; pa.p[a].lsd_hist = c.hist[0][a]; pa.p[a].lsd_ticket = c.ticket + 4 * a;
-      pa.p[a].bucket_of_bin = a == 0 ? c.bucket_of_bin : nullptr; pa.p[a].bucket_lo = a == 0 ? c.bucket_lo : nullptr;
+      pa.p[a].bucket_of_bin = c.bucket_of_bin[a]; pa.p[a].bucket_cursor = c.bucket_cursor[a]; pa.p[a].bucket_lo = a == 0 ? c.bucket_lo : nullptr;
     }
     // fuller buckets pay once there are enough of them to fill the GPU either way (config 2, 10^6 keys: 0.089 ms per
     // call with the prefix rule, 0.103 ms packed; config 4, 10^7 keys: bucket sort 146 us against 124 us)
@@ -457,7 +461,7 @@ static int sort_arrays(const SortCtx& c, const uint32_t* src0, const uint32_t* s
     msd::ScatterArgs sa;
     for (int a = 0; a < 2; ++a) {
       const int aa = a < n_arrays ? a : 0;
-      sa.arr[a].src = p.src[aa]; sa.arr[a].dst = p.x[aa]; sa.arr[a].bin_cursor = c.bin_cursor[aa]; sa.arr[a].flag = c.msd_flag + aa;
+      sa.arr[a].src = p.src[aa]; sa.arr[a].dst = p.x[aa]; sa.arr[a].bucket_of_bin = c.bucket_of_bin[aa]; sa.arr[a].bucket_cursor = c.bucket_cursor[aa]; sa.arr[a].flag = c.msd_flag + aa;
     }
     sa.n = c.n;
     ProfScope prof(kClsScatter, st);
@@ -587,8 +591,8 @@ static int launch_binned_count(const uint32_t* a_start, const uint32_t* a_end, u
     if (device >= 0 && device < 64) configured[device].store(1, std::memory_order_release);
   }
   qb::Plan p;
-  p.flag = L.b.msd_flag; p.bucket_of_bin = L.b.bucket_of_bin; p.bucket_lo = L.b.bucket_lo; p.bucket_start = L.b.bucket_start[0];
-  p.n_buckets = L.b.n_buckets; p.end_cursor = L.b.bin_cursor[1];
+  p.flag = L.b.msd_flag; p.bucket_of_bin = L.b.bucket_of_bin[0]; p.bucket_lo = L.b.bucket_lo; p.bucket_start = L.b.bucket_start[0];
+  p.n_buckets = L.b.n_buckets; p.end_prefix = L.b.bin_cursor[1];
   const uint32_t n_tiles = (uint32_t)ceil_div(n_a, (uint64_t)qb::kScTile);
   {
     ProfScope prof(kClsQueryScatter, st);

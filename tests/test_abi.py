@@ -47,7 +47,10 @@ def test_workspace_sizes():
     assert big % 256 == 0
     mc_a = w(bits.FN_MC_ROUNDS, 10_000, 1_000_000, 24, bits.PERMUTE_A)
     mc_b = w(bits.FN_MC_ROUNDS, 10_000, 1_000_000, 24, bits.PERMUTE_B)
-    assert mc_b > mc_a > w(bits.FN_COUNT, 10_000, 1_000_000)
+    assert mc_b > mc_a > w(bits.FN_SORT, 0, 1_000_000)
+    # the count workspaces also hold the queries in bucket order (12 bytes per query with per-interval counts, 8 without)
+    assert w(bits.FN_COUNT_PER_INTERVAL, 1_000_000, 1_000_000) - w(bits.FN_COUNT, 1_000_000, 1_000_000) >= 4 * 1_000_000 - 4096
+    assert w(bits.FN_COUNT, 1_000_000, 1_000_000) - w(bits.FN_COUNT, 0, 1_000_000) >= 8 * 1_000_000
     assert w(bits.FN_MC_ROUNDS, 0, 0, 1, 0) > 0
     assert bits.host_staging_bytes(bits.FN_MC_ROUNDS, 1000, 1000, 100) >= 4 * 4 * 1000 + 8 * 100
 
@@ -135,7 +138,7 @@ def test_new_entry_points_reject_bad_arguments_on_the_host():
     # workspace missing
     assert L.bits_decide(p, p, 1, p, p, 1, 0, 0, 0, p, 0) == 5
     assert L.bits_enumerate(p, p, 1, p, p, 1, 0, 0, 0, 0, 0, 0, C.addressof(tot), 0) == 5
-    assert bits.workspace_bytes(bits.FN_ENUMERATE, 1000, 1000) > bits.workspace_bytes(bits.FN_COUNT, 1000, 1000)
+    assert bits.workspace_bytes(bits.FN_ENUMERATE, 1000, 1000) > bits.workspace_bytes(bits.FN_SORT, 0, 1000) + 1000 * 24
     off = C.c_size_t(0)
     assert L.bits_workspace_sorted_offset(bits.FN_COUNT, 10, 1000, 0, 0, 1, C.addressof(off)) == 0 and off.value > 0
     assert L.bits_workspace_sorted_offset(bits.FN_SORT, 10, 1000, 0, 0, 0, C.addressof(off)) == 6
