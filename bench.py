@@ -660,6 +660,17 @@ def run_b200(args):
         line["cpu_baseline"] = {"value": rps, "unit": "rounds/s", "cores": 1, "kind": "oracle",
                                 "sample": oracle_sample_text(n_cpu, w), "observed_count_s": t_obs,
                                 "host_cores": os.cpu_count()}
+        # the oracle on the other configs: counting configs in full, config 3 on 100 of its rounds
+        import oracle
+        other = {}
+        for k in (2, 4):
+            wk = W.make_config(k)
+            t0 = time.perf_counter(); oracle.count_per_interval(wk.a_start, wk.a_end, wk.b_start, wk.b_end); dt = time.perf_counter() - t0
+            other[wk.name] = {"seconds": dt, "intervals_searched_per_s": wk.n_a / dt, "sample": "the whole call: std::sort of both key arrays + one ICOUNT per query"}
+        w3 = W.make_config(3)
+        rps3, _, _ = oracle_marginal_rounds_per_s(w3, 0, 0, 100)
+        other[w3.name] = {"rounds_per_s": rps3, "intervals_searched_per_s": rps3 * w3.n_a, "sample": "100 of its 10,000 rounds (marginal cost per round)"}
+        line["cpu_baseline"]["other_configs"] = other
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

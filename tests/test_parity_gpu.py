@@ -890,3 +890,23 @@ def test_launches_are_counted():
     bits.count(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end))
     sync()
     assert bits.launch_count() >= before + 7     # histogram + 4 passes + index + count
+
+
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two CUDA devices")
+def test_second_device_gets_its_own_kernel_attributes():
+    """cudaFuncSetAttribute applies per device: the kernels that need more than 48 KB of shared memory must be
+    configured on every device the library is used on (round 1 cached the opt-in process-wide)."""
+    w = W.make_config(5, scale=0.02)
+    want = None
+    for d in (0, 1):
+        with torch.cuda.device(d):
+            t = [torch.from_numpy(np.ascontiguousarray(x, dtype=np.uint32).view(np.int32)).to(f"cuda:{d}")
+                 for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+            obs, rc = bits.mc_rounds(*t, w.chrom_offsets, 1, 3, 0, 4)
+            counts, total = bits.count_per_interval(*t)
+            torch.cuda.synchronize(d)
+            got = (int(host_u64(obs)[0]), host_u64(rc).tolist(), int(host_u64(total)[0]))
+        if want is None:
+            o_obs, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 3, 0, 4)
+            want = (o_obs, o_rc.tolist(), o_obs)
+        assert got == want
