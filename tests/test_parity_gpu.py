@@ -81,6 +81,24 @@ def test_sort_lsd_only(n):
         bits.set_option("sort_msd", 1)
 
 
+@pytest.mark.parametrize("pack", [7168, 8192, 3000, 0])
+def test_sort_large_sets_with_packed_buckets(pack):
+    """Sorts of at least 4M keys pack consecutive bins greedily into buckets (msd_pack): uniform keys over the genome's
+    range, and keys in clusters (uneven bins: some buckets hold one bin, some dozens, some bins overflow a bucket)."""
+    rng = np.random.default_rng(pack + 3)
+    G = 3_564_000_011
+    uniform = rng.integers(0, G, 4_500_001, dtype=np.uint64)
+    centres = rng.integers(0, G, 3000, dtype=np.uint64)
+    clustered = (centres[rng.integers(0, 3000, 5_000_003)] + rng.integers(0, 400_000, 5_000_003, dtype=np.uint64)) % np.uint64(2**32)
+    bits.set_option("msd_pack", pack)
+    try:
+        for k in (uniform, clustered, np.concatenate([uniform[:2_500_000], clustered[:2_500_000]])):
+            k = k.astype(np.uint32)
+            assert np.array_equal(host_u32(bits.sort_u32(dev(k))), oracle.sort_u32(k))
+    finally:
+        bits.set_option("msd_pack", 7168)
+
+
 def test_sort_repeated_calls_share_workspace():
     rng = np.random.default_rng(17)
     n = 50_000
@@ -170,6 +188,16 @@ def test_count_binned_queries_special_cases():
     # (3) 40,000 queries inside one bucket (ten work items), the rest spread out
     qs = 1_000_000_000 + rng.integers(0, 500_000, 40_000)
     check_counts(np.concatenate([qs, a_s[:5000]]), np.concatenate([qs + rng.integers(0, 300, 40_000), a_e[:5000]]), b_s, b_e)
+    # (5) at a size where the library itself picks the binned design and packs buckets: 4.2M intervals, half of them in
+    # clusters, against 1.5M queries of which a million sit in a few dozen buckets (work items of 16,384 queries, several
+    # per bucket, answered in steps) and 20,000 are longer than a bucket
+    n_b5 = 4_200_000
+    u = rng.integers(0, G, n_b5 // 2)
+    c5 = rng.integers(0, G, 2000)[rng.integers(0, 2000, n_b5 - n_b5 // 2)] + rng.integers(0, 300_000, n_b5 - n_b5 // 2)
+    b5_s = np.concatenate([u, c5]); b5_e = b5_s + rng.integers(0, 20_000, n_b5)
+    q5 = np.concatenate([rng.integers(0, G, 480_000), 1_700_000_000 + rng.integers(0, 40_000_000, 1_000_000), rng.integers(0, G, 20_000)])
+    q5_e = q5 + np.concatenate([rng.integers(0, 3000, 1_480_000), rng.integers(2**20, 2**24, 20_000)])
+    check_counts(q5, q5_e, b5_s, b5_e)
     # (4) 60,000 starts inside one bin: the MSD sort raises its flag, the LSD sort and the index path take over
     cs = 123_456_789 + rng.integers(0, 200_000, 60_000)
     b4_s, b4_e = np.concatenate([b_s[:50_000], cs]), np.concatenate([b_e[:50_000], cs + rng.integers(0, 100, 60_000)])
