@@ -370,6 +370,24 @@ def secondary_workloads(device, peak_gbs):
     out["cfg3_mc_permuteA_1e4x1M"] = {"mc_rounds_per_s": w.n_rounds / (med * 1e-3),
                                       "intervals_searched_per_s": w.n_rounds * w.n_a / (med * 1e-3),
                                       "ms_median": med, "ms_min": mn}
+    # config 1 (1,000 x 1,000, one chromosome): Monte Carlo rounds of a set that fits one block's shared memory
+    # (mc_small.cuh: one block per round), beside the two-launch path on the same rounds
+    w = W.make_config(1)
+    d1 = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    R1 = 10_000
+    ws1 = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, w.n_a, w.n_b, 1, 1), dtype=torch.uint8, device=device)
+    rc1 = torch.empty(R1, dtype=torch.int64, device=device)
+    run1 = lambda: bits.mc_rounds(*d1, w.chrom_offsets, 1, w.mc_seed, 0, R1, workspace=ws1, observed_out=obs, round_counts_out=rc1)
+    med, mn = time_device(run1, 5)
+    ref1 = rc1.clone()
+    bits.set_option("mc_small", 0)
+    try:
+        med2, _ = time_device(run1, 3, warmup=1)
+    finally:
+        bits.set_option("mc_small", 1)
+    out["cfg1_tiny_permuteB_10000_rounds"] = {"mc_rounds_per_s": R1 / (med * 1e-3), "ms_median": med, "ms_min": mn,
+                                              "two_launch_path_rounds_per_s": R1 / (med2 * 1e-3),
+                                              "same_counts_as_two_launch_path": bool(torch.equal(ref1, rc1))}
     # config 2: 1e6 x 1e6 count
     w = W.make_config(2)
     d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]

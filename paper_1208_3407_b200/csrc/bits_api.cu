@@ -13,6 +13,7 @@
 #include "radix_sort.cuh"
 #include "msd_sort.cuh"
 #include "mc_tile.cuh"
+#include "mc_small.cuh"
 #include "search.cuh"
 #include "enumerate.cuh"
 #include "screen.cuh"
@@ -37,6 +38,7 @@ struct Options {
   int64_t msd_pack = 7168;         // MSD sort plan: 0 = buckets by the prefix / target rule, n = consecutive bins packed greedily up to n keys (measured on config 4: 0 -> 146 us, 8192 -> 134, 7168 -> 124 for the bucket sort)
   int64_t msd_scatter_shape = 0;   // MSD scatter pass: 0 = one 1,024-thread block per SM and 16,384-key tiles, 1 = two 512-thread blocks and 8,192-key tiles
   int64_t count_binned = -1;       // count path: 1 = queries binned by B's buckets and searched out of shared memory (binned_count.cuh), 0 = bucket index + count_kernel, -1 = by size
+  int64_t mc_small = 1;            // PERMUTE_B rounds of a set that fits one block's shared memory: 1 = one block per round (mc_small.cuh)
   int64_t mc_shift_bias = 0;       // PERMUTE_B fused rounds: added to the bin width (log2) the host picked; > 0 overflows bins on purpose (tests)
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
 };
@@ -399,6 +401,8 @@ static int msd_configure() {
       e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024::kSmem);
     if (e4 == cudaSuccess)
       e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024L::kSmem);
+    if (e4 == cudaSuccess)
+      e4 = cudaFuncSetAttribute(mcs::mc_small_b_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mcs::kSmem);
     if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { (void)cudaGetLastError(); return BITS_ERR_CUDA; }
     if (tracked) done_on[device].store(1, std::memory_order_release);
   }
@@ -810,6 +814,22 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       BITS_LAUNCH_CHECK();
       done += chunk;
     }
+    return BITS_OK;
+  }
+  if (g_opt.mc_small != 0 && n_b <= (uint64_t)mcs::kMaxKeys && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0) {
+    // a set that fits one block's shared memory: one block per round, the grid strides over the rounds (mc_small.cuh)
+    BITS_TRY(msd_configure());
+    mcs::SmallArgs m;
+    m.spans = L.spans; m.n = (uint32_t)n_b; m.tag = 1u; m.round0 = round_begin; m.n_rounds = n_rounds;
+    const uint32_t g_bits = 32u - (uint32_t)__builtin_clz((off[n_chrom] - 1u) | 1u);      // bits of the largest coordinate
+    m.sshift = g_bits > (uint32_t)mcs::Cfg::kSubBits ? g_bits - (uint32_t)mcs::Cfg::kSubBits : 0u;
+    m.key = key; m.chrom = chrom; m.q_sorted[0] = q_end_sorted; m.q_sorted[1] = q_start_sorted; m.n_q = (uint32_t)n_a;
+    m.dst[0] = L.b.buf[0][0]; m.dst[1] = L.b.buf[1][0];
+    m.round_counts = reinterpret_cast<unsigned long long*>(round_counts_out);
+    const uint32_t blocks = (uint32_t)mcs::Cfg::kBlocksPerSm * (uint32_t)kSMs;
+    ProfScope prof(kClsBucketSortSearch, st);
+    mcs::mc_small_b_kernel<<<n_rounds < blocks ? n_rounds : blocks, mcs::Cfg::kThreads, mcs::kSmem, st>>>(m);
+    BITS_LAUNCH_CHECK();
     return BITS_OK;
   }
   const bool msd_on = g_opt.sort_msd != 0;
@@ -1419,6 +1439,7 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "msd_pack")) { if (value < 0 || value > msd::kBucketCap) return BITS_ERR_FLAGS; g_opt.msd_pack = value; return BITS_OK; }
   if (!strcmp(name, "msd_scatter_shape")) { if (value < 0 || value > 1) return BITS_ERR_FLAGS; g_opt.msd_scatter_shape = value; return BITS_OK; }
   if (!strcmp(name, "count_binned")) { if (value < -1 || value > 1) return BITS_ERR_FLAGS; g_opt.count_binned = value; return BITS_OK; }
+  if (!strcmp(name, "mc_small")) { g_opt.mc_small = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_shift_bias")) { if (value < 0 || value > 8) return BITS_ERR_FLAGS; g_opt.mc_shift_bias = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }

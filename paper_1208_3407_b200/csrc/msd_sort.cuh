@@ -159,7 +159,7 @@ struct PlanArgs {
 __global__ void __launch_bounds__(1024) plan_kernel(PlanArgs a) {
   static_assert(kBins == 4096, "4 bins per thread");
   __shared__ uint32_t s_w[32];
-  __shared__ uint32_t s_raw[kBins + 1];
+  __shared__ uint32_t s_raw[kBins + kBins / 32 + 2];
   __shared__ uint32_t s_start[kBins + 1];
   const PlanArr P = blockIdx.x ? a.p[1] : a.p[0];
   const int t = threadIdx.x;
@@ -190,23 +190,28 @@ __global__ void __launch_bounds__(1024) plan_kernel(PlanArgs a) {
     // greedy packing: a bucket takes consecutive bins while it stays within pack_cap keys (fuller buckets than the
     // rule below: fewer of them, fewer fixed costs per bucket).  Sequential inside chunks of 64 bins, one thread per
     // chunk; a chunk boundary always starts a bucket.
-    __shared__ uint8_t s_first[kBins];
+    // (prefixes are read with a stride of 64 words by the chunk threads: one pad word per 32 keeps them off one bank;
+    // a chunk's 64 "starts a bucket" flags travel as one 64-bit mask)
+    uint32_t* s_pad = s_raw;                              // [kBins + kBins / 32 + 2]
+    __shared__ unsigned long long s_mask[kBins / 64];
+    auto pad = [](uint32_t i) { return i + (i >> 5); };
 #pragma unroll
-    for (int j = 0; j < 4; ++j) s_raw[4 * t + j] = ex[j];
-    if (t == 0) s_raw[kBins] = total;
+    for (int j = 0; j < 4; ++j) s_pad[pad(4 * t + j)] = ex[j];
+    if (t == 0) s_pad[pad(kBins)] = total;
     __syncthreads();
     if (t < kBins / 64) {
-      uint32_t from = s_raw[64 * t];
-      s_first[64 * t] = 1;
+      uint32_t from = s_pad[pad(64 * t)];
+      unsigned long long mask = 1ull;
       for (int b = 64 * t + 1; b < 64 * t + 64; ++b) {
-        const bool brk = s_raw[b + 1] - from > a.pack_cap;
-        if (brk) from = s_raw[b];
-        s_first[b] = brk ? 1 : 0;
+        const bool brk = s_pad[pad(b + 1)] - from > a.pack_cap;
+        if (brk) { from = s_pad[pad(b)]; mask |= 1ull << (b & 63); }
       }
+      s_mask[t] = mask;
     }
     __syncthreads();
+    const unsigned long long m = s_mask[t >> 4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) { first[j] = s_first[4 * t + j]; fex[j] = nf; nf += first[j]; }
+    for (int j = 0; j < 4; ++j) { first[j] = (uint32_t)(m >> ((4 * t + j) & 63)) & 1u; fex[j] = nf; nf += first[j]; }
   } else {
 #pragma unroll
     for (int j = 0; j < 4; ++j) s_raw[4 * t + j + 1] = ex[j] / target;

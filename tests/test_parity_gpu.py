@@ -667,6 +667,7 @@ def test_mc_permute_b_kernel_shapes(tile_variant, bin_variant):
     """Every shape of the two fused kernels gives the oracle's integers (config 5 at 3 % and config 1)."""
     bits.set_option("mc_tile_variant", tile_variant)
     bits.set_option("mc_bin_variant", bin_variant)
+    bits.set_option("mc_small", 0)                   # (config 1 would otherwise take the one-block-per-round kernel)
     try:
         for k, scale, rounds in ((5, 0.03, 3), (1, 1.0, 4)):
             w = W.make_config(k, scale=scale)
@@ -674,6 +675,39 @@ def test_mc_permute_b_kernel_shapes(tile_variant, bin_variant):
     finally:
         bits.set_option("mc_tile_variant", 2)
         bits.set_option("mc_bin_variant", 0)
+        bits.set_option("mc_small", 1)
+
+
+def test_mc_permute_b_small_sets_one_block_per_round():
+    """Sets of at most 8,188 intervals: one block does a whole round in shared memory and the grid strides over the
+    rounds (mc_small.cuh).  Sizes around the limit, more rounds than blocks, tiny genomes with heavy ties, a query
+    beyond the genome's end, and the same rounds by the two-launch path."""
+    rng = np.random.default_rng(55)
+    w = W.make_config(1)
+    _mc_b_case(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 0, 100, expect_fused=False)
+    _mc_b_case(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 7, 4_294_960_000, 700, expect_fused=False)   # 700 rounds > 296 blocks
+    off = W.genome_offsets(W.GENOME24_LENGTHS)
+    def draw(n, max_len):
+        c = rng.integers(0, 24, n); ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        st = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        return st.astype(np.uint32), (st + ln - 1).astype(np.uint32)
+    a_s, a_e = draw(30_000, 5000)
+    for n_b, fused in ((1, False), (3, False), (8187, False), (8188, False), (8189, True)):
+        b_s, b_e = draw(n_b, 100_000)
+        _mc_b_case(a_s, a_e, b_s, b_e, off, 3, 2, 5, expect_fused=fused if n_b > 8188 else False)
+    off2 = np.array([0, 300, 500], dtype=np.uint32)             # every coordinate hit dozens of times: long tie runs
+    b_s2 = rng.integers(0, 250, 6000).astype(np.uint32); b_e2 = np.minimum(b_s2 + rng.integers(0, 40, 6000), 299).astype(np.uint32)
+    a_s2 = np.array([0, 5, 100, 299, 450, 600_000], dtype=np.uint32); a_e2 = np.array([0, 50, 100, 400, 499, 700_000], dtype=np.uint32)
+    _mc_b_case(a_s2, a_e2, b_s2, b_e2, off2, 9, 0, 6, expect_fused=False)
+    bits.set_option("mc_small", 0)                                # the two-launch path gives the same integers
+    try:
+        obs0, rc0 = bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, 1, 1, 0, 30)
+    finally:
+        bits.set_option("mc_small", 1)
+    obs1, rc1 = bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, 1, 1, 0, 30)
+    sync()
+    assert torch.equal(rc0, rc1) and torch.equal(obs0, obs1)
 
 
 def test_mc_permute_b_redo_path_gives_the_same_counts():
