@@ -388,6 +388,29 @@ def secondary_workloads(device, peak_gbs):
     out["cfg1_tiny_permuteB_10000_rounds"] = {"mc_rounds_per_s": R1 / (med * 1e-3), "ms_median": med, "ms_min": mn,
                                               "two_launch_path_rounds_per_s": R1 / (med2 * 1e-3),
                                               "same_counts_as_two_launch_path": bool(torch.equal(ref1, rc1))}
+    # config 5's recipe at the smaller sizes of the paper's Table 1 (1e5 and 1e6 re-placed intervals):
+    # one round does not fill the GPU there, so several rounds share a launch pair (gridDim.y = rounds)
+    sizes = {}
+    for scale in (0.01, 0.1):
+        ws_ = W.make_config(5, scale=scale)
+        ds = [to_dev(x, device) for x in (ws_.a_start, ws_.a_end, ws_.b_start, ws_.b_end)]
+        Rm = 2000
+        wsp = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, ws_.n_a, ws_.n_b, 24, 1), dtype=torch.uint8, device=device)
+        rcm = torch.empty(Rm, dtype=torch.int64, device=device)
+        runm = lambda: bits.mc_rounds(*ds, ws_.chrom_offsets, 1, ws_.mc_seed, 0, Rm, workspace=wsp, observed_out=obs, round_counts_out=rcm)
+        medm, _ = time_device(runm, 3, warmup=2)
+        refm = rcm.clone()
+        bits.set_option("mc_batch", 0)
+        try:
+            medm0, _ = time_device(runm, 2, warmup=1)
+        finally:
+            bits.set_option("mc_batch", 1)
+        sizes[f"n_b_{ws_.n_b}_n_a_{ws_.n_a}"] = {"mc_rounds_per_s": Rm / (medm * 1e-3), "us_per_round": 1e3 * medm / Rm,
+                                                 "sort_keys_per_s": 2 * ws_.n_b * Rm / (medm * 1e-3),
+                                                 "one_round_per_launch_rounds_per_s": Rm / (medm0 * 1e-3),
+                                                 "same_counts": bool(torch.equal(refm, rcm))}
+        del ds, wsp
+    out["cfg5_recipe_at_table1_sizes_2000_rounds"] = sizes
     # config 2: 1e6 x 1e6 count
     w = W.make_config(2)
     d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]

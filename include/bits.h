@@ -86,6 +86,8 @@ enum {
 /* Bytes of device workspace `fn` needs for these sizes (device-pointer entry points).
  * `which` matters only for BITS_FN_MC_ROUNDS; n_chrom only for MC_ROUNDS and PLACE; for
  * BITS_FN_SORT n_b is the key count (n_a ignored).  Add bits_host_staging_bytes for *_host.
+ * The size is NOT monotone in the set sizes (a small re-placed set gets room for several rounds per
+ * launch): size a workspace that is shared between calls by the maximum over the calls.
  * Returns 0 for an unknown fn. */
 size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which,
                             uint32_t flags);

@@ -38,6 +38,7 @@ struct Options {
   int64_t msd_pack = 7168;         // MSD sort plan: 0 = buckets by the prefix / target rule, n = consecutive bins packed greedily up to n keys (measured on config 4: 0 -> 146 us, 8192 -> 134, 7168 -> 124 for the bucket sort)
   int64_t msd_scatter_shape = 0;   // MSD scatter pass: 0 = one 1,024-thread block per SM and 16,384-key tiles, 1 = two 512-thread blocks and 8,192-key tiles
   int64_t count_binned = -1;       // count path: 1 = queries binned by B's buckets and searched out of shared memory (binned_count.cuh), 0 = bucket index + count_kernel, -1 = by size
+  int64_t mc_batch = 1;            // PERMUTE_B fused rounds of small sets: 1 = several rounds per launch pair (gridDim.y), 0 = one
   int64_t mc_small = 1;            // PERMUTE_B rounds of a set that fits one block's shared memory: 1 = one block per round (mc_small.cuh)
   int64_t mc_shift_bias = 0;       // PERMUTE_B fused rounds: added to the bin width (log2) the host picked; > 0 overflows bins on purpose (tests)
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
@@ -204,6 +205,15 @@ struct Layout {
   uint32_t* cross_keys = nullptr;        // [kMaxBins * kCrossCap]
   uint32_t* qb[2] = {nullptr, nullptr};
   uint32_t* round_flags = nullptr;       // uint32[kFlagChunk]
+  // several fused rounds per launch pair (small re-placed sets): `batch_slots` copies of the per-round buffers,
+  // slot_words 32-bit words apart; null when the set is too large for that to pay
+  uint32_t batch_slots = 1, batch_rows = 0;
+  size_t slot_words = 0;
+  uint2* bt_pairs = nullptr;
+  uint32_t* bt_off = nullptr;
+  uint32_t* bt_cross_cnt[2] = {nullptr, nullptr};
+  uint32_t* bt_cross_keys = nullptr;
+  uint32_t* bt_dst[2] = {nullptr, nullptr};
   // count path with binned queries (binned_count.cuh)
   qb::Lists ql = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // (eight pointers)
   // enumeration (enumerate.cuh)
@@ -218,6 +228,13 @@ struct Layout {
 };
 constexpr uint32_t kFlagChunk = 4096;    // fused rounds are checked for raised flags in chunks of this many
 constexpr uint64_t kFusedMaxKeys = 24u << 20;   // beyond this the bins of the fused path cannot hold the set
+constexpr uint64_t kBatchMaxKeys = 2u << 20;    // re-placed sets up to this size run several rounds per launch pair
+constexpr uint32_t kBatchMaxSlots = 32, kBatchBins = 512;
+static inline uint32_t batch_slots_for(uint64_t n) {
+  if (n <= (uint64_t)mcs::kMaxKeys || n > kBatchMaxKeys) return 1;     // (smaller sets: one block per round, mc_small.cuh)
+  const uint64_t s = (4ull << 20) / n;
+  return (uint32_t)(s < 2 ? 2 : (s > kBatchMaxSlots ? kBatchMaxSlots : s));
+}
 // Tiles are balanced: every block of place_tile_kernel gets the same number of equally sized tiles.
 static inline uint32_t tile_size_for(uint64_t n, uint32_t blocks, uint32_t max_tile) {
   const uint64_t per_block = ceil_div(n, (uint64_t)blocks * max_tile);
@@ -266,6 +283,31 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
           }
           L.cross_keys = c.take<uint32_t>((uint64_t)mct::kMaxBins * mct::kCrossCap);
           L.round_flags = c.take<uint32_t>(kFlagChunk);
+          L.batch_slots = batch_slots_for(n_b);
+          if (L.batch_slots > 1) {
+            // one slot, carved relative to its own start; every slot has the same shape
+            L.batch_rows = (uint32_t)ceil_div(n_b, 4096) + 2;
+            size_t used = 0;
+            auto place = [&](uint64_t bytes) { used = align_up(used, 256); const size_t o = used; used += bytes; return o; };
+            const size_t o_pairs = place(sizeof(uint2) * (align_up(n_b, 4) + 4));
+            const size_t o_off = place(sizeof(uint32_t) * (uint64_t)L.batch_rows * L.tile_stride);
+            size_t o_cc[2], o_dst[2];
+            for (int a = 0; a < 2; ++a) o_cc[a] = place(sizeof(uint32_t) * (mct::kMaxBins + 4));
+            const size_t o_ck = place(sizeof(uint32_t) * (uint64_t)kBatchBins * mct::kCrossCap);
+            for (int a = 0; a < 2; ++a) o_dst[a] = place(sizeof(uint32_t) * align_up(n_b + kPad, 64));
+            const size_t slot_bytes = align_up(used, 256);
+            L.slot_words = slot_bytes / sizeof(uint32_t);
+            char* base = c.take<char>((uint64_t)slot_bytes * L.batch_slots);
+            if (base) {
+              L.bt_pairs = reinterpret_cast<uint2*>(base + o_pairs);
+              L.bt_off = reinterpret_cast<uint32_t*>(base + o_off);
+              for (int a = 0; a < 2; ++a) {
+                L.bt_cross_cnt[a] = reinterpret_cast<uint32_t*>(base + o_cc[a]);
+                L.bt_dst[a] = reinterpret_cast<uint32_t*>(base + o_dst[a]);
+              }
+              L.bt_cross_keys = reinterpret_cast<uint32_t*>(base + o_ck);
+            }
+          }
         }
       }
       break;
@@ -713,15 +755,15 @@ static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* en
 }
 
 template <class C>
-static void launch_place_tile(const mct::PlaceTileArgs& pt, cudaStream_t st) {
+static void launch_place_tile(const mct::PlaceTileArgs& pt, uint32_t rounds, cudaStream_t st) {
   const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
-  launch_pdl(mct::place_tile_kernel<C>, pt.n_tiles < blocks ? pt.n_tiles : blocks, C::kThreads, C::kSmem, st, pt);
+  launch_pdl(mct::place_tile_kernel<C>, dim3(pt.n_tiles < blocks ? pt.n_tiles : blocks, rounds), C::kThreads, C::kSmem, st, pt);
 }
 
 template <class C>
-static void launch_bin_sort(const mct::BinSortArgs& bs, cudaStream_t st) {
+static void launch_bin_sort(const mct::BinSortArgs& bs, uint32_t rounds, cudaStream_t st) {
   const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
-  launch_pdl(mct::bin_sort_search_kernel<C>, bs.n_bins < blocks ? bs.n_bins : blocks, C::kThreads, C::smem_bytes(bs.n_tiles), st, bs);
+  launch_pdl(mct::bin_sort_search_kernel<C>, dim3(bs.n_bins < blocks ? bs.n_bins : blocks, rounds), C::kThreads, C::smem_bytes(bs.n_tiles), st, bs);
 }
 
 static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
@@ -892,6 +934,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
   // span d), every span is shorter than a bin, and few ends fall into the bin after their start's.
   mct::PlaceTileArgs pt;
   mct::BinSortArgs bs;
+  uint32_t rounds_per_launch = 1, batch_tile = 0;
   bool fused_ok = msd_on && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0 && L.pairs != nullptr;
   const int variant = (int)g_opt.mc_bin_variant;
   const int tile_variant = (int)g_opt.mc_tile_variant;
@@ -917,6 +960,27 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     // a small set: narrower bins (finer sub-buckets, more blocks) as long as there are no more bins than blocks
     while (best > 1 && fits(best - 1) && ((G + (1ull << (best - 1)) - 1) >> (best - 1)) <= 2ull * kSMs) --best;
     fused_ok = best >= 0;
+    // A small set does not fill the GPU with one round: several rounds per launch pair (gridDim.y), each in its own
+    // slot of the workspace, and the WIDEST bins that fit (few, full bins per round instead of many nearly empty ones).
+    if (fused_ok && L.batch_slots > 1 && L.bt_pairs && g_opt.mc_batch != 0 && g_opt.mc_shift_bias == 0) {
+      int wide = -1;
+      for (int sh = 31; sh >= 1; --sh)
+        if (fits(sh)) { wide = sh; break; }
+      if (wide >= 0) {
+        const uint64_t nb = (G + (1ull << wide) - 1) >> wide;
+        const uint32_t per = (uint32_t)(nb < 2ull * kSMs ? nb : 2ull * kSMs);
+        uint32_t r = 4u * (uint32_t)kSMs / (per ? per : 1u);           // about two waves of bin blocks per launch
+        if (r > L.batch_slots) r = L.batch_slots;
+        const uint32_t max_tile = tile_variant == 0 ? (uint32_t)mct::TileCfg2x512::kTile
+                                : (tile_variant == 1 ? (uint32_t)mct::TileCfg1x1024::kTile : (uint32_t)mct::TileCfg1x1024L::kTile);
+        const uint32_t blocks_per_round = r ? ((uint32_t)kSMs / r ? (uint32_t)kSMs / r : 1u) : 1u;
+        uint32_t tile = tile_size_for(n_b, blocks_per_round, max_tile);
+        if (tile < 4096u) tile = (uint32_t)(align_up(n_b, 4) < 4096u ? align_up(n_b, 4) : 4096u);
+        if (r >= 2 && nb <= (uint64_t)kBatchBins && ceil_div(n_b, tile) + 1 <= (uint64_t)L.batch_rows) {
+          rounds_per_launch = r; best = wide; batch_tile = tile;
+        }
+      }
+    }
     if (fused_ok && g_opt.mc_shift_bias > 0) {     // tests: wider bins than the margin allows, so that bins overflow on the device
       best += (int)g_opt.mc_shift_bias;
       if (best > mct::kMaxShift) best = mct::kMaxShift;
@@ -926,11 +990,15 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       pt.shift = (uint32_t)best; pt.n_bins = (uint32_t)((G + (1ull << best) - 1) >> best);
       pt.tile = tile_variant == 0 ? tile_size_cfg<mct::TileCfg2x512>(n_b)
                                   : (tile_variant == 1 ? tile_size_cfg<mct::TileCfg1x1024>(n_b) : tile_size_cfg<mct::TileCfg1x1024L>(n_b));
+      const bool batched = rounds_per_launch > 1;
+      if (batched) pt.tile = batch_tile;
       pt.n_tiles = (uint32_t)ceil_div(n_b, pt.tile);
-      pt.pairs = L.pairs; pt.off = L.tile_off; pt.stride = L.tile_stride; pt.cross_keys = L.cross_keys;
-      bs.pairs = L.pairs; bs.off = L.tile_off; bs.stride = L.tile_stride; bs.n_tiles = pt.n_tiles; bs.tile = pt.tile;
-      bs.n = (uint32_t)n_b; bs.shift = pt.shift; bs.n_bins = pt.n_bins; bs.cross_keys = L.cross_keys;
-      bs.dst[0] = L.b.buf[0][0]; bs.dst[1] = L.b.buf[1][0];
+      pt.pairs = batched ? L.bt_pairs : L.pairs; pt.off = batched ? L.bt_off : L.tile_off; pt.stride = L.tile_stride;
+      pt.cross_keys = batched ? L.bt_cross_keys : L.cross_keys;
+      pt.slot_words = bs.slot_words = batched ? (uint32_t)L.slot_words : 0u;
+      bs.pairs = pt.pairs; bs.off = pt.off; bs.stride = L.tile_stride; bs.n_tiles = pt.n_tiles; bs.tile = pt.tile;
+      bs.n = (uint32_t)n_b; bs.shift = pt.shift; bs.n_bins = pt.n_bins; bs.cross_keys = pt.cross_keys;
+      bs.dst[0] = batched ? L.bt_dst[0] : L.b.buf[0][0]; bs.dst[1] = batched ? L.bt_dst[1] : L.b.buf[1][0];
       bs.q_sorted[0] = q_end_sorted; bs.q_sorted[1] = q_start_sorted; bs.qb[0] = L.qb[0]; bs.qb[1] = L.qb[1];
       bs.n_q = (uint32_t)n_a;
       // lanes per gathered segment: the power of two at or above the mean segment length
@@ -948,8 +1016,15 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     return BITS_OK;
   }
   BITS_TRY(msd_configure());
-  BITS_CUDA_TRY(cudaMemsetAsync(L.cross_cnt[0], 0, sizeof(uint32_t) * (mct::kMaxBins + 4), st));
-  BITS_CUDA_TRY(cudaMemsetAsync(L.cross_cnt[1], 0, sizeof(uint32_t) * (mct::kMaxBins + 4), st));
+  const bool batched = rounds_per_launch > 1;
+  uint32_t* const cc[2] = {batched ? L.bt_cross_cnt[0] : L.cross_cnt[0], batched ? L.bt_cross_cnt[1] : L.cross_cnt[1]};
+  if (batched) {     // both hand-over count arrays of every slot (they are neighbours inside a slot)
+    const size_t width = (size_t)(reinterpret_cast<char*>(cc[1]) - reinterpret_cast<char*>(cc[0])) + sizeof(uint32_t) * (mct::kMaxBins + 4);
+    BITS_CUDA_TRY(cudaMemset2DAsync(cc[0], L.slot_words * sizeof(uint32_t), 0, width, L.batch_slots, st));
+  } else {
+    BITS_CUDA_TRY(cudaMemsetAsync(cc[0], 0, sizeof(uint32_t) * (mct::kMaxBins + 4), st));
+    BITS_CUDA_TRY(cudaMemsetAsync(cc[1], 0, sizeof(uint32_t) * (mct::kMaxBins + 4), st));
+  }
   {
     mct::QueryBinsArgs qa;
     qa.q_sorted[0] = q_end_sorted; qa.q_sorted[1] = q_start_sorted; qa.qb[0] = L.qb[0]; qa.qb[1] = L.qb[1];
@@ -958,31 +1033,42 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     BITS_LAUNCH_CHECK();
   }
   std::vector<uint32_t> h_flags;
-  uint32_t n_fused = 0;     // fused rounds launched so far (parity of the hand-over counters)
+  uint32_t n_fused = 0;     // launch pairs so far (parity of the hand-over counters)
+  // flags are read back per chunk of rounds; a chunk is a whole number of launch pairs, so that only the call's last
+  // launch pair can be a partial one (a slot that sat out a pair would miss the clearing of its hand-over counts)
+  const uint32_t flag_chunk = kFlagChunk / rounds_per_launch * rounds_per_launch;
   for (uint32_t done = 0; done < n_rounds;) {
-    const uint32_t chunk = n_rounds - done < kFlagChunk ? n_rounds - done : kFlagChunk;
+    const uint32_t chunk = n_rounds - done < flag_chunk ? n_rounds - done : flag_chunk;
     BITS_CUDA_TRY(cudaMemsetAsync(L.round_flags, 0, sizeof(uint32_t) * chunk, st));
-    for (uint32_t j = 0; j < chunk; ++j, ++n_fused) {
+    for (uint32_t j = 0; j < chunk; ++n_fused) {
       const uint32_t k = done + j;
+      const uint32_t nr = chunk - j < rounds_per_launch ? chunk - j : rounds_per_launch;
       const int par = (int)(n_fused & 1u);
-      pt.round = round_begin + k; pt.flag = L.round_flags + j; pt.cross_cnt = L.cross_cnt[par];
+      pt.round = round_begin + k; pt.flag = L.round_flags + j; pt.cross_cnt = cc[par];
       {
         ProfScope prof(kClsPlaceScatter, st);
-        if (tile_variant == 0) launch_place_tile<mct::TileCfg2x512>(pt, st);
-        else if (tile_variant == 1) launch_place_tile<mct::TileCfg1x1024>(pt, st);
-        else launch_place_tile<mct::TileCfg1x1024L>(pt, st);
+        if (tile_variant == 0) launch_place_tile<mct::TileCfg2x512>(pt, nr, st);
+        else if (tile_variant == 1) launch_place_tile<mct::TileCfg1x1024>(pt, nr, st);
+        else launch_place_tile<mct::TileCfg1x1024L>(pt, nr, st);
         BITS_LAUNCH_CHECK();
       }
-      bs.cross_cnt = L.cross_cnt[par]; bs.cross_cnt_next = L.cross_cnt[par ^ 1]; bs.flag = pt.flag;
+      bs.cross_cnt = cc[par]; bs.cross_cnt_next = cc[par ^ 1]; bs.flag = pt.flag;
       bs.round_total = reinterpret_cast<unsigned long long*>(round_counts_out + k);
       {
         ProfScope prof(kClsBucketSortSearch, st);
-        if (variant == 0) launch_bin_sort<mct::BinCfgWide>(bs, st);
-        else if (variant == 1) launch_bin_sort<mct::BinCfgNarrow>(bs, st);
-        else if (variant == 2) launch_bin_sort<mct::BinCfgSmall>(bs, st);
-        else launch_bin_sort<mct::BinCfgHuge>(bs, st);
+        if (variant == 0) launch_bin_sort<mct::BinCfgWide>(bs, nr, st);
+        else if (variant == 1) launch_bin_sort<mct::BinCfgNarrow>(bs, nr, st);
+        else if (variant == 2) launch_bin_sort<mct::BinCfgSmall>(bs, nr, st);
+        else launch_bin_sort<mct::BinCfgHuge>(bs, nr, st);
         BITS_LAUNCH_CHECK();
       }
+      j += nr;
+    }
+    if (batched && done + chunk == n_rounds) {
+      // B_S and B_E of the call's last round go from their slot to where bits_workspace_sorted_offset points
+      const size_t slot = (size_t)((chunk - 1) % rounds_per_launch) * L.slot_words;
+      for (int a = 0; a < 2; ++a)
+        BITS_CUDA_TRY(cudaMemcpyAsync(L.b.buf[a][0], L.bt_dst[a] + slot, sizeof(uint32_t) * (size_t)n_b, cudaMemcpyDeviceToDevice, st));
     }
     // rounds whose flag was raised are redone by the general path (one synchronisation per chunk)
     h_flags.assign(chunk, 0);
@@ -1439,6 +1525,7 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "msd_pack")) { if (value < 0 || value > msd::kBucketCap) return BITS_ERR_FLAGS; g_opt.msd_pack = value; return BITS_OK; }
   if (!strcmp(name, "msd_scatter_shape")) { if (value < 0 || value > 1) return BITS_ERR_FLAGS; g_opt.msd_scatter_shape = value; return BITS_OK; }
   if (!strcmp(name, "count_binned")) { if (value < -1 || value > 1) return BITS_ERR_FLAGS; g_opt.count_binned = value; return BITS_OK; }
+  if (!strcmp(name, "mc_batch")) { g_opt.mc_batch = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_small")) { g_opt.mc_small = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_shift_bias")) { if (value < 0 || value > 8) return BITS_ERR_FLAGS; g_opt.mc_shift_bias = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }

@@ -103,10 +103,18 @@ struct PlaceTileArgs {
   uint32_t* cross_cnt;       // [n_bins + 1] ends handed over to each bin this round (zero on entry)
   uint32_t* cross_keys;      // [n_bins * kCrossCap]
   uint32_t* flag;            // round flag
+  // several rounds per launch (gridDim.y = rounds; small sets): round blockIdx.y works on its own copy of pairs /
+  // off / cross_cnt / cross_keys, `slot_words` 32-bit words further on, takes flag[blockIdx.y] and round + blockIdx.y
+  uint32_t slot_words;
 };
 
 template <class C>
 __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kernel(PlaceTileArgs a) {
+  if (blockIdx.y) {
+    const size_t o = (size_t)blockIdx.y * a.slot_words;
+    a.pairs = reinterpret_cast<uint2*>(reinterpret_cast<uint32_t*>(a.pairs) + o);
+    a.off += o; a.cross_cnt += o; a.cross_keys += o; a.flag += blockIdx.y; a.round += blockIdx.y;
+  }
   constexpr int kPer = kMaxBins / C::kThreads;   // bin counters per thread (4 or 8)
   static_assert(kPer % 4 == 0, "uint4 accesses");
   extern __shared__ __align__(16) uint8_t smem_raw[];
@@ -254,6 +262,7 @@ struct BinSortArgs {
   uint32_t group, group_log2;           // lanes that gather one (tile, bin) segment together: a power of two, 1..32
   unsigned long long* round_total;      // += sum of ranks in B_S - sum of ranks in B_E
   uint32_t* flag;
+  uint32_t slot_words;                  // several rounds per launch (gridDim.y): as in PlaceTileArgs; dst, round_total and flag move too
 };
 
 // Counter arrays of one bin: uint16 cursors, two per word.  Entry kFront + sb belongs to
@@ -400,6 +409,12 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
 
 template <class C>
 __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_kernel(BinSortArgs a) {
+  if (blockIdx.y) {
+    const size_t o = (size_t)blockIdx.y * a.slot_words;
+    a.pairs = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(a.pairs) + o);
+    a.off += o; a.cross_cnt += o; a.cross_keys += o; a.cross_cnt_next += o; a.dst[0] += o; a.dst[1] += o;
+    a.round_total += blockIdx.y; a.flag += blockIdx.y;
+  }
   extern __shared__ __align__(16) uint8_t smem_raw[];
   uint32_t* s_ks = reinterpret_cast<uint32_t*>(smem_raw);          // [C::kCap] starts
   uint32_t* s_ke = s_ks + C::kCap;                                    // [C::kCap] ends (own + handed over)

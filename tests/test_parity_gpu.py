@@ -588,8 +588,8 @@ def _mc_b_case(a_s, a_e, b_s, b_e, off, seed, r0, n, expect_fused=None):
         fused_launches = bits.profile_read()["place_scatter"][1]
     finally:
         bits.set_option("profile", 0)
-    if expect_fused is not None:                              # which path ran: the two fused launches per round, or the general one
-        assert fused_launches == (n if expect_fused else 0)
+    if expect_fused is not None:                              # which path ran: the fused launch pairs (one per round, or one per
+        assert (0 < fused_launches <= n) if expect_fused else fused_launches == 0   # batch of rounds for small sets), or not
     o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, 1, seed, r0, n)
     assert int(host_u64(obs)[0]) == o_obs
     assert np.array_equal(host_u64(rc), o_rc)
@@ -678,6 +678,47 @@ def test_mc_permute_b_kernel_shapes(tile_variant, bin_variant):
         bits.set_option("mc_small", 1)
 
 
+def test_mc_permute_b_several_rounds_per_launch():
+    """Re-placed sets between 8,189 and 2M intervals run several rounds per launch pair (gridDim.y, one workspace slot
+    per round, the widest bins that fit): more rounds than one flag chunk holds, a partial last launch pair, forced
+    redo of some rounds, the sorted arrays of the last round out of their slot, and the one-round-per-launch path."""
+    rng = np.random.default_rng(66)
+    off = W.genome_offsets(W.GENOME24_LENGTHS)
+    def draw(n, max_len):
+        c = rng.integers(0, 24, n); ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        st = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        return st.astype(np.uint32), (st + ln - 1).astype(np.uint32)
+    b_s, b_e = draw(20_000, 3000)
+    a_s, a_e = draw(5_000, 20_000)
+    R = 4_321                                                   # > 4,096: two flag chunks, the last launch pair partial
+    obs, rc = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, 1, 5, 10, R)
+    sync()
+    o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, 1, 5, 10, R)
+    assert int(host_u64(obs)[0]) == o_obs
+    bad = np.nonzero(host_u64(rc) != o_rc)[0]
+    assert bad.size == 0, (bad.size, bad[:8])
+    bits.set_option("mc_force_redo", 7)
+    try:
+        _mc_b_case(a_s, a_e, b_s, b_e, off, 5, 10, 45, expect_fused=True)
+    finally:
+        bits.set_option("mc_force_redo", 0)
+    for rounds in (1, 2, 30, 31):                               # the last round sits in different slots
+        ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, 5_000, 20_000, 24, 1), dtype=torch.uint8, device=DEV)
+        bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, 1, 5, 3, rounds, workspace=ws)
+        sync()
+        g_s, g_e = bits.sorted_arrays_in_workspace(ws, bits.FN_MC_ROUNDS, 5_000, 20_000, 24, 1)
+        p_s, p_e = oracle.place_round((b_e - b_s).astype(np.uint32), off, 5, 3 + rounds - 1, 1)
+        assert np.array_equal(host_u32(g_s), oracle.sort_u32(p_s)) and np.array_equal(host_u32(g_e), oracle.sort_u32(p_e))
+    bits.set_option("mc_batch", 0)
+    try:
+        _, rc1 = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, 1, 5, 10, 40)
+        sync()
+    finally:
+        bits.set_option("mc_batch", 1)
+    assert np.array_equal(host_u64(rc1), o_rc[:40])
+
+
 def test_mc_permute_b_small_sets_one_block_per_round():
     """Sets of at most 8,188 intervals: one block does a whole round in shared memory and the grid strides over the
     rounds (mc_small.cuh).  Sizes around the limit, more rounds than blocks, tiny genomes with heavy ties, a query
@@ -760,7 +801,8 @@ def test_mc_workspace_contents_do_not_matter():
     big = W.make_config(5, scale=0.03)
     small = W.make_config(5, scale=0.01)
     n_chrom = int(big.chrom_offsets.size - 1)
-    ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, big.n_a, big.n_b, n_chrom, 1), dtype=torch.uint8, device=DEV)
+    # (the smaller set takes more round slots per launch pair: its workspace is not the smaller one)
+    ws = torch.empty(max(bits.workspace_bytes(bits.FN_MC_ROUNDS, x.n_a, x.n_b, n_chrom, 1) for x in (big, small)), dtype=torch.uint8, device=DEV)
     for fill, w, which, rounds in ((0xFF, big, 1, 3), (0xAB, small, 1, 4), (0x01, big, 0, 3), (0x80, small, 1, 2), (0x00, big, 1, 2)):
         ws.fill_(fill)
         obs, rc = bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, which, 9, 2, rounds,
