@@ -232,7 +232,7 @@ constexpr uint64_t kBatchMaxKeys = 2u << 20;    // re-placed sets up to this siz
 constexpr uint32_t kBatchMaxSlots = 32, kBatchBins = 512;
 static inline uint32_t batch_slots_for(uint64_t n) {
   if (n <= (uint64_t)mcs::kMaxKeys || n > kBatchMaxKeys) return 1;     // (smaller sets: one block per round, mc_small.cuh)
-  const uint64_t s = (4ull << 20) / n;
+  const uint64_t s = (16ull << 20) / n;
   return (uint32_t)(s < 2 ? 2 : (s > kBatchMaxSlots ? kBatchMaxSlots : s));
 }
 // Tiles are balanced: every block of place_tile_kernel gets the same number of equally sized tiles.
@@ -969,7 +969,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       if (wide >= 0) {
         const uint64_t nb = (G + (1ull << wide) - 1) >> wide;
         const uint32_t per = (uint32_t)(nb < 2ull * kSMs ? nb : 2ull * kSMs);
-        uint32_t r = 4u * (uint32_t)kSMs / (per ? per : 1u);           // about two waves of bin blocks per launch
+        uint32_t r = 8u * (uint32_t)kSMs / (per ? per : 1u);           // about four waves of bin blocks per launch
         if (r > L.batch_slots) r = L.batch_slots;
         const uint32_t max_tile = tile_variant == 0 ? (uint32_t)mct::TileCfg2x512::kTile
                                 : (tile_variant == 1 ? (uint32_t)mct::TileCfg1x1024::kTile : (uint32_t)mct::TileCfg1x1024L::kTile);
