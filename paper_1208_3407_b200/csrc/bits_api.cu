@@ -429,6 +429,12 @@ static int msd_configure() {
     const cudaError_t e2 = cudaFuncSetAttribute(msd::bucket_sort_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)msd::kBkSmem);
     cudaError_t e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgWide>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)mct::BinCfgWide::smem_bytes(mct::kMaxTiles));
+    // (the several-rounds-per-launch instantiations)
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgWide, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::BinCfgWide::smem_bytes(mct::kMaxTiles));
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgNarrow, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::BinCfgNarrow::smem_bytes(mct::kMaxTiles));
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgSmall, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::BinCfgSmall::smem_bytes(mct::kMaxTiles));
+    if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgHuge, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                     (int)(mct::BinCfgHuge::smem_bytes(mct::kMaxTiles) < kMaxSmemPerBlock ? mct::BinCfgHuge::smem_bytes(mct::kMaxTiles) : kMaxSmemPerBlock));
     if (e3 == cudaSuccess)
       e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgNarrow>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)mct::BinCfgNarrow::smem_bytes(mct::kMaxTiles));
@@ -439,6 +445,9 @@ static int msd_configure() {
       e3 = cudaFuncSetAttribute(mct::bin_sort_search_kernel<mct::BinCfgSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)mct::BinCfgSmall::smem_bytes(mct::kMaxTiles));
     cudaError_t e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg2x512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg2x512::kSmem);
+    if (e4 == cudaSuccess) e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg2x512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg2x512::kSmem);
+    if (e4 == cudaSuccess) e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024::kSmem);
+    if (e4 == cudaSuccess) e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024L::kSmem);
     if (e4 == cudaSuccess)
       e4 = cudaFuncSetAttribute(mct::place_tile_kernel<mct::TileCfg1x1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mct::TileCfg1x1024::kSmem);
     if (e4 == cudaSuccess)
@@ -757,13 +766,15 @@ static int launch_place(const uint32_t* spans, uint32_t* start_out, uint32_t* en
 template <class C>
 static void launch_place_tile(const mct::PlaceTileArgs& pt, uint32_t rounds, cudaStream_t st) {
   const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
-  launch_pdl(mct::place_tile_kernel<C>, dim3(pt.n_tiles < blocks ? pt.n_tiles : blocks, rounds), C::kThreads, C::kSmem, st, pt);
+  if (pt.slot_words) launch_pdl(mct::place_tile_kernel<C, true>, dim3(pt.n_tiles < blocks ? pt.n_tiles : blocks, rounds), C::kThreads, C::kSmem, st, pt);
+  else launch_pdl(mct::place_tile_kernel<C, false>, dim3(pt.n_tiles < blocks ? pt.n_tiles : blocks, 1), C::kThreads, C::kSmem, st, pt);
 }
 
 template <class C>
 static void launch_bin_sort(const mct::BinSortArgs& bs, uint32_t rounds, cudaStream_t st) {
   const uint32_t blocks = (uint32_t)C::kBlocksPerSm * (uint32_t)kSMs;
-  launch_pdl(mct::bin_sort_search_kernel<C>, dim3(bs.n_bins < blocks ? bs.n_bins : blocks, rounds), C::kThreads, C::smem_bytes(bs.n_tiles), st, bs);
+  if (bs.slot_words) launch_pdl(mct::bin_sort_search_kernel<C, true>, dim3(bs.n_bins < blocks ? bs.n_bins : blocks, rounds), C::kThreads, C::smem_bytes(bs.n_tiles), st, bs);
+  else launch_pdl(mct::bin_sort_search_kernel<C, false>, dim3(bs.n_bins < blocks ? bs.n_bins : blocks, 1), C::kThreads, C::smem_bytes(bs.n_tiles), st, bs);
 }
 
 static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,

@@ -108,9 +108,11 @@ struct PlaceTileArgs {
   uint32_t slot_words;
 };
 
-template <class C>
+// kSlots: several rounds per launch (the arguments are then moved to the round's slot; the one-round instantiation
+// keeps reading them straight from the parameter bank).
+template <class C, bool kSlots = false>
 __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) place_tile_kernel(PlaceTileArgs a) {
-  if (blockIdx.y) {
+  if (kSlots && blockIdx.y) {
     const size_t o = (size_t)blockIdx.y * a.slot_words;
     a.pairs = reinterpret_cast<uint2*>(reinterpret_cast<uint32_t*>(a.pairs) + o);
     a.off += o; a.cross_cnt += o; a.cross_keys += o; a.flag += blockIdx.y; a.round += blockIdx.y;
@@ -407,9 +409,9 @@ __device__ __forceinline__ uint64_t write_and_rank(const uint32_t* buf, uint32_t
   return qsum;
 }
 
-template <class C>
+template <class C, bool kSlots = false>
 __global__ void __launch_bounds__(C::kThreads, C::kBlocksPerSm) bin_sort_search_kernel(BinSortArgs a) {
-  if (blockIdx.y) {
+  if (kSlots && blockIdx.y) {
     const size_t o = (size_t)blockIdx.y * a.slot_words;
     a.pairs = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(a.pairs) + o);
     a.off += o; a.cross_cnt += o; a.cross_keys += o; a.cross_cnt_next += o; a.dst[0] += o; a.dst[1] += o;
