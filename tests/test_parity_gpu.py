@@ -1014,3 +1014,59 @@ def test_second_device_gets_its_own_kernel_attributes():
             o_obs, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, 3, 0, 4)
             want = (o_obs, o_rc.tolist(), o_obs)
         assert got == want
+
+
+# ------------------------------------------------------------------------------------- randomised sweep
+@pytest.mark.parametrize("seed,cases,big", [(1, 400, False), (2, 400, False), (3, 30, True), (4, 30, True)])
+def test_randomised_cases_against_the_oracle(seed, cases, big):
+    """Seeded random genomes (1-39 chromosomes of 10^3..2*10^8 bp), set sizes over all size classes of every path
+    (one block per round, several rounds per launch pair, one round per launch pair; bucket index and binned search),
+    uniform and clustered placement, spans up to the chromosome length: Monte Carlo rounds of both kinds, counts by
+    both search designs, screens -- every integer against the oracle."""
+    rng = np.random.default_rng(seed)
+    def genome():
+        k = int(rng.integers(1, 40))
+        scale = int(10 ** (rng.uniform(6.5, 8.3) if big else rng.uniform(3, 8.3)))
+        lens = rng.integers(max(2, scale // 10), scale + 2, k)
+        while lens.sum() >= 2**32 - 1:
+            lens = lens // 2 + 1
+        return W.genome_offsets(lens)
+    def draw(off, n, max_len):
+        c = rng.integers(0, off.size - 1, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        ln = np.minimum(rng.integers(1, max_len + 1, n), hi - lo)
+        frac = rng.beta(0.3, 0.3, n) if rng.random() < 0.3 else rng.random(n)     # clustered at the chromosome ends, or uniform
+        st = np.minimum(lo + ((hi - lo - ln + 1) * frac).astype(np.int64), hi - ln)
+        return st.astype(np.uint32), (st + ln - 1).astype(np.uint32)
+    done = 0
+    while done < cases:
+        off = genome()
+        lmax = int(np.diff(off.astype(np.int64)).max())
+        kind = int(rng.integers(0, 3))
+        if kind == 0:
+            n_b = int(10 ** (rng.uniform(3.9, 6.5) if big else rng.uniform(0, 4.9)))
+            n_a = int(10 ** (rng.uniform(2, 5.3) if big else rng.uniform(0, 4.3)))
+            max_len = max(1, int(min(lmax - 1, 10 ** rng.uniform(0, 5))))
+            b_s, b_e = draw(off, n_b, max_len); a_s, a_e = draw(off, n_a, max_len)
+            which = 1 if big else int(rng.integers(0, 2))
+            R = int(rng.integers(1, 10 if big else 70)); r0 = int(rng.integers(0, 2**32 - 100)); mc_seed = int(rng.integers(0, 2**63))
+            if int(((b_e - b_s) if which else (a_e - a_s)).max()) >= lmax:
+                continue
+            obs, rc = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, which, mc_seed, r0, R)
+            sync()
+            o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, which, mc_seed, r0, R)
+            assert int(host_u64(obs)[0]) == o_obs and np.array_equal(host_u64(rc), o_rc), ("mc", n_a, n_b, off.size - 1, which, R, r0, mc_seed)
+        elif kind == 1:
+            n_b = int(10 ** (rng.uniform(5, 6.7) if big else rng.uniform(0, 5.5)))
+            n_a = int(10 ** (rng.uniform(5, 6.4) if big else rng.uniform(0, 5.3)))
+            b_s, b_e = draw(off, n_b, int(10 ** rng.uniform(0, 7))); a_s, a_e = draw(off, n_a, int(10 ** rng.uniform(0, 7)))
+            check_counts(a_s, a_e, b_s, b_e)
+        else:
+            K = int(rng.integers(1, 6)); R = int(rng.integers(0, 8))
+            tracks = [draw(off, int(10 ** rng.uniform(0, 4)), max(1, int(min(lmax - 1, 10 ** rng.uniform(0, 4))))) for _ in range(K)]
+            if max(int((e - st).max()) for st, e in tracks) >= lmax:
+                continue
+            obs, enr, rc = bits.screen([(dev(st), dev(e)) for st, e in tracks], off, 7, R, round_begin=3)
+            o_obs, o_rc, o_enr = oracle.screen(tracks, off, 7, 3, R)
+            assert np.array_equal(obs, o_obs) and np.array_equal(rc, o_rc) and np.array_equal(enr, o_enr, equal_nan=True), ("screen", K, R)
+        done += 1
