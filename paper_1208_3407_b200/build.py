@@ -22,10 +22,11 @@ FLAGS = [
 
 
 def csrc_hash() -> str:
-    """sha256 over the kernel sources (csrc/*.cu, *.cuh, sorted by name): identifies the build a profile was taken of."""
+    """sha256 over the kernel sources (csrc/*.cuh, sorted by name; the host-side orchestration in bits_api.cu is not
+    part of it): identifies the kernels a profile was taken of."""
     import hashlib
     h = hashlib.sha256()
-    for path in sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))):
+    for path in sorted(glob.glob(os.path.join(CSRC, "*.cuh"))):
         h.update(os.path.basename(path).encode())
         with open(path, "rb") as f:
             h.update(f.read())

@@ -228,7 +228,7 @@ struct Layout {
 };
 constexpr uint32_t kFlagChunk = 4096;    // fused rounds are checked for raised flags in chunks of this many
 constexpr uint64_t kFusedMaxKeys = 24u << 20;   // beyond this the bins of the fused path cannot hold the set
-constexpr uint64_t kBatchMaxKeys = 2u << 20;    // re-placed sets up to this size run several rounds per launch pair
+constexpr uint64_t kBatchMaxKeys = 4u << 20;    // re-placed sets up to this size run several rounds per launch pair
 constexpr uint32_t kBatchMaxSlots = 32, kBatchBins = 512;
 static inline uint32_t batch_slots_for(uint64_t n) {
   if (n <= (uint64_t)mcs::kMaxKeys || n > kBatchMaxKeys) return 1;     // (smaller sets: one block per round, mc_small.cuh)
