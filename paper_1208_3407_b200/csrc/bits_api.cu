@@ -38,6 +38,7 @@ struct Options {
   int64_t msd_pack = 7168;         // MSD sort plan: 0 = buckets by the prefix / target rule, n = consecutive bins packed greedily up to n keys (measured on config 4: 0 -> 146 us, 8192 -> 134, 7168 -> 124 for the bucket sort)
   int64_t msd_scatter_shape = 0;   // MSD scatter pass: 0 = one 1,024-thread block per SM and 16,384-key tiles, 1 = two 512-thread blocks and 8,192-key tiles
   int64_t count_binned = -1;       // count path: 1 = queries binned by B's buckets and searched out of shared memory (binned_count.cuh), 0 = bucket index + count_kernel, -1 = by size
+  int64_t mc_a_rounds_per_block = 4;   // PERMUTE_A rounds (and the sort-free variant): rounds a block serves for its query tile
   int64_t mc_batch = 1;            // PERMUTE_B fused rounds of small sets: 1 = several rounds per launch pair (gridDim.y), 0 = one
   int64_t mc_small = 1;            // PERMUTE_B rounds of a set that fits one block's shared memory: 1 = one block per round (mc_small.cuh)
   int64_t mc_shift_bias = 0;       // PERMUTE_B fused rounds: added to the bin width (log2) the host picked; > 0 overflows bins on purpose (tests)
@@ -834,9 +835,10 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     const unsigned gx = (unsigned)ceil_div(ceil_div(n_a, 4), 256);
     for (uint32_t done = 0; done < n_rounds;) {
       const uint32_t chunk = n_rounds - done < 32768u ? n_rounds - done : 32768u;
-      m.round0 = round_begin + done; m.out0 = done;
+      m.round0 = round_begin + done; m.out0 = done; m.n_launch = chunk;
+      m.rpb = (uint32_t)g_opt.mc_a_rounds_per_block;
       ProfScope prof(kClsMcA, st);
-      mc_permute_a_kernel<<<dim3(gx, chunk), 256, 0, st>>>(m);
+      mc_permute_a_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
       BITS_LAUNCH_CHECK();
       done += chunk;
     }
@@ -861,9 +863,10 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     const unsigned gx = (unsigned)ceil_div(ceil_div(n_b, 4), 256);
     for (uint32_t done = 0; done < n_rounds;) {
       const uint32_t chunk = n_rounds - done < 4096u ? n_rounds - done : 4096u;
-      m.round0 = round_begin + done; m.out0 = done;
+      m.round0 = round_begin + done; m.out0 = done; m.n_launch = chunk;
+      m.rpb = (uint32_t)g_opt.mc_a_rounds_per_block;
       ProfScope prof(kClsMcA, st);
-      mc_permute_a_kernel<<<dim3(gx, chunk), 256, 0, st>>>(m);
+      mc_permute_a_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
       BITS_LAUNCH_CHECK();
       done += chunk;
     }
@@ -1216,6 +1219,7 @@ static int screen_impl(const uint32_t* starts, const uint32_t* ends, const uint6
   scr::ScreenArgs a;
   a.tracks = L.tracks; a.tile_track = L.tile_track; a.tile_first = L.tile_first; a.n_tracks = K;
   a.round0 = round_begin; a.out0 = 0; a.n_rounds = n_rounds; a.key = make_philox_keys(seed); a.chrom = chrom;
+  a.rpb = 1; a.n_launch = 1;
   a.observed = reinterpret_cast<unsigned long long*>(observed_out);
   a.round_counts = reinterpret_cast<unsigned long long*>(round_counts_out);
   {
@@ -1225,9 +1229,9 @@ static int screen_impl(const uint32_t* starts, const uint32_t* ends, const uint6
   }
   for (uint32_t done = 0; done < n_rounds;) {
     const uint32_t chunk = n_rounds - done < 4096u ? n_rounds - done : 4096u;
-    a.round0 = round_begin + done; a.out0 = done;
+    a.round0 = round_begin + done; a.out0 = done; a.n_launch = chunk; a.rpb = (uint32_t)g_opt.mc_a_rounds_per_block;
     ProfScope prof(kClsMcA, st);
-    scr::screen_kernel<false><<<dim3((unsigned)L.n_tiles, K, chunk), scr::kThreads, 0, st>>>(a);
+    scr::screen_kernel<false><<<dim3((unsigned)L.n_tiles, K, (unsigned)ceil_div(chunk, a.rpb)), scr::kThreads, 0, st>>>(a);
     BITS_LAUNCH_CHECK();
     done += chunk;
   }
@@ -1536,6 +1540,7 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "msd_pack")) { if (value < 0 || value > msd::kBucketCap) return BITS_ERR_FLAGS; g_opt.msd_pack = value; return BITS_OK; }
   if (!strcmp(name, "msd_scatter_shape")) { if (value < 0 || value > 1) return BITS_ERR_FLAGS; g_opt.msd_scatter_shape = value; return BITS_OK; }
   if (!strcmp(name, "count_binned")) { if (value < -1 || value > 1) return BITS_ERR_FLAGS; g_opt.count_binned = value; return BITS_OK; }
+  if (!strcmp(name, "mc_a_rounds_per_block")) { if (value < 1 || value > 64) return BITS_ERR_FLAGS; g_opt.mc_a_rounds_per_block = value; return BITS_OK; }
   if (!strcmp(name, "mc_batch")) { g_opt.mc_batch = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_small")) { g_opt.mc_small = value != 0; return BITS_OK; }
   if (!strcmp(name, "mc_shift_bias")) { if (value < 0 || value > 8) return BITS_ERR_FLAGS; g_opt.mc_shift_bias = value; return BITS_OK; }

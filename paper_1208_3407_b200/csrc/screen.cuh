@@ -38,6 +38,8 @@ struct ScreenArgs {
   uint32_t round0;                // round of blockIdx.z == 0
   uint32_t out0;                  // its position in a pair's row of round_counts
   uint32_t n_rounds;              // row length of round_counts
+  uint32_t rpb;                   // rounds a block serves for its (query tile, partner): gridDim.z = ceil(n_launch / rpb)
+  uint32_t n_launch;              // rounds of this launch
   PhiloxKeys key;
   ChromTable chrom;
   unsigned long long* observed;       // dev [n_tracks * n_tracks]
@@ -61,25 +63,34 @@ __global__ void __launch_bounds__(kThreads) screen_kernel(ScreenArgs a) {
   const uint32_t t = (blockIdx.x - __ldg(a.tile_first + i)) * kThreads + threadIdx.x;
   const uint32_t i0 = t << 2;
   const uint32_t pair = i * a.n_tracks + j;
-  uint64_t sum = 0;
-  if (i0 < ti.n) {
-    if (kObserved) {
+  const bool active = i0 < ti.n;
+  if (kObserved) {
+    uint64_t sum = 0;
+    if (active) {
 #pragma unroll
       for (int q = 0; q < 4; ++q)
         if (i0 + q < ti.n) sum += icount(bs, be, __ldg(ti.start + i0 + q), __ldg(ti.end + i0 + q));
-    } else {
-      const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(ti.spans) + t);
-      const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
+    }
+    block_sum_atomic(sum, s_red, a.observed + pair);
+    return;
+  }
+  // the staged chromosome table and the spans are paid once for a.rpb consecutive rounds; one atomicAdd per warp and round
+  const uint4 d4 = active ? __ldg(reinterpret_cast<const uint4*>(ti.spans) + t) : make_uint4(0, 0, 0, 0);
+  const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
+  const uint32_t r_first = blockIdx.z * a.rpb, r_end = min(r_first + a.rpb, a.n_launch);
+  unsigned long long* row = a.round_counts + (size_t)pair * a.n_rounds + a.out0;
+  for (uint32_t r = r_first; r < r_end; ++r) {
+    uint64_t sum = 0;
+    if (active) {
       uint32_t st[4];
-      place4(i0, a.round0 + blockIdx.z, 0u, a.key, d, off, a.chrom, st, pair);
+      place4(i0, a.round0 + r, 0u, a.key, d, off, a.chrom, st, pair);
 #pragma unroll
       for (int q = 0; q < 4; ++q)
         if (i0 + q < ti.n) sum += icount(bs, be, st[q], st[q] + d[q]);
     }
+    sum = warp_sum_u64(sum);
+    if ((threadIdx.x & 31) == 0 && sum) atomicAdd(row + r, (unsigned long long)sum);
   }
-  unsigned long long* out = kObserved ? a.observed + pair
-                                      : a.round_counts + (size_t)pair * a.n_rounds + a.out0 + blockIdx.z;
-  block_sum_atomic(sum, s_red, out);
 }
 
 }  // namespace scr

@@ -308,29 +308,37 @@ struct McAArgs {
   PhiloxKeys key;
   ChromTable chrom;
   SortedSet bs, be;
-  unsigned long long* round_counts;   // indexed by blockIdx.y + out0
+  unsigned long long* round_counts;   // indexed by out0 + round of the launch
   uint32_t out0;
+  uint32_t rpb;              // rounds per block: gridDim.y = ceil(n_launch / rpb)
+  uint32_t n_launch;         // rounds of this launch
 };
 
 __global__ void __launch_bounds__(256) mc_permute_a_kernel(McAArgs a) {
   __shared__ uint32_t s_off[kMaxChromSmem];
   __shared__ __align__(16) uint16_t s_lut[kLutSize];
-  __shared__ uint64_t s_red[8];
   const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);
-  const uint32_t round = a.round0 + blockIdx.y;
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t i0 = t << 2;
-  uint64_t sum = 0;
-  if (i0 < a.n_a) {
-    const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans) + t);
-    const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
-    uint32_t st[4];
-    place4(i0, round, a.tag, a.key, d, off, a.chrom, st);
+  const bool active = i0 < a.n_a;
+  const uint4 d4 = active ? __ldg(reinterpret_cast<const uint4*>(a.spans) + t) : make_uint4(0, 0, 0, 0);
+  const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
+  // a block serves the same query tile for a.rpb consecutive rounds: the staged chromosome table and the spans are
+  // paid once; one atomicAdd per warp and round (no block barrier inside the loop)
+  const uint32_t r_first = blockIdx.y * a.rpb;
+  const uint32_t r_end = min(r_first + a.rpb, a.n_launch);
+  for (uint32_t r = r_first; r < r_end; ++r) {
+    uint64_t sum = 0;
+    if (active) {
+      uint32_t st[4];
+      place4(i0, a.round0 + r, a.tag, a.key, d, off, a.chrom, st);
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
-      if (i0 + j < a.n_a) sum += icount(a.bs, a.be, st[j], st[j] + d[j]);
+      for (int j = 0; j < 4; ++j)
+        if (i0 + j < a.n_a) sum += icount(a.bs, a.be, st[j], st[j] + d[j]);
+    }
+    sum = warp_sum_u64(sum);
+    if ((threadIdx.x & 31) == 0 && sum) atomicAdd(a.round_counts + a.out0 + r, (unsigned long long)sum);
   }
-  block_sum_atomic(sum, s_red, a.round_counts + a.out0 + blockIdx.y);
 }
 
 }  // namespace bits
