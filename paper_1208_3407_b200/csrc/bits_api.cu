@@ -778,6 +778,14 @@ static void launch_bin_sort(const mct::BinSortArgs& bs, uint32_t rounds, cudaStr
   else launch_pdl(mct::bin_sort_search_kernel<C, false>, dim3(bs.n_bins < blocks ? bs.n_bins : blocks, 1), C::kThreads, C::smem_bytes(bs.n_tiles), st, bs);
 }
 
+// Rounds a block of the PERMUTE_A / screen kernels serves for its query tile: the option's value, fewer when the
+// launch would otherwise not fill the GPU (eight 256-thread blocks per SM).
+static inline uint32_t rounds_per_block(uint64_t tile_rounds) {
+  const uint64_t fill = tile_rounds / ((uint64_t)kSMs * 8u);
+  const uint64_t want = (uint64_t)g_opt.mc_a_rounds_per_block;
+  return (uint32_t)(fill < 1 ? 1 : (fill < want ? fill : want));
+}
+
 static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
                    const uint32_t* b_end, uint64_t n_b, const uint32_t* off, uint32_t n_chrom, int which, uint64_t seed,
                    uint32_t round_begin, uint32_t n_rounds, uint32_t flags, void* ws, size_t ws_bytes,
@@ -836,7 +844,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     for (uint32_t done = 0; done < n_rounds;) {
       const uint32_t chunk = n_rounds - done < 32768u ? n_rounds - done : 32768u;
       m.round0 = round_begin + done; m.out0 = done; m.n_launch = chunk;
-      m.rpb = (uint32_t)g_opt.mc_a_rounds_per_block;
+      m.rpb = rounds_per_block((uint64_t)gx * chunk);
       ProfScope prof(kClsMcA, st);
       mc_permute_a_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
       BITS_LAUNCH_CHECK();
@@ -864,7 +872,7 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     for (uint32_t done = 0; done < n_rounds;) {
       const uint32_t chunk = n_rounds - done < 4096u ? n_rounds - done : 4096u;
       m.round0 = round_begin + done; m.out0 = done; m.n_launch = chunk;
-      m.rpb = (uint32_t)g_opt.mc_a_rounds_per_block;
+      m.rpb = rounds_per_block((uint64_t)gx * chunk);
       ProfScope prof(kClsMcA, st);
       mc_permute_a_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
       BITS_LAUNCH_CHECK();
@@ -1229,7 +1237,7 @@ static int screen_impl(const uint32_t* starts, const uint32_t* ends, const uint6
   }
   for (uint32_t done = 0; done < n_rounds;) {
     const uint32_t chunk = n_rounds - done < 4096u ? n_rounds - done : 4096u;
-    a.round0 = round_begin + done; a.out0 = done; a.n_launch = chunk; a.rpb = (uint32_t)g_opt.mc_a_rounds_per_block;
+    a.round0 = round_begin + done; a.out0 = done; a.n_launch = chunk; a.rpb = rounds_per_block((uint64_t)L.n_tiles * K * chunk);
     ProfScope prof(kClsMcA, st);
     scr::screen_kernel<false><<<dim3((unsigned)L.n_tiles, K, (unsigned)ceil_div(chunk, a.rpb)), scr::kThreads, 0, st>>>(a);
     BITS_LAUNCH_CHECK();
