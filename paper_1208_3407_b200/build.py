@@ -21,12 +21,15 @@ FLAGS = [
 ]
 
 
+FUSED_KERNEL_SOURCES = ("common.cuh", "mc_tile.cuh", "msd_sort.cuh", "philox_place.cuh")
+
+
 def csrc_hash() -> str:
-    """sha256 over the kernel sources (csrc/*.cuh, sorted by name; the host-side orchestration in bits_api.cu is not
-    part of it): identifies the kernels a profile was taken of."""
+    """sha256 over the sources the two fused Monte Carlo kernels are compiled from (FUSED_KERNEL_SOURCES): identifies
+    the kernels whose ncu counters profiles/r2b_fused_ncu_counters.json holds."""
     import hashlib
     h = hashlib.sha256()
-    for path in sorted(glob.glob(os.path.join(CSRC, "*.cuh"))):
+    for path in [os.path.join(CSRC, f) for f in FUSED_KERNEL_SOURCES]:
         h.update(os.path.basename(path).encode())
         with open(path, "rb") as f:
             h.update(f.read())

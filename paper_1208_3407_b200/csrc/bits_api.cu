@@ -846,7 +846,8 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       m.round0 = round_begin + done; m.out0 = done; m.n_launch = chunk;
       m.rpb = rounds_per_block((uint64_t)gx * chunk);
       ProfScope prof(kClsMcA, st);
-      mc_permute_a_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
+      if (m.rpb > 1) mc_permute_a_rounds_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
+      else mc_permute_a_kernel<<<dim3(gx, chunk), 256, 0, st>>>(m);
       BITS_LAUNCH_CHECK();
       done += chunk;
     }
@@ -874,7 +875,8 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
       m.round0 = round_begin + done; m.out0 = done; m.n_launch = chunk;
       m.rpb = rounds_per_block((uint64_t)gx * chunk);
       ProfScope prof(kClsMcA, st);
-      mc_permute_a_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
+      if (m.rpb > 1) mc_permute_a_rounds_kernel<<<dim3(gx, (unsigned)ceil_div(chunk, m.rpb)), 256, 0, st>>>(m);
+      else mc_permute_a_kernel<<<dim3(gx, chunk), 256, 0, st>>>(m);
       BITS_LAUNCH_CHECK();
       done += chunk;
     }
@@ -1239,7 +1241,8 @@ static int screen_impl(const uint32_t* starts, const uint32_t* ends, const uint6
     const uint32_t chunk = n_rounds - done < 4096u ? n_rounds - done : 4096u;
     a.round0 = round_begin + done; a.out0 = done; a.n_launch = chunk; a.rpb = rounds_per_block((uint64_t)L.n_tiles * K * chunk);
     ProfScope prof(kClsMcA, st);
-    scr::screen_kernel<false><<<dim3((unsigned)L.n_tiles, K, (unsigned)ceil_div(chunk, a.rpb)), scr::kThreads, 0, st>>>(a);
+    if (a.rpb > 1) scr::screen_kernel<false><<<dim3((unsigned)L.n_tiles, K, (unsigned)ceil_div(chunk, a.rpb)), scr::kThreads, 0, st>>>(a);
+    else scr::screen_round_kernel<<<dim3((unsigned)L.n_tiles, K, chunk), scr::kThreads, 0, st>>>(a);
     BITS_LAUNCH_CHECK();
     done += chunk;
   }

@@ -93,5 +93,46 @@ __global__ void __launch_bounds__(kThreads) screen_kernel(ScreenArgs a) {
   }
 }
 
+// One round per block (grid = (query tiles of all tracks, partner track j, rounds of this launch)): for launches too
+// small to give every block several rounds.
+__global__ void __launch_bounds__(kThreads) screen_round_kernel(ScreenArgs a) {
+  constexpr bool kObserved = false;
+  __shared__ uint32_t s_off[kObserved ? 1 : kMaxChromSmem];
+  __shared__ __align__(16) uint16_t s_lut[kObserved ? 8 : kLutSize];
+  __shared__ uint64_t s_red[kThreads / 32];
+  const uint32_t i = __ldg(a.tile_track + blockIdx.x), j = blockIdx.y;
+  const Track ti = a.tracks[i], tj = a.tracks[j];
+  if (tj.n == 0) return;                                  // nothing to intersect: the counts stay 0
+  ChromView off;
+  if (!kObserved) off = stage_chrom_table(a.chrom, s_off, s_lut);
+  SortedSet bs, be;
+  bs.keys = tj.keys[0]; bs.idx = tj.idx[0]; bs.n = tj.n; bs.shift = tj.shift;
+  be.keys = tj.keys[1]; be.idx = tj.idx[1]; be.n = tj.n; be.shift = tj.shift;
+  const uint32_t t = (blockIdx.x - __ldg(a.tile_first + i)) * kThreads + threadIdx.x;
+  const uint32_t i0 = t << 2;
+  const uint32_t pair = i * a.n_tracks + j;
+  uint64_t sum = 0;
+  if (i0 < ti.n) {
+    if (kObserved) {
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+        if (i0 + q < ti.n) sum += icount(bs, be, __ldg(ti.start + i0 + q), __ldg(ti.end + i0 + q));
+    } else {
+      const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(ti.spans) + t);
+      const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
+      uint32_t st[4];
+      place4(i0, a.round0 + blockIdx.z, 0u, a.key, d, off, a.chrom, st, pair);
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+        if (i0 + q < ti.n) sum += icount(bs, be, st[q], st[q] + d[q]);
+    }
+  }
+  unsigned long long* out = kObserved ? a.observed + pair
+                                      : a.round_counts + (size_t)pair * a.n_rounds + a.out0 + blockIdx.z;
+  block_sum_atomic(sum, s_red, out);
+}
+
+
+
 }  // namespace scr
 }  // namespace bits

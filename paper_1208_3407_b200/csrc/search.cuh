@@ -314,7 +314,7 @@ struct McAArgs {
   uint32_t n_launch;         // rounds of this launch
 };
 
-__global__ void __launch_bounds__(256) mc_permute_a_kernel(McAArgs a) {
+__global__ void __launch_bounds__(256) mc_permute_a_rounds_kernel(McAArgs a) {
   __shared__ uint32_t s_off[kMaxChromSmem];
   __shared__ __align__(16) uint16_t s_lut[kLutSize];
   const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);
@@ -339,6 +339,28 @@ __global__ void __launch_bounds__(256) mc_permute_a_kernel(McAArgs a) {
     sum = warp_sum_u64(sum);
     if ((threadIdx.x & 31) == 0 && sum) atomicAdd(a.round_counts + a.out0 + r, (unsigned long long)sum);
   }
+}
+
+// One round per block (grid = (query tiles, rounds)): for launches too small to give every block several rounds.
+__global__ void __launch_bounds__(256) mc_permute_a_kernel(McAArgs a) {
+  __shared__ uint32_t s_off[kMaxChromSmem];
+  __shared__ __align__(16) uint16_t s_lut[kLutSize];
+  __shared__ uint64_t s_red[8];
+  const ChromView off = stage_chrom_table(a.chrom, s_off, s_lut);
+  const uint32_t round = a.round0 + blockIdx.y;
+  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t i0 = t << 2;
+  uint64_t sum = 0;
+  if (i0 < a.n_a) {
+    const uint4 d4 = __ldg(reinterpret_cast<const uint4*>(a.spans) + t);
+    const uint32_t d[4] = {d4.x, d4.y, d4.z, d4.w};
+    uint32_t st[4];
+    place4(i0, round, a.tag, a.key, d, off, a.chrom, st);
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (i0 + j < a.n_a) sum += icount(a.bs, a.be, st[j], st[j] + d[j]);
+  }
+  block_sum_atomic(sum, s_red, a.round_counts + a.out0 + blockIdx.y);
 }
 
 }  // namespace bits
