@@ -159,8 +159,8 @@ int bits_count_per_interval(const uint32_t* a_start, const uint32_t* a_end, uint
  * own no longer pair a start with its end, so the lengths the re-placement must keep are lost.
  * Synchronisation: `stream` is synchronised once before the first round (the longest span of the
  * permuted set is checked against the longest chromosome: BITS_ERR_NO_PLACEMENT) and, with
- * BITS_PERMUTE_B, once more per 4,096 rounds (overflow flags of the fused rounds are read back; a
- * flagged round is redone by the general path).  After such a redo the "sorted arrays of the last
+ * BITS_PERMUTE_B and more than 8,188 re-placed intervals, once more per (at most) 4,096 rounds: the
+ * overflow flags of the fused rounds are read back; a flagged round is redone by the general path.  After such a redo the "sorted arrays of the last
  * round" (bits_workspace_sorted_offset) are those of the round that was redone last. */
 int bits_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
                    const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
