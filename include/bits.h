@@ -55,7 +55,8 @@ typedef enum {
   BITS_ERR_WORKSPACE = 5,     /* workspace NULL, misaligned (256 B) or smaller than required */
   BITS_ERR_FLAGS = 6,         /* unknown flag bit, bad `which`, bad `fn`, bad `tail` */
   BITS_ERR_MALFORMED = 7,     /* BITS_VALIDATE: some start > end */
-  BITS_ERR_CUDA = 8           /* a CUDA call failed (including: no device) */
+  BITS_ERR_CUDA = 8,          /* a CUDA call failed (including: no device) */
+  BITS_ERR_STATIC_LIMIT = 9   /* bits_count_static only: the problem needs more scratch than the built-in array holds */
 } bits_status;
 
 /* flags */
@@ -111,6 +112,40 @@ int bits_count(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
                const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
                uint32_t flags, void* workspace, size_t workspace_bytes,
                uint64_t* total_out, void* stream);
+
+/* The counting problem for a caller that cannot supply a workspace.
+ *
+ * Every other compute entry point takes its scratch from a caller-allocated device workspace.  Some callers
+ * have no way to make one: they are handed their input and output buffers by somebody else and may not, or
+ * cannot, create device memory themselves.  Typical cases: a processing stage plugged into a host application
+ * that owns the whole device-memory pool and gives a stage nothing but its buffers; code on a latency-critical
+ * path where cudaMalloc / cudaFree are banned because they synchronise the whole device; a process on a GPU whose
+ * memory another framework's caching allocator has already claimed, so that a fresh cudaMalloc would fail.
+ * bits_count_static serves them: same result as bits_count (Algorithm 2), same kernels in the
+ * same order, but the scratch is an array of BITS_STATIC_SCRATCH_BYTES that is part of the library's device image.
+ * The call makes no cudaMalloc / cudaFree and no CUDA call that allocates (it also runs with the "profile" event
+ * timers paused, because those create events); the caller passes inputs and the output only.
+ *
+ * Cost and limit: every GPU on which the library is used holds those BITS_STATIC_SCRATCH_BYTES (32 MiB) from the
+ * moment the library's device code is loaded there until the process ends, whether or not this function is ever
+ * called.  The problem must fit: bits_workspace_bytes(BITS_FN_COUNT, n_a, n_b, 0, 0, flags) <=
+ * BITS_STATIC_SCRATCH_BYTES -- e.g. 10^6 x 10^6 intervals (25.7 MB) fits, 2*10^6 x 10^6 does not.  A larger problem
+ * is refused with BITS_ERR_STATIC_LIMIT before anything is enqueued; nothing is truncated.
+ *
+ * Set-up: the first call on each device asks the CUDA runtime for the array's device address
+ * (cudaGetSymbolAddress, with that device current) and keeps it; the return code is checked (BITS_ERR_CUDA).
+ * Make that first call per device outside any stream capture.
+ *
+ * Sharing: there is ONE array per device and every call uses it, from whichever host thread or stream.  Two calls
+ * whose GPU work overlaps in time (different streams, or different threads without ordering between them) race
+ * on it and give undefined counts; calls enqueued one after the other on the same stream are safe.  The array
+ * keeps what the last call left there; each call clears on `stream` whatever it needs zeroed before use.
+ *
+ * Arguments, flags, errors and synchronisation otherwise as bits_count. */
+#define BITS_STATIC_SCRATCH_BYTES (32u << 20)
+int bits_count_static(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
+                      const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
+                      uint32_t flags, uint64_t* total_out, void* stream);
 
 /* Decision problem (PAPER.md:47, sub-problem 1; :91): *any_out = 1 if at least one interval of A
  * intersects an interval of B, else 0 (dev uint32[1]).  Same inputs, workspace (BITS_FN_COUNT) and

@@ -32,6 +32,7 @@ _SIGNATURES = {
     "bits_host_staging_bytes": (C.c_size_t, [C.c_int, C.c_uint64, C.c_uint64, C.c_uint32]),
     "bits_count": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t,
                              _u64p, _vp]),
+    "bits_count_static": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _u64p, _vp]),
     "bits_decide": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t, _u32p, _vp]),
     "bits_enumerate": (C.c_int, [_u32p, _u32p, C.c_uint64, _u32p, _u32p, C.c_uint64, C.c_uint32, _vp, C.c_size_t, _u32p, _u32p,
                                  C.c_uint64, _u64p, _vp]),
@@ -190,6 +191,25 @@ def count(a_start, a_end, b_start, b_end, flags: int = 0, workspace=None, total_
     _chk(lib().bits_count(_dev_u32(a_start, "a_start"), _dev_u32(a_end, "a_end"), n_a,
                           _dev_u32(b_start, "b_start"), _dev_u32(b_end, "b_end"), n_b, flags,
                           ws.data_ptr(), ws.numel(), out.data_ptr(), _stream()))
+    return out
+
+
+STATIC_SCRATCH_BYTES = 32 << 20     # BITS_STATIC_SCRATCH_BYTES of include/bits.h
+
+
+def count_static(a_start, a_end, b_start, b_end, flags: int = 0, total_out=None) -> torch.Tensor:
+    """bits_count_static -> device int64[1] tensor holding the uint64 total (valid after stream sync).
+
+    bits_count for callers that cannot allocate a workspace (a stage inside an application that owns all device
+    memory, a path on which cudaMalloc is banned, a GPU whose memory is already claimed): the scratch is a 32 MiB
+    array built into the library, so the problem must satisfy workspace_bytes(FN_COUNT, n_a, n_b) <=
+    STATIC_SCRATCH_BYTES (else BitsError with status 9).  Pass `total_out` (int64[1], device) and this wrapper
+    allocates nothing either.  One array per device: calls that overlap on the GPU race; calls on one stream do not."""
+    n_a, n_b = a_start.numel(), b_start.numel()
+    out = total_out if total_out is not None else torch.empty(1, dtype=torch.int64, device=a_start.device)
+    _chk(lib().bits_count_static(_dev_u32(a_start, "a_start"), _dev_u32(a_end, "a_end"), n_a,
+                                 _dev_u32(b_start, "b_start"), _dev_u32(b_end, "b_end"), n_b, flags,
+                                 out.data_ptr(), _stream()))
     return out
 
 

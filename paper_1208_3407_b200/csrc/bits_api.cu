@@ -1283,6 +1283,41 @@ static int stage_in(const HostStage& h, const uint32_t* a_start, const uint32_t*
   return BITS_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Built-in scratch for bits_count_static (bits.h): one fixed array that lives in the library's own device image,
+// so the counting path can run for a caller that has no way to hand over a workspace.  Every CUDA context that
+// loads this library carries these BITS_STATIC_SCRATCH_BYTES until the process (or the context) ends.
+//
+// In host code the name `g_static_scratch` is only the host-side handle of the symbol -- it is NOT a device
+// address and must never be given to a kernel or a cudaMemsetAsync.  The address the device sees comes from
+// cudaGetSymbolAddress, asked once per device while that device is current, and kept.
+static __device__ __align__(256) unsigned char g_static_scratch[BITS_STATIC_SCRATCH_BYTES];
+
+static int static_scratch_address(void** out) {
+  constexpr int kMaxDevices = 64;
+  static std::atomic<void*> addr_on[kMaxDevices];     // zero-initialised; one slot per device ordinal
+  int device = 0;
+  BITS_CUDA_TRY(cudaGetDevice(&device));
+  const bool tracked = device >= 0 && device < kMaxDevices;
+  void* p = tracked ? addr_on[device].load(std::memory_order_acquire) : nullptr;
+  if (!p) {
+    // first call on this device (or a device ordinal past the table: asked every time, which is cheap)
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || p == nullptr) { (void)cudaGetLastError(); return BITS_ERR_CUDA; }
+    if (tracked) addr_on[device].store(p, std::memory_order_release);
+  }
+  *out = p;
+  return BITS_OK;
+}
+
+// The per-kernel event timers create CUDA events on demand (ProfScope); a call that promises to allocate nothing
+// runs with them switched off and puts the caller's setting back afterwards.
+struct ProfilerPause {
+  bool was;
+  ProfilerPause() : was(g_prof.on) { g_prof.on = false; }
+  ~ProfilerPause() { g_prof.on = was; }
+};
+
 }  // namespace bits
 
 using namespace bits;
@@ -1317,6 +1352,23 @@ int bits_count(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, con
                uint64_t* total_out, void* stream) {
   return count_impl(a_start, a_end, n_a, b_start, b_end, n_b, flags, workspace, workspace_bytes, BITS_FN_COUNT,
                     nullptr, total_out, static_cast<cudaStream_t>(stream));
+}
+
+int bits_count_static(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
+                      const uint32_t* b_end, uint64_t n_b, uint32_t flags, uint64_t* total_out, void* stream) {
+  // argument errors first, exactly as bits_count reports them (no CUDA call yet)
+  BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
+  if (!total_out) return BITS_ERR_NULL;
+  // the limit: the scratch this problem needs must fit the built-in array
+  if (make_layout(nullptr, BITS_FN_COUNT, n_a, n_b, 0, 0).bytes > (size_t)BITS_STATIC_SCRATCH_BYTES) return BITS_ERR_STATIC_LIMIT;
+  void* scratch = nullptr;
+  BITS_TRY(static_scratch_address(&scratch));   // device address of the array on the current device (set up on first use)
+  ProfilerPause no_event_creation;
+  // Same kernels, same order as bits_count; only the scratch pointer differs.  count_impl clears every word of the
+  // scratch that must start at zero (sort bookkeeping, query histogram, validation flag) on `stream` before the first
+  // kernel reads it, so whatever the previous call left in the array does not matter.
+  return count_impl(a_start, a_end, n_a, b_start, b_end, n_b, flags, scratch, (size_t)BITS_STATIC_SCRATCH_BYTES,
+                    BITS_FN_COUNT, nullptr, total_out, static_cast<cudaStream_t>(stream));
 }
 
 int bits_decide(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, const uint32_t* b_start,
@@ -1577,6 +1629,7 @@ const char* bits_strerror(int status) {
     case BITS_ERR_FLAGS: return "unknown flag, option, fn, which or tail";
     case BITS_ERR_MALFORMED: return "malformed interval (start > end)";
     case BITS_ERR_CUDA: return "CUDA error (or no CUDA device)";
+    case BITS_ERR_STATIC_LIMIT: return "problem too large for the built-in scratch of bits_count_static (BITS_STATIC_SCRATCH_BYTES); use bits_count with a workspace";
     default: return "unknown status";
   }
 }
