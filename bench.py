@@ -388,6 +388,24 @@ def secondary_workloads(device, peak_gbs):
     out["cfg1_tiny_permuteB_10000_rounds"] = {"mc_rounds_per_s": R1 / (med * 1e-3), "ms_median": med, "ms_min": mn,
                                               "two_launch_path_rounds_per_s": R1 / (med2 * 1e-3),
                                               "same_counts_as_two_launch_path": bool(torch.equal(ref1, rc1))}
+    # a re-placed set that fits one block (6,000 intervals), a large A (1e6) and few rounds: round slicing / warm-up calls.
+    # The one-block-per-round kernel would rank all of A on 4 SMs; the library takes the two-launch path instead.
+    wf = W.make_config(5, scale=0.0006)
+    wa = W.make_config(4, scale=0.1)
+    dfr = [to_dev(x, device) for x in (wa.a_start, wa.a_end, wf.b_start, wf.b_end)]
+    wsf = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, wa.n_a, wf.n_b, 24, 1), dtype=torch.uint8, device=device)
+    rcf = torch.empty(4, dtype=torch.int64, device=device)
+    runf = lambda: bits.mc_rounds(*dfr, wf.chrom_offsets, 1, wf.mc_seed, 0, 4, workspace=wsf, observed_out=obs, round_counts_out=rcf)
+    medf, _ = time_device(runf, 5)
+    reff = rcf.clone()
+    bits.set_option("mc_small", 2)
+    try:
+        medf2, _ = time_device(runf, 3, warmup=1)
+    finally:
+        bits.set_option("mc_small", 1)
+    out["small_b_large_a_4_rounds"] = {"n_a": wa.n_a, "n_b": wf.n_b, "ms_median_call": medf, "one_block_per_round_ms_median_call": medf2,
+                                       "same_counts": bool(torch.equal(reff, rcf))}
+    del dfr, wsf
     # config 5's recipe at the smaller sizes of the paper's Table 1 (1e5 and 1e6 re-placed intervals):
     # one round does not fill the GPU there, so several rounds share a launch pair (gridDim.y = rounds)
     sizes = {}
@@ -733,7 +751,9 @@ def run_study(args):
     reps = 1 if args.once else 8
     w = W.make_config(4, scale=args.scale)
     d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    bits.set_option("count_binned", 1)                     # (sized for the design that needs the most: the query lists)
     ws = torch.empty(bits.workspace_bytes(bits.FN_COUNT_PER_INTERVAL, w.n_a, w.n_b), dtype=torch.uint8, device=device)
+    bits.set_option("count_binned", -1)
     counts = torch.empty(w.n_a, dtype=torch.int32, device=device)
     total = torch.empty(1, dtype=torch.int64, device=device)
     out = {"study": args.study, "workload": w.name, "n_a": w.n_a, "n_b": w.n_b, "calls_per_design": reps, "designs": {}}

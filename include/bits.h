@@ -89,6 +89,10 @@ enum {
  * BITS_FN_SORT n_b is the key count (n_a ignored).  Add bits_host_staging_bytes for *_host.
  * The size is NOT monotone in the set sizes (a small re-placed set gets room for several rounds per
  * launch): size a workspace that is shared between calls by the maximum over the calls.
+ * BITS_FN_COUNT / COUNT_PER_INTERVAL: four key buffers of n_b plus sort bookkeeping (about 19 bytes per interval
+ * of B); only where the call can bin the queries by B's buckets -- n_a >= 2^20 and n_b >= 3 * 2^20, `flags` without
+ * BITS_B_SORTED -- another 8 (COUNT) or 12 (COUNT_PER_INTERVAL) bytes per query.  Pass the flags the call will get;
+ * the study knobs count_binned / sort_msd (bits_set_option) change this rule, so size after setting them.
  * Returns 0 for an unknown fn. */
 size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which,
                             uint32_t flags);
@@ -129,8 +133,9 @@ int bits_count(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
  * Cost and limit: every GPU on which the library is used holds those BITS_STATIC_SCRATCH_BYTES (32 MiB) from the
  * moment the library's device code is loaded there until the process ends, whether or not this function is ever
  * called.  The problem must fit: bits_workspace_bytes(BITS_FN_COUNT, n_a, n_b, 0, 0, flags) <=
- * BITS_STATIC_SCRATCH_BYTES -- e.g. 10^6 x 10^6 intervals (25.7 MB) fits, 2*10^6 x 10^6 does not.  A larger problem
- * is refused with BITS_ERR_STATIC_LIMIT before anything is enqueued; nothing is truncated.
+ * BITS_STATIC_SCRATCH_BYTES -- about 19 bytes per interval of B, so up to about 1.75 million intervals in B with any
+ * number of queries (10^6 x 10^6 intervals take 17.9 MiB; n_b = 2*10^6 does not fit).  A larger problem is refused
+ * with BITS_ERR_STATIC_LIMIT before anything is enqueued; nothing is truncated.
  *
  * Set-up: the first call on each device asks the CUDA runtime for the array's device address
  * (cudaGetSymbolAddress, with that device current) and keeps it; the return code is checked (BITS_ERR_CUDA).
@@ -195,8 +200,9 @@ int bits_count_per_interval(const uint32_t* a_start, const uint32_t* a_end, uint
  * Synchronisation: `stream` is synchronised once before the first round (the longest span of the
  * permuted set is checked against the longest chromosome: BITS_ERR_NO_PLACEMENT) and, with
  * BITS_PERMUTE_B and more than 8,188 re-placed intervals, once more per (at most) 4,096 rounds: the
- * overflow flags of the fused rounds are read back; a flagged round is redone by the general path.  After such a redo the "sorted arrays of the last
- * round" (bits_workspace_sorted_offset) are those of the round that was redone last. */
+ * overflow flags of the fused rounds are read back; a flagged round is redone by the general path.  The "sorted
+ * arrays of the last round" (bits_workspace_sorted_offset) are those of round round_begin + n_rounds - 1 either way:
+ * if a redo overwrote them, the last round is done once more by the general path. */
 int bits_mc_rounds(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
                    const uint32_t* b_start, const uint32_t* b_end, uint64_t n_b,
                    const uint32_t* chrom_offsets, uint32_t n_chrom, int which, uint64_t seed,

@@ -203,7 +203,7 @@ def count_static(a_start, a_end, b_start, b_end, flags: int = 0, total_out=None)
     bits_count for callers that cannot allocate a workspace (a stage inside an application that owns all device
     memory, a path on which cudaMalloc is banned, a GPU whose memory is already claimed): the scratch is a 32 MiB
     array built into the library, so the problem must satisfy workspace_bytes(FN_COUNT, n_a, n_b) <=
-    STATIC_SCRATCH_BYTES (else BitsError with status 9).  Pass `total_out` (int64[1], device) and this wrapper
+    STATIC_SCRATCH_BYTES -- up to about 1.75 million intervals in B, any number of queries (else BitsError with status 9).  Pass `total_out` (int64[1], device) and this wrapper
     allocates nothing either.  One array per device: calls that overlap on the GPU race; calls on one stream do not."""
     n_a, n_b = a_start.numel(), b_start.numel()
     out = total_out if total_out is not None else torch.empty(1, dtype=torch.int64, device=a_start.device)
@@ -374,9 +374,9 @@ def screen(tracks, chrom_offsets, seed: int, n_rounds: int, round_begin: int = 0
 
 
 def host_workspace(fn: int, n_a: int, n_b: int, n_chrom: int = 0, which: int = 0, n_rounds: int = 0,
-                   device="cuda:0") -> torch.Tensor:
+                   device="cuda:0", flags: int = 0) -> torch.Tensor:
     """Device workspace big enough for the *_host variant of `fn`."""
-    nbytes = workspace_bytes(fn, n_a, n_b, n_chrom, which) + host_staging_bytes(fn, n_a, n_b, n_rounds)
+    nbytes = workspace_bytes(fn, n_a, n_b, n_chrom, which, flags) + host_staging_bytes(fn, n_a, n_b, n_rounds)
     return torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
 
 

@@ -40,7 +40,7 @@ struct Options {
   int64_t count_binned = -1;       // count path: 1 = queries binned by B's buckets and searched out of shared memory (binned_count.cuh), 0 = bucket index + count_kernel, -1 = by size
   int64_t mc_a_rounds_per_block = 4;   // PERMUTE_A rounds (and the sort-free variant): rounds a block serves for its query tile
   int64_t mc_batch = 1;            // PERMUTE_B fused rounds of small sets: 1 = several rounds per launch pair (gridDim.y), 0 = one
-  int64_t mc_small = 1;            // PERMUTE_B rounds of a set that fits one block's shared memory: 1 = one block per round (mc_small.cuh)
+  int64_t mc_small = 1;            // PERMUTE_B rounds of a set that fits one block's shared memory: 1 = one block per round (mc_small.cuh) when the rounds fill the GPU, 2 = always, 0 = never
   int64_t mc_shift_bias = 0;       // PERMUTE_B fused rounds: added to the bin width (log2) the host picked; > 0 overflows bins on purpose (tests)
   int64_t grid_mult = 8;           // grid-stride kernels launch min(needed, 148 * grid_mult) blocks
 };
@@ -249,7 +249,15 @@ static inline uint32_t tile_size_cfg(uint64_t n) { return tile_size_for(n, (uint
 // the workspace is sized for the shape with the most tiles, whatever shape a call ends up using
 static inline uint32_t max_tiles_for(uint64_t n) { return (uint32_t)ceil_div(n, tile_size_cfg<mct::TileCfg2x512>(n)); }
 
-static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which) {
+// The count path bins the queries by B's buckets (binned_count.cuh) when both sets are large, B is not already sorted
+// and the MSD sort is in use; knob count_binned forces it on (> 0) or off (0).  The same rule sizes the workspace: the
+// query lists (8-12 bytes per query) are carved only for calls that can take that path.
+static inline bool count_can_bin(uint32_t flags) { return g_opt.sort_msd != 0 && !(flags & BITS_B_SORTED); }
+static inline bool count_bins_queries(uint64_t n_a, uint64_t n_b, uint32_t flags) {
+  return count_can_bin(flags) && (g_opt.count_binned > 0 || (g_opt.count_binned < 0 && n_a >= (1u << 20) && n_b >= (3u << 20)));
+}
+
+static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which, uint32_t flags = 0) {
   Layout L;
   Carver c(ws);
   L.small.carve(c, n_chrom);
@@ -257,6 +265,7 @@ static Layout make_layout(void* ws, int fn, uint64_t n_a, uint64_t n_b, uint32_t
     case BITS_FN_COUNT:
     case BITS_FN_COUNT_PER_INTERVAL:
       L.b.carve(c, n_b, true);
+      if (!count_bins_queries(n_a, n_b, flags)) break;     // (L.ql stays null: the index path needs no query lists)
       L.ql.q_end = c.take<uint32_t>(n_a + 4);
       L.ql.q_start = c.take<uint32_t>(n_a + 4);
       L.ql.q_idx = c.take<uint32_t>(fn == BITS_FN_COUNT_PER_INTERVAL ? n_a + 4 : 4);
@@ -389,9 +398,10 @@ static int launch_histogram(const uint32_t* k0, const uint32_t* k1, uint32_t* h0
   h.n = n;
   h.run_if[0] = run_if; h.run_if[1] = run_if ? run_if + (n_arrays > 1 ? 1 : 0) : nullptr;
   ProfScope prof(kClsHist, st);
-  // (a gated launch is almost always skipped: fewer blocks to start and retire)
+  // (a gated launch gets the same grid as an ungated one: when the gate opens -- the MSD sort fell back on a
+  // clustered set -- this is the whole job, and retiring the blocks of a closed gate costs well under a microsecond)
   const int grid = grid_for(ceil_div(n, 4), 512);
-  launch_pdl(rs::histogram_kernel, dim3(run_if && grid > 2 * kSMs ? 2 * kSMs : grid, n_arrays), 512, 0, st, h);
+  launch_pdl(rs::histogram_kernel, dim3(grid, n_arrays), 512, 0, st, h);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -566,8 +576,10 @@ static int launch_build_index(const SortCtx& c, cudaStream_t st, const uint32_t*
   const uint64_t blocks = ceil_div(threads, 256);
   ia.total = blocks * 256;
   ProfScope prof(kClsIndex, st);
-  // (a gated launch is almost always skipped: fewer blocks to start and retire)
-  launch_pdl(build_index_kernel, dim3((unsigned)(run_if && blocks > 2u * kSMs ? 2u * kSMs : blocks), 2), 256, 0, st, ia);
+  // (a gated launch is almost always skipped, so it is capped like the grid-stride kernels -- 148 * grid_mult blocks,
+  // which fill the GPU when the gate does open -- rather than given one block per 1,024 keys)
+  const uint64_t gate_cap = (uint64_t)kSMs * (uint64_t)g_opt.grid_mult;
+  launch_pdl(build_index_kernel, dim3((unsigned)(run_if && blocks > gate_cap ? gate_cap : blocks), 2), 256, 0, st, ia);
   BITS_LAUNCH_CHECK();
   return BITS_OK;
 }
@@ -598,7 +610,7 @@ static int launch_count(const uint32_t* a_start, const uint32_t* a_end, uint32_t
   const SortedSet s0 = sorted_set(b, 0), s1 = sorted_set(b, 1);
   unsigned long long* tot = reinterpret_cast<unsigned long long*>(total);
   const int sv = (int)g_opt.search_variant;
-#define BITS_COUNT_LAUNCH(V, S) launch_pdl(count_kernel<V, S>, run_if && grid > 2 * kSMs ? 2 * kSMs : grid, 256, 0, st, a_start, a_end, n_a, s0, s1, counts, tot, run_if)
+#define BITS_COUNT_LAUNCH(V, S) launch_pdl(count_kernel<V, S>, grid, 256, 0, st, a_start, a_end, n_a, s0, s1, counts, tot, run_if)
   if (vec) {
     if (sv == kSearchPlain) BITS_COUNT_LAUNCH(true, kSearchPlain);
     else if (sv == kSearchStaged) BITS_COUNT_LAUNCH(true, kSearchStaged);
@@ -677,7 +689,7 @@ static int count_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n
   BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
   if (fn == BITS_FN_COUNT && !total_out) return BITS_ERR_NULL;
   if (fn == BITS_FN_COUNT_PER_INTERVAL && n_a && !counts_out) return BITS_ERR_NULL;
-  const Layout L = make_layout(ws, fn, n_a, n_b, 0, 0);
+  const Layout L = make_layout(ws, fn, n_a, n_b, 0, 0, flags);
   if (!ws_ok(ws, ws_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
   if (flags & BITS_VALIDATE)
     BITS_TRY(validate_inputs(a_start, a_end, (uint32_t)n_a, b_start, b_end, (uint32_t)n_b, L.small.bad, st));
@@ -691,8 +703,7 @@ static int count_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n
   BITS_TRY(reset_sort_ctx(L.b, st));
   // Large query sets against a large B: queries binned by B's buckets, every bucket searched out of shared
   // memory (binned_count.cuh); needs the MSD sort's plan.  The index path behind it runs only if the sort fell back.
-  const bool can_bin = g_opt.sort_msd != 0 && !(flags & BITS_B_SORTED);
-  const bool binned = can_bin && (g_opt.count_binned > 0 || (g_opt.count_binned < 0 && n_a >= (1u << 20) && n_b >= (3u << 20)));
+  const bool binned = count_bins_queries(n_a, n_b, flags);   // (the rule that carved L.ql)
   if (!binned) {
     BITS_TRY(setup_searched_set(L.b, b_start, b_end, flags, &epoch, st));
     return launch_count(a_start, a_end, (uint32_t)n_a, L.b, counts_out, total_out, st);
@@ -882,7 +893,11 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     }
     return BITS_OK;
   }
-  if (g_opt.mc_small != 0 && n_b <= (uint64_t)mcs::kMaxKeys && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0) {
+  // (each block ranks all n_a sorted queries on its own: with fewer rounds than the GPU has SMs and a large A -- round
+  // slicing, warm-up calls -- a launch would run on a handful of SMs for milliseconds; such calls take the two-launch
+  // path below, which spreads the queries of ONE round over all blocks.  Knob mc_small = 2 takes the path regardless.)
+  const bool small_fills_gpu = n_rounds >= (uint32_t)kSMs || n_a * (uint64_t)n_rounds <= (1ull << 22) || g_opt.mc_small == 2;
+  if (g_opt.mc_small != 0 && small_fills_gpu && n_b <= (uint64_t)mcs::kMaxKeys && g_opt.mc_fused != 0 && g_opt.mc_sorted_queries != 0) {
     // a set that fits one block's shared memory: one block per round, the grid strides over the rounds (mc_small.cuh)
     BITS_TRY(msd_configure());
     mcs::SmallArgs m;
@@ -1098,11 +1113,20 @@ static int mc_impl(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a,
     h_flags.assign(chunk, 0);
     BITS_CUDA_TRY(cudaMemcpyAsync(h_flags.data(), L.round_flags, sizeof(uint32_t) * chunk, cudaMemcpyDeviceToHost, st));
     BITS_CUDA_TRY(cudaStreamSynchronize(st));
+    uint32_t last_redone = 0xffffffffu;
     for (uint32_t j = 0; j < chunk; ++j) {
       const bool forced = g_opt.mc_force_redo > 0 && (done + j) % (uint32_t)g_opt.mc_force_redo == 0;
       if (!h_flags[j] && !forced) continue;
       BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out + done + j, 0, sizeof(uint64_t), st));
       BITS_TRY(general_round(done + j));
+      last_redone = done + j;
+    }
+    // general_round sorts into the buffers bits_workspace_sorted_offset points to.  If a redo in the call's final
+    // chunk left another round's arrays there, the last round is done once more by the general path (same count,
+    // bit for bit), so that the workspace holds B_S and B_E of the LAST round whatever the overflow flags were.
+    if (done + chunk == n_rounds && last_redone != 0xffffffffu && last_redone != n_rounds - 1) {
+      BITS_CUDA_TRY(cudaMemsetAsync(round_counts_out + (n_rounds - 1), 0, sizeof(uint64_t), st));
+      BITS_TRY(general_round(n_rounds - 1));
     }
     done += chunk;
   }
@@ -1328,7 +1352,7 @@ size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom
   (void)flags;
   if (fn < BITS_FN_COUNT || fn > BITS_FN_ENUMERATE) return 0;
   if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return 0;
-  return make_layout(nullptr, fn, n_a, n_b, n_chrom, which).bytes;
+  return make_layout(nullptr, fn, n_a, n_b, n_chrom, which, flags).bytes;
 }
 
 int bits_workspace_sorted_offset(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which, int array,
@@ -1360,7 +1384,7 @@ int bits_count_static(const uint32_t* a_start, const uint32_t* a_end, uint64_t n
   BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
   if (!total_out) return BITS_ERR_NULL;
   // the limit: the scratch this problem needs must fit the built-in array
-  if (make_layout(nullptr, BITS_FN_COUNT, n_a, n_b, 0, 0).bytes > (size_t)BITS_STATIC_SCRATCH_BYTES) return BITS_ERR_STATIC_LIMIT;
+  if (make_layout(nullptr, BITS_FN_COUNT, n_a, n_b, 0, 0, flags).bytes > (size_t)BITS_STATIC_SCRATCH_BYTES) return BITS_ERR_STATIC_LIMIT;
   void* scratch = nullptr;
   BITS_TRY(static_scratch_address(&scratch));   // device address of the array on the current device (set up on first use)
   ProfilerPause no_event_creation;
@@ -1377,7 +1401,7 @@ int bits_decide(const uint32_t* a_start, const uint32_t* a_end, uint64_t n_a, co
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   BITS_TRY(check_common(a_start, a_end, n_a, b_start, b_end, n_b, flags));
   if (!any_out) return BITS_ERR_NULL;
-  const Layout L = make_layout(workspace, BITS_FN_COUNT, n_a, n_b, 0, 0);
+  const Layout L = make_layout(workspace, BITS_FN_COUNT, n_a, n_b, 0, 0, flags);
   if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
   if (flags & BITS_VALIDATE)
     BITS_TRY(validate_inputs(a_start, a_end, (uint32_t)n_a, b_start, b_end, (uint32_t)n_b, L.small.bad, st));
@@ -1605,7 +1629,7 @@ int bits_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "count_binned")) { if (value < -1 || value > 1) return BITS_ERR_FLAGS; g_opt.count_binned = value; return BITS_OK; }
   if (!strcmp(name, "mc_a_rounds_per_block")) { if (value < 1 || value > 64) return BITS_ERR_FLAGS; g_opt.mc_a_rounds_per_block = value; return BITS_OK; }
   if (!strcmp(name, "mc_batch")) { g_opt.mc_batch = value != 0; return BITS_OK; }
-  if (!strcmp(name, "mc_small")) { g_opt.mc_small = value != 0; return BITS_OK; }
+  if (!strcmp(name, "mc_small")) { if (value < 0 || value > 2) return BITS_ERR_FLAGS; g_opt.mc_small = value; return BITS_OK; }
   if (!strcmp(name, "mc_shift_bias")) { if (value < 0 || value > 8) return BITS_ERR_FLAGS; g_opt.mc_shift_bias = value; return BITS_OK; }
   if (!strcmp(name, "sort_msd")) { g_opt.sort_msd = value; return BITS_OK; }
   if (!strcmp(name, "mc_sorted_queries")) { g_opt.mc_sorted_queries = value; return BITS_OK; }

@@ -48,9 +48,15 @@ def test_workspace_sizes():
     mc_a = w(bits.FN_MC_ROUNDS, 10_000, 1_000_000, 24, bits.PERMUTE_A)
     mc_b = w(bits.FN_MC_ROUNDS, 10_000, 1_000_000, 24, bits.PERMUTE_B)
     assert mc_b > mc_a > w(bits.FN_SORT, 0, 1_000_000)
-    # the count workspaces also hold the queries in bucket order (12 bytes per query with per-interval counts, 8 without)
-    assert w(bits.FN_COUNT_PER_INTERVAL, 1_000_000, 1_000_000) - w(bits.FN_COUNT, 1_000_000, 1_000_000) >= 4 * 1_000_000 - 4096
-    assert w(bits.FN_COUNT, 1_000_000, 1_000_000) - w(bits.FN_COUNT, 0, 1_000_000) >= 8 * 1_000_000
+    # where the count path can bin the queries by B's buckets (both sets large, B not already sorted) the workspace also
+    # holds the queries in bucket order: 12 bytes per query with per-interval counts, 8 without ...
+    na, nb = 1 << 20, 3 << 20
+    assert w(bits.FN_COUNT_PER_INTERVAL, na, nb) - w(bits.FN_COUNT, na, nb) >= 4 * na - 4096
+    assert w(bits.FN_COUNT, na, nb) - w(bits.FN_COUNT, 0, nb) >= 8 * na
+    # ... and nowhere else: smaller sets and BITS_B_SORTED calls take the index path, whose workspace does not grow with n_a
+    assert w(bits.FN_COUNT, na, nb, 0, 0, bits.B_SORTED) == w(bits.FN_COUNT, 0, nb)
+    assert w(bits.FN_COUNT_PER_INTERVAL, 10_000_000, 1_000_000) == w(bits.FN_COUNT, 0, 1_000_000)
+    assert w(bits.FN_COUNT, na - 1, nb) == w(bits.FN_COUNT, 0, nb)
     assert w(bits.FN_MC_ROUNDS, 0, 0, 1, 0) > 0
     assert bits.host_staging_bytes(bits.FN_MC_ROUNDS, 1000, 1000, 100) >= 4 * 4 * 1000 + 8 * 100
 

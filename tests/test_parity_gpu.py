@@ -206,6 +206,11 @@ def test_count_binned_queries_special_cases():
         check_counts(a_s[:20_000], a_e[:20_000], b4_s, b4_e)
     finally:
         bits.set_option("count_binned", -1)
+    # (6) the same fallback at a size where the library picks the binned design itself and the gated launches behind it
+    # (histogram, sort passes, index, count) are the whole job: 3.3M intervals of which 60,000 start inside one bin, 1.3M queries
+    b6_s = np.concatenate([rng.integers(0, G, 3_240_000), cs]); b6_e = b6_s + rng.integers(0, 2000, b6_s.size)
+    q6 = rng.integers(0, G, 1_300_000)
+    check_counts(q6, q6 + rng.integers(0, 4000, q6.size), b6_s, b6_e)
 
 
 
@@ -749,6 +754,52 @@ def test_mc_permute_b_small_sets_one_block_per_round():
     obs1, rc1 = bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, 1, 1, 0, 30)
     sync()
     assert torch.equal(rc0, rc1) and torch.equal(obs0, obs1)
+
+
+def test_mc_permute_b_small_set_few_rounds_large_query_set():
+    """A re-placed set that fits one block, a large A and fewer rounds than SMs (round slicing, warm-up calls): the
+    one-block-per-round kernel would rank all of A on a handful of SMs, so the call takes the two-launch path; with
+    knob mc_small = 2 it takes the one-block path.  Both must give the oracle's integers."""
+    rng = np.random.default_rng(77)
+    off = W.genome_offsets(W.GENOME24_LENGTHS)
+    def draw(n, max_len):
+        c = rng.integers(0, 24, n); ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        st = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        return st.astype(np.uint32), (st + ln - 1).astype(np.uint32)
+    a_s, a_e = draw(1_500_000, 3000)
+    b_s, b_e = draw(6_000, 200_000)
+    _mc_b_case(a_s, a_e, b_s, b_e, off, 4, 7, 3, expect_fused=True)          # 3 rounds x 1.5M queries: two-launch path
+    bits.set_option("mc_small", 2)
+    try:
+        _mc_b_case(a_s, a_e, b_s, b_e, off, 4, 7, 3, expect_fused=False)     # forced: one block per round
+    finally:
+        bits.set_option("mc_small", 1)
+    _mc_b_case(a_s, a_e, b_s, b_e, off, 4, 7, 150, expect_fused=False)       # 150 rounds fill the GPU: one block per round
+
+
+def test_mc_permute_b_redo_leaves_the_last_rounds_arrays():
+    """A redo of an EARLIER round of the final chunk (forced here for rounds 0 and 2 of 4) sorts into the buffers that
+    hold 'the sorted arrays of the last round'; the library then puts the last round's arrays back.  With one round per
+    launch pair and with several rounds per launch pair."""
+    for k, scale in ((5, 0.02), (5, 0.6)):                       # 2e5 intervals: round batches; 6e6: one round per launch pair
+        w = W.make_config(k, scale=scale)
+        n_chrom = int(w.chrom_offsets.size - 1)
+        ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, 1), dtype=torch.uint8, device=DEV)
+        bits.set_option("mc_force_redo", 2)
+        try:
+            _, rc = bits.mc_rounds(dev(w.a_start), dev(w.a_end), dev(w.b_start), dev(w.b_end), w.chrom_offsets, 1, w.mc_seed, 0, 4,
+                                   workspace=ws)
+            sync()
+        finally:
+            bits.set_option("mc_force_redo", 0)
+        _, o_rc = oracle.mc_rounds(w.a_start, w.a_end, w.b_start, w.b_end, w.chrom_offsets, 1, w.mc_seed, 0, 4)
+        assert np.array_equal(host_u64(rc), o_rc)
+        b_s, b_e = bits.sorted_arrays_in_workspace(ws, bits.FN_MC_ROUNDS, w.n_a, w.n_b, n_chrom, 1)
+        spans = (w.b_end - w.b_start).astype(np.uint32)
+        o_s, o_e = oracle.place_round(spans, w.chrom_offsets, w.mc_seed, 3, 1)
+        assert np.array_equal(host_u32(b_s), oracle.sort_u32(o_s))
+        assert np.array_equal(host_u32(b_e), oracle.sort_u32(o_e))
 
 
 def test_mc_permute_b_redo_path_gives_the_same_counts():

@@ -44,11 +44,12 @@ def _ragged_case(seed, n_a, n_b, genome=3_000_000_000, max_len=5_000):
 def test_limit_and_argument_errors_are_reported_on_the_host():
     """No GPU needed: sizes and pointers are checked before the first CUDA call."""
     L = bits.lib()
-    # the limit is the size of the workspace bits_count would ask for
+    # the limit is the size of the workspace bits_count would ask for: about 19 bytes per interval of B
     assert bits.workspace_bytes(bits.FN_COUNT, 1_000_000, 1_000_000) <= bits.STATIC_SCRATCH_BYTES
-    assert bits.workspace_bytes(bits.FN_COUNT, 2_000_000, 1_000_000) > bits.STATIC_SCRATCH_BYTES
+    assert bits.workspace_bytes(bits.FN_COUNT, 50_000_000, 1_700_000) <= bits.STATIC_SCRATCH_BYTES
+    assert bits.workspace_bytes(bits.FN_COUNT, 1_000, 2_000_000) > bits.STATIC_SCRATCH_BYTES
     fake = 0x1000                                           # never dereferenced: the call is refused first
-    assert L.bits_count_static(fake, fake, 2_000_000, fake, fake, 1_000_000, 0, fake, 0) == 9
+    assert L.bits_count_static(fake, fake, 1_000, fake, fake, 2_000_000, 0, fake, 0) == 9
     assert L.bits_count_static(fake, fake, 10, fake, fake, 10_000_000, 0, fake, 0) == 9
     assert "BITS_STATIC_SCRATCH_BYTES" in bits.strerror(9)
     assert L.bits_count_static(fake, fake, 10, fake, fake, 10, 0, 0, 0) == 1          # total_out NULL
@@ -60,7 +61,7 @@ def test_limit_and_argument_errors_are_reported_on_the_host():
 @pytest.mark.gpu
 def test_static_scratch_count_equals_workspace_count_on_consecutive_calls():
     assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
-    w2 = W.make_config(2)                                   # 10^6 x 10^6: 25.7 MB of the 32 MiB array
+    w2 = W.make_config(2)                                   # 10^6 x 10^6: 17.9 MiB of the 32 MiB array
     cases = [
         (w2.a_start, w2.a_end, w2.b_start, w2.b_end),
         _ragged_case(11, 10_001, 70_001),                   # small, right after the big one: stale scratch all around it
@@ -119,7 +120,7 @@ def test_static_scratch_count_equals_workspace_count_on_consecutive_calls():
     assert e.value.status == 7
     big = torch.zeros(2_000_000, dtype=torch.int32, device=DEV)
     with pytest.raises(bits.BitsError) as e:
-        bits.count_static(big, big, on_dev[0][2], on_dev[0][3], total_out=outs[0])
+        bits.count_static(on_dev[0][0], on_dev[0][1], big, big, total_out=outs[0])
     assert e.value.status == 9
     # and the array still works after the refusals
     bits.count_static(*on_dev[1], total_out=outs[1])
