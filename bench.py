@@ -2,6 +2,7 @@
 """bench.py -- Monte Carlo rounds/s of the BITS hot path (place -> sort -> search -> reduce) on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 5] [--rounds R]
+    python bench.py --config 2|4          the counting configs as a line of their own (metric intervals_searched_per_s)
 
 Workload (config.workload): BASELINE.json configs[4], "Monte Carlo at scale with per-round sort":
 24-chromosome genome, A = 1e6 query intervals, B = 1e7 intervals re-placed with Philox and radix-
@@ -35,23 +36,52 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # Counters of the dominant kernels that only ncu can give (DRAM bytes, warp instructions, what bounds the kernel) live
-# in profiles/r2b_fused_ncu_counters.json, written from the committed `ncu --set full` capture together with the hash
-# of the kernel sources it was taken of (paper_1208_3407_b200.build.csrc_hash()).  They are reported only while that
-# hash is the one of the sources this run was built from; otherwise the line says "stale_capture".
-NCU_COUNTERS_FILE = os.path.join(ROOT, "profiles", "r2b_fused_ncu_counters.json")
+# in profiles/r3_fused_ncu_counters.json, written by paper_1208_3407_b200/ncu_counters.py in the same gpurun command as
+# the `ncu --set full` capture, together with the hash of the sources it was taken of (build.csrc_hash(): all of csrc/,
+# kernels and host launch geometry).  They are reported only while that hash is the one of the sources this run was
+# built from; otherwise the line says "stale_capture".
+NCU_COUNTERS_FILE = os.path.join(ROOT, "profiles", "r3_fused_ncu_counters.json")
 
 
-def ncu_counters():
-    """(counters by kernel, note) -- counters are {} when the capture is missing or belongs to other kernel sources."""
+# The same for the L2-bound kernels (config 3's PERMUTE_A rounds at the benchmarked 10,000 rounds per launch, the screen):
+# L2 sectors read per launch and the hit rate, from which other_workloads prints an l2_roofline.
+NCU_L2_COUNTERS_FILE = os.path.join(ROOT, "profiles", "r3_l2_ncu_counters.json")
+
+
+def ncu_counters(path=None):
+    """(counters by kernel, note) -- counters are {} when the capture is missing or belongs to other sources."""
     from paper_1208_3407_b200 import build as B
-    if not os.path.exists(NCU_COUNTERS_FILE):
+    path = path or NCU_COUNTERS_FILE
+    if not os.path.exists(path):
         return {}, "no capture file"
-    with open(NCU_COUNTERS_FILE) as f:
+    with open(path) as f:
         d = json.load(f)
     have = B.csrc_hash()
     if d.get("csrc_hash") != have:
-        return {}, f"stale_capture: {os.path.basename(NCU_COUNTERS_FILE)} was taken of csrc {d.get('csrc_hash')}, this build is {have}"
-    return d.get("kernels", {}), f"from {os.path.basename(NCU_COUNTERS_FILE)} (csrc {have}, workload {d.get('workload')})"
+        return {}, f"stale_capture: {os.path.basename(path)} was taken of csrc {d.get('csrc_hash')}, this build is {have}"
+    return d.get("kernels", {}), f"from {os.path.basename(path)} (csrc {have}, workload {d.get('workload')})"
+
+
+def kernel_counters(counters: dict, kname: str) -> dict:
+    """Counters of the kernel whose name (without namespace and template arguments) is kname."""
+    return next((v for k, v in sorted(counters.items()) if k.split("<")[0] == kname), {})
+
+
+def l2_roofline(kname: str, intervals_per_launch: float, intervals_per_s: float, gather_gsectors_per_s: float) -> dict:
+    """SURVEY 8(d), L2-bound search kernels: 32-byte sectors read from L2 per searched interval (ncu capture of the
+    kernel at the benchmarked shape) x the interval rate measured in this run, against the random-sector gather rate
+    measured in this run (probe/l2_probe.cu)."""
+    counters, note = ncu_counters(NCU_L2_COUNTERS_FILE)
+    kc = kernel_counters(counters, kname)
+    if not kc.get("l2_sectors_read"):
+        return {"kernel": kname, "ncu_counters": note if not counters else f"{kname} not in the capture"}
+    spi = kc["l2_sectors_read"] / intervals_per_launch
+    ach = spi * intervals_per_s / 1e9
+    return {"kernel": kname, "bound": "l2", "sectors_per_interval": spi, "achieved_gsectors_per_s": ach,
+            "peak": gather_gsectors_per_s, "unit": "Gsectors/s", "frac": ach / gather_gsectors_per_s if gather_gsectors_per_s else None,
+            "l2_hit_rate_pct": kc.get("l2_hit_rate_pct"), "l2_throughput_pct_under_ncu": kc.get("l2_throughput_pct"),
+            "dram_bytes_per_launch": kc.get("dram_bytes"), "ncu_counters": note,
+            "peak_source": "l2_yardsticks.l2_random_sector_gather_gsectors_per_s_80MB of this run"}
 
 
 N_SMS, SCHEDULERS_PER_SM = 148, 4
@@ -69,7 +99,7 @@ def parse_args():
     p.add_argument("--rounds", type=int, default=0, help="rounds per step (0 = the configuration's own count)")
     p.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                    help="bits_set_option knob for design studies (DESIGN.md section 10); results never change")
-    p.add_argument("--study", default=None, choices=["search", "count"],
+    p.add_argument("--study", default=None, choices=["search", "count", "screen"],
                    help="design studies instead of the bench line: 'search' = config 4 with every search design of the count "
                         "path + 100 rounds of config 3; 'count' = config 4's bits_count_per_interval only (the command the "
                         "ncu captures under profiles/ run); with --once every call runs once, without warm-up")
@@ -194,7 +224,24 @@ def run_reference(args):
     oracle.build()
     w = W.make_config(args.config, scale=args.scale)
     if w.which is None:
-        raise SystemExit("--impl reference times the Monte Carlo configs (1, 3, 5)")
+        # counting configs: a step is the oracle's whole call (std::sort of B's two key arrays + one ICOUNT per query + sum)
+        for _ in range(min(args.warmup, 1)):
+            oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end)
+        dt = time.perf_counter() - t0
+        value = w.n_a * args.steps / dt
+        print(json.dumps({
+            "impl": "reference", "metric": "intervals_searched_per_s", "value": value, "unit": "intervals/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+            "config": {"workload": w.name, "n_a": w.n_a, "n_b": w.n_b, "data_seed": w.spec.get("seed"), "scale": w.spec.get("scale", 1.0)},
+            "cpu_baseline": {"value": value, "unit": "intervals/s", "cores": 1, "kind": "oracle",
+                             "sample": "the whole call per step: std::sort of both key arrays of B + one ICOUNT per query + sum"},
+            "e2e": {"value": value, "unit": "intervals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "host_cores": os.cpu_count()}))
+        return 0
     r_sample = 1 if args.config == 5 else (args.rounds or 100)
     for i in range(args.warmup):
         oracle_marginal_rounds_per_s(w, w.which, i * r_sample, r_sample)
@@ -312,7 +359,48 @@ def library_yardsticks(device, w4, d4):
     return out
 
 
-def secondary_workloads(device, peak_gbs):
+def screen_workload(device, w, gather_gsectors=0.0):
+    """The many-pair screen on synthetic tracks (w = config 2, whose B the tracks are drawn from)."""
+    import torch
+    from paper_1208_3407_b200 import bits
+    # SURVEY 8(f).3: the paper's screen (PAPER.md:165-171: 159 tracks, 25,281 ordered pairs) on synthetic tracks of 1e5
+    # intervals drawn from config 2's recipe, as ONE bits_screen call (every track sorted and indexed once, all pairs and
+    # rounds in gridded launches); 20 of the paper's 10,000 rounds per pair, device time by CUDA events
+    K, n_t, R_s = 159, 100_000, 20
+    rng = np.random.default_rng(8)
+    idx = [rng.choice(w.n_b, n_t, replace=False) for _ in range(K)]
+    starts = to_dev(np.concatenate([w.b_start[i] for i in idx]), device)
+    ends = to_dev(np.concatenate([w.b_end[i] for i in idx]), device)
+    toff = np.arange(K + 1, dtype=np.uint64) * n_t
+    obs_s = torch.empty((K, K), dtype=torch.int64, device=device)
+    rc_s = torch.empty((K, K, R_s), dtype=torch.int64, device=device)
+    ws = torch.empty(int(bits.lib().bits_screen_workspace_bytes(toff.ctypes.data, K, 24)), dtype=torch.uint8, device=device)
+    run = lambda R: bits.screen_concat(starts, ends, toff, w.chrom_offsets, 1, R, workspace=ws, observed_out=obs_s,
+                                       round_counts_out=rc_s[:, :, :R].contiguous() if R != R_s else rc_s)
+    launches0 = bits.launch_count()
+    med0, _ = time_device(lambda: run(0), 2, warmup=1)               # setup + observed counts only
+    med, mn = time_device(lambda: run(R_s), 2, warmup=1)
+    per_call_launches = (bits.launch_count() - launches0) // 6
+    enr = bits.screen_enrichment(obs_s.cpu().numpy().view(np.uint64), rc_s.cpu().numpy().view(np.uint64))
+    rounds_ms = max(med - med0, 1e-6)
+    sectors_per_interval = 6.0      # two index words + four key sectors per ICOUNT (search.cuh rank_le x 2)
+    res = {
+        "tracks": K, "pairs": K * K, "intervals_per_track": n_t, "rounds_per_pair": R_s, "ms_median": med, "ms_min": mn,
+        "setup_and_observed_ms": med0, "launches_per_call": per_call_launches, "synchronisations_per_call": 1,
+        "pair_rounds_per_s": K * K * R_s / (rounds_ms * 1e-3),
+        "intervals_searched_per_s": K * K * R_s * n_t / (rounds_ms * 1e-3),
+        "l2_sectors_per_s_model": K * K * R_s * n_t * sectors_per_interval / (rounds_ms * 1e-3),
+        "paper_scale_estimate_s": {"pairs": K * K, "rounds": 10_000, "seconds": med0 * 1e-3 + rounds_ms * 1e-3 * 10_000 / R_s,
+                                   "paper": "9,069 min on one GPU of 2012 for 25,281 pairs x 10,000 rounds of the ENCODE/UCSC "
+                                            "tracks (PAPER.md:171; other data, other hardware: context only)"},
+        "enrichment_diag_mean": float(np.mean(np.diag(enr))),
+        "enrichment_offdiag_mean": float(np.mean(enr[~np.eye(K, dtype=bool)]))}
+    res["l2_roofline"] = l2_roofline("screen_kernel", float(K) * K * R_s * n_t, K * K * R_s * n_t / (rounds_ms * 1e-3), gather_gsectors)
+    return res
+
+
+
+def secondary_workloads(device, peak_gbs, gather_gsectors=0.0):
     """The other throughputs BASELINE.json's metric names, on their own configs (not the timed headline)."""
     import torch
     from paper_1208_3407_b200 import bits
@@ -369,7 +457,9 @@ def secondary_workloads(device, peak_gbs):
                                                  observed_out=obs, round_counts_out=rc), 5)
     out["cfg3_mc_permuteA_1e4x1M"] = {"mc_rounds_per_s": w.n_rounds / (med * 1e-3),
                                       "intervals_searched_per_s": w.n_rounds * w.n_a / (med * 1e-3),
-                                      "ms_median": med, "ms_min": mn}
+                                      "ms_median": med, "ms_min": mn,
+                                      "l2_roofline": l2_roofline("mc_permute_a_rounds_kernel", float(w.n_a) * min(w.n_rounds, 32768),
+                                                                 w.n_rounds * w.n_a / (med * 1e-3), gather_gsectors)}
     # config 1 (1,000 x 1,000, one chromosome): Monte Carlo rounds of a set that fits one block's shared memory
     # (mc_small.cuh: one block per round), beside the two-launch path on the same rounds
     w = W.make_config(1)
@@ -442,38 +532,7 @@ def secondary_workloads(device, peak_gbs):
     out["cfg2_enumerate"] = {"pairs": n_pairs, "pairs_per_s": n_pairs / (med * 1e-3), "ms_median": med, "ms_min": mn}
     med, mn = time_device(lambda: bits.decide(*d, workspace=ws), 5)
     out["cfg2_decide"] = {"ms_median": med, "ms_min": mn}
-    # the paper's screen (159 tracks, 25,281 ordered pairs) on synthetic tracks of 1e5
-    # intervals drawn from config 2's recipe, as ONE bits_screen call (every track sorted and indexed once, all pairs and
-    # rounds in gridded launches); 20 of the paper's 10,000 rounds per pair, device time by CUDA events
-    K, n_t, R_s = 159, 100_000, 20
-    rng = np.random.default_rng(8)
-    idx = [rng.choice(w.n_b, n_t, replace=False) for _ in range(K)]
-    starts = to_dev(np.concatenate([w.b_start[i] for i in idx]), device)
-    ends = to_dev(np.concatenate([w.b_end[i] for i in idx]), device)
-    toff = np.arange(K + 1, dtype=np.uint64) * n_t
-    obs_s = torch.empty((K, K), dtype=torch.int64, device=device)
-    rc_s = torch.empty((K, K, R_s), dtype=torch.int64, device=device)
-    ws = torch.empty(int(bits.lib().bits_screen_workspace_bytes(toff.ctypes.data, K, 24)), dtype=torch.uint8, device=device)
-    run = lambda R: bits.screen_concat(starts, ends, toff, w.chrom_offsets, 1, R, workspace=ws, observed_out=obs_s,
-                                       round_counts_out=rc_s[:, :, :R].contiguous() if R != R_s else rc_s)
-    launches0 = bits.launch_count()
-    med0, _ = time_device(lambda: run(0), 2, warmup=1)               # setup + observed counts only
-    med, mn = time_device(lambda: run(R_s), 2, warmup=1)
-    per_call_launches = (bits.launch_count() - launches0) // 6
-    enr = bits.screen_enrichment(obs_s.cpu().numpy().view(np.uint64), rc_s.cpu().numpy().view(np.uint64))
-    rounds_ms = max(med - med0, 1e-6)
-    sectors_per_interval = 6.0      # two index words + four key sectors per ICOUNT (search.cuh rank_le x 2)
-    out["screen_159_tracks_of_1e5"] = {
-        "tracks": K, "pairs": K * K, "intervals_per_track": n_t, "rounds_per_pair": R_s, "ms_median": med, "ms_min": mn,
-        "setup_and_observed_ms": med0, "launches_per_call": per_call_launches, "synchronisations_per_call": 1,
-        "pair_rounds_per_s": K * K * R_s / (rounds_ms * 1e-3),
-        "intervals_searched_per_s": K * K * R_s * n_t / (rounds_ms * 1e-3),
-        "l2_sectors_per_s_model": K * K * R_s * n_t * sectors_per_interval / (rounds_ms * 1e-3),
-        "paper_scale_estimate_s": {"pairs": K * K, "rounds": 10_000, "seconds": med0 * 1e-3 + rounds_ms * 1e-3 * 10_000 / R_s,
-                                   "paper": "9,069 min on one GPU of 2012 for 25,281 pairs x 10,000 rounds of the ENCODE/UCSC "
-                                            "tracks (PAPER.md:171; other data, other hardware: context only)"},
-        "enrichment_diag_mean": float(np.mean(np.diag(enr))),
-        "enrichment_offdiag_mean": float(np.mean(enr[~np.eye(K, dtype=bool)]))}
+    out["screen_159_tracks_of_1e5"] = screen_workload(device, w, gather_gsectors)
     return out
 
 
@@ -499,7 +558,7 @@ def run_b200(args):
 
     w = W.make_config(args.config, scale=args.scale)
     if w.which is None:
-        raise SystemExit("the timed headline is a Monte Carlo config (1, 3 or 5); counts are reported as extras")
+        return run_count_config(args, w, device, rank, world, dist)
     R = args.rounds or w.n_rounds
     from paper_1208_3407_b200 import shard
     r0, _ = shard.weak_slice(rank, R)                     # this rank's slice of the round space
@@ -580,7 +639,8 @@ def run_b200(args):
             launch_ms = timed[dom][0] / timed[dom][1]
             achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
             counters, counters_note = ncu_counters() if (args.config == 5 and args.scale == 1.0 and not args.opt) else ({}, "not the captured workload")
-            kc = counters.get(kname, {})
+            # (keys are kernel names with their template arguments; the one-round-per-launch instantiation `..., 0>` is the timed one)
+            kc = kernel_counters(counters, kname)
             roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                         "frac": achieved / peak,
                         "traffic": kc.get("dram_bytes"), "ncu_limiter": kc.get("limiter"), "ncu_counters": counters_note,
@@ -681,8 +741,8 @@ def run_b200(args):
         del hws, hp
 
     if rank == 0 and world == 1 and not args.no_extras:
-        line["other_workloads"] = secondary_workloads(device, peak)
         line["l2_yardsticks"] = l2_yardsticks(device)
+        line["other_workloads"] = secondary_workloads(device, peak, line["l2_yardsticks"]["l2_random_sector_gather_gsectors_per_s_80MB"])
         if w.which == 1:
             # SURVEY 8(f).1, reported BESIDE the headline: the sort-free variant of the same rounds
             # (count(A, B') = count(B', A): fresh B intervals searched against the once-sorted A; no B_S / B_E)
@@ -748,6 +808,10 @@ def run_study(args):
     for kv in args.opt:
         name, _, val = kv.partition("=")
         bits.set_option(name, int(val))
+    if args.study == "screen":      # the screen alone (one JSON object): the command the ncu capture of scr::screen_kernel runs
+        gather = 0.0 if args.once else l2_yardsticks(device)["l2_random_sector_gather_gsectors_per_s_80MB"]
+        print(json.dumps({"study": "screen", "screen_159_tracks_of_1e5": screen_workload(device, W.make_config(2), gather)}))
+        return 0
     reps = 1 if args.once else 8
     w = W.make_config(4, scale=args.scale)
     d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
@@ -797,6 +861,153 @@ def run_study(args):
         us = 1e3 * prof["mc_permute_a"][0] / prof["mc_permute_a"][1]
         out["cfg3_mc_permute_a_100_rounds_per_launch"] = {"kernel_us": us, "intervals_searched_per_s": R * w3.n_a / (us * 1e-6)}
     print(json.dumps(out))
+    return 0
+
+
+def run_count_config(args, w, device, rank, world, dist):
+    """`--config 2|4`: the counting configs as a full bench line.  A step is ONE bits_count_per_interval call (sort B_S and
+    B_E, two ranks per query, per-interval counts written, total reduced; Algorithm 2) on inputs resident
+    in HBM; metric intervals_searched_per_s.  With N > 1 every rank runs the same call (replicas, no collective)."""
+    import torch
+    from paper_1208_3407_b200 import bits
+    peak, peak_src = measured_peaks()
+    n, q = w.n_b, w.n_a
+    d = [to_dev(x, device) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+    ws = torch.empty(bits.workspace_bytes(bits.FN_COUNT_PER_INTERVAL, q, n), dtype=torch.uint8, device=device)
+    counts = torch.empty(q, dtype=torch.int32, device=device)
+    total = torch.empty(1, dtype=torch.int64, device=device)
+    step = lambda: bits.count_per_interval(*d, workspace=ws, counts_out=counts, total_out=total)
+    # L2: a step reads 8 (n + q) bytes of input and writes 4 q; below twice the 126 MB L2 the cache is flushed between steps
+    # (a 256 MB fill outside the per-step event pairs), above it the inputs evict themselves
+    footprint = 8 * (n + q) + 4 * q
+    flush = footprint < 2 * 126 * 2**20
+    junk = torch.empty(256 << 20, dtype=torch.uint8, device=device) if flush else None
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_steps(k):
+        ms = 0.0
+        for _ in range(k):
+            if flush:
+                junk.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); step(); b.record(); b.synchronize()
+            ms += a.elapsed_time(b)
+        return ms
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    bits.set_option("profile", 0)
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+    if rank == 0:
+        sampler.start()
+    launches0 = bits.launch_count()
+    barrier()
+    elapsed_ms = timed_steps(args.steps)
+    barrier()
+    launches = bits.launch_count() - launches0
+    # per-kernel durations right behind the timed region (event pairs cost time, so they stay out of `value`)
+    prof_steps = max(1, min(args.steps, 5))
+    bits.set_option("profile", 2); bits.set_option("profile", 1)
+    for _ in range(prof_steps):
+        if flush:
+            junk.fill_(1)
+        step()
+    barrier()
+    prof = bits.profile_read(); bits.set_option("profile", 0)
+    # a short timed region gives nvidia-smi (100 ms period) nothing to sample: keep the GPU on the same step until it has
+    t_end = time.perf_counter() + 0.6
+    while rank == 0 and time.perf_counter() < t_end:
+        step()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([elapsed_ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(t.item())
+        lt = torch.tensor([launches], dtype=torch.int64, device=device)
+        dist.all_reduce(lt, op=dist.ReduceOp.SUM)
+        launches = int(lt.item())
+    value = world * q * args.steps / (elapsed_ms * 1e-3)
+    ms = {k: v[0] / prof_steps for k, v in prof.items() if v[1]}
+    binned = bool(ms.get("bucket_search"))
+    # algorithmic HBM bytes per call of every kernel class (DESIGN.md section 5)
+    alg = {"histogram": 8 * n + (4 * q if binned else 0), "scatter": 16 * n, "bucket_sort": 16 * n,
+           "query_scatter": 20 * q, "bucket_search": 16 * q + 8 * n, "index_build": 8 * n, "count": 12 * q}
+    alg = {k: b for k, b in alg.items() if ms.get(k)}
+    dom = max(alg, key=lambda k: ms[k])
+    own = sum(alg.values())
+    survey = 72 * n + 8 * n + 12 * q           # SURVEY 8(d): histogram read + four LSD passes over both arrays, queries in, counts out
+    line = {
+        "metric": "intervals_searched_per_s", "value": value, "unit": "intervals/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": elapsed_ms / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": w.name, "n_a": q, "n_b": n, "data_seed": w.spec.get("seed"), "scale": w.spec.get("scale", 1.0),
+                   "step": "one bits_count_per_interval call: sort B_S and B_E, two ranks per query, counts written, total reduced",
+                   "search_design": "queries binned by B's buckets (binned_count.cuh)" if binned else "bucket index (search.cuh)",
+                   "parallelism": f"{world} replica(s), no collective",
+                   "l2": ("flushed between steps: a 256 MB fill outside each step's event pair (the step's footprint, "
+                          f"{footprint / 1e6:.0f} MB, would otherwise stay in the 126 MB L2)") if flush else
+                         f"no flush: a step's footprint ({footprint / 1e6:.0f} MB) is larger than the 126 MB L2"},
+        "gpu_launches": launches, "sort_keys_per_s": None, "profile_events_in_timed_region": False,
+        "roofline": {"bound": "hbm", "kernel": {"histogram": "bin_hist_kernel", "scatter": "scatter_kernel", "bucket_sort": "bucket_sort_kernel",
+                                                "query_scatter": "query_scatter_kernel", "bucket_search": "bucket_search_kernel",
+                                                "index_build": "build_index_kernel", "count": "count_kernel"}[dom],
+                     "achieved": alg[dom] / (ms[dom] * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": alg[dom] / (ms[dom] * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                     "avg_launch_ms": ms[dom], "algorithmic_bytes_per_launch": alg[dom],
+                     "timed_in": f"{prof_steps} extra step(s) right behind the timed region, one event pair per launch",
+                     "kernel_ms_per_step": ms,
+                     "kernel_roofline": {k: {"algorithmic_bytes": b, "ms": ms[k], "frac_of_hbm_peak": b / (ms[k] * 1e-3) / 1e9 / peak}
+                                         for k, b in alg.items()},
+                     "step_hbm_bytes_this_design": own,
+                     "step_frac_of_peak_this_design": own * value / world / q / 1e9 / peak,
+                     "step_hbm_bytes_model_survey": survey,
+                     "step_frac_of_peak_model_survey": survey * value / world / q / 1e9 / peak},
+        "clocks": clocks,
+    }
+    if not args.no_extras:
+        # end to end: host arrays in pinned memory -> bits_count_per_interval_host -> counts and total back on the host
+        hp = [pinned(x) for x in (w.a_start, w.a_end, w.b_start, w.b_end)]
+        hws = bits.host_workspace(bits.FN_COUNT_PER_INTERVAL, q, n, device=device)
+        counts_host_t = torch.empty(q, dtype=torch.int32).pin_memory()
+        counts_host = counts_host_t.numpy().view(np.uint32)
+        e2e_step = lambda: bits.count_per_interval_host(hp[0][1], hp[1][1], hp[2][1], hp[3][1], workspace=hws, device=device,
+                                                        counts_out=counts_host)
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        e2e_steps = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            res = e2e_step()
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        h_counts, h_total = res
+        line["e2e"] = {"value": world * q * e2e_steps / t_e2e, "unit": "intervals/s",
+                       "h2d_bytes_per_step": 4 * (2 * q + 2 * n), "d2h_bytes_per_step": 4 * q + 8, "steps": e2e_steps,
+                       "api": "bits_count_per_interval_host (pinned host buffers)",
+                       "matches_device_path": bool(np.array_equal(np.asarray(h_counts).view(np.uint32), counts.cpu().numpy().view(np.uint32))
+                                                   and int(h_total) == int(total.cpu().numpy().view(np.uint64)[0]))}
+        if rank == 0:
+            import oracle
+            t0 = time.perf_counter(); o_total, o_counts = oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end); dt = time.perf_counter() - t0
+            line["cpu_baseline"] = {"value": q / dt, "unit": "intervals/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
+                                    "sample": f"the whole call once ({dt:.2f} s): std::sort of both key arrays of B + one ICOUNT per query + sum"}
+            line["oracle_match"] = bool(int(total.cpu().numpy().view(np.uint64)[0]) == o_total and
+                                        np.array_equal(counts.cpu().numpy().view(np.uint32), o_counts))
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
     return 0
 
 

@@ -21,15 +21,19 @@ FLAGS = [
 ]
 
 
-FUSED_KERNEL_SOURCES = ("common.cuh", "mc_tile.cuh", "msd_sort.cuh", "philox_place.cuh")
+# Every source a captured kernel's ncu counters depend on: the kernel headers AND the host orchestration, whose launch
+# geometry (tile size, bin width, grid, rounds per launch, knob defaults) changes DRAM bytes, durations and limiters
+# just as a kernel edit does.
+HASHED_SOURCES = ("binned_count.cuh", "bits_api.cu", "common.cuh", "enumerate.cuh", "mc_small.cuh", "mc_tile.cuh", "msd_sort.cuh",
+                  "philox_place.cuh", "place_kernels.cuh", "radix_sort.cuh", "screen.cuh", "search.cuh")
 
 
 def csrc_hash() -> str:
-    """sha256 over the sources the two fused Monte Carlo kernels are compiled from (FUSED_KERNEL_SOURCES): identifies
-    the kernels whose ncu counters profiles/r2b_fused_ncu_counters.json holds."""
+    """sha256 over HASHED_SOURCES (all of csrc/): identifies the build whose ncu counters a profiles/*_ncu_counters.json
+    holds.  Written into that file by ncu_counters.py at capture time, compared by bench.py at run time."""
     import hashlib
     h = hashlib.sha256()
-    for path in [os.path.join(CSRC, f) for f in FUSED_KERNEL_SOURCES]:
+    for path in [os.path.join(CSRC, f) for f in HASHED_SOURCES]:
         h.update(os.path.basename(path).encode())
         with open(path, "rb") as f:
             h.update(f.read())
@@ -89,3 +93,5 @@ if __name__ == "__main__":
     build_probe(force="--force" in sys.argv)
     build_yardsticks(force="--force" in sys.argv)
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--hash" in sys.argv:
+        print(csrc_hash())
