@@ -359,14 +359,18 @@ def library_yardsticks(device, w4, d4):
     return out
 
 
-def screen_workload(device, w, gather_gsectors=0.0):
+SCREEN_CAPTURE_ROUNDS = 4     # rounds per pair in the ncu capture of scr::screen_kernel (ncu loses the counters of a 0.9 s launch;
+                              # a block serves four rounds for its query tile either way, so sectors per interval carry over)
+
+
+def screen_workload(device, w, gather_gsectors=0.0, rounds=20):
     """The many-pair screen on synthetic tracks (w = config 2, whose B the tracks are drawn from)."""
     import torch
     from paper_1208_3407_b200 import bits
     # SURVEY 8(f).3: the paper's screen (PAPER.md:165-171: 159 tracks, 25,281 ordered pairs) on synthetic tracks of 1e5
     # intervals drawn from config 2's recipe, as ONE bits_screen call (every track sorted and indexed once, all pairs and
     # rounds in gridded launches); 20 of the paper's 10,000 rounds per pair, device time by CUDA events
-    K, n_t, R_s = 159, 100_000, 20
+    K, n_t, R_s = 159, 100_000, rounds
     rng = np.random.default_rng(8)
     idx = [rng.choice(w.n_b, n_t, replace=False) for _ in range(K)]
     starts = to_dev(np.concatenate([w.b_start[i] for i in idx]), device)
@@ -395,7 +399,8 @@ def screen_workload(device, w, gather_gsectors=0.0):
                                             "tracks (PAPER.md:171; other data, other hardware: context only)"},
         "enrichment_diag_mean": float(np.mean(np.diag(enr))),
         "enrichment_offdiag_mean": float(np.mean(enr[~np.eye(K, dtype=bool)]))}
-    res["l2_roofline"] = l2_roofline("screen_kernel", float(K) * K * R_s * n_t, K * K * R_s * n_t / (rounds_ms * 1e-3), gather_gsectors)
+    # (the kernel name matches both instantiations; the sorted lookup takes `screen_kernel<0>`, the rounds kernel)
+    res["l2_roofline"] = l2_roofline("screen_kernel", float(K) * K * SCREEN_CAPTURE_ROUNDS * n_t, K * K * R_s * n_t / (rounds_ms * 1e-3), gather_gsectors)
     return res
 
 
@@ -810,7 +815,7 @@ def run_study(args):
         bits.set_option(name, int(val))
     if args.study == "screen":      # the screen alone (one JSON object): the command the ncu capture of scr::screen_kernel runs
         gather = 0.0 if args.once else l2_yardsticks(device)["l2_random_sector_gather_gsectors_per_s_80MB"]
-        print(json.dumps({"study": "screen", "screen_159_tracks_of_1e5": screen_workload(device, W.make_config(2), gather)}))
+        print(json.dumps({"study": "screen", "screen_159_tracks_of_1e5": screen_workload(device, W.make_config(2), gather, args.rounds or 20)}))
         return 0
     reps = 1 if args.once else 8
     w = W.make_config(4, scale=args.scale)
@@ -938,6 +943,8 @@ def run_count_config(args, w, device, rank, world, dist):
     # algorithmic HBM bytes per call of every kernel class
     alg = {"histogram": 8 * n + (4 * q if binned else 0), "scatter": 16 * n, "bucket_sort": 16 * n,
            "query_scatter": 20 * q, "bucket_search": 16 * q + 8 * n, "index_build": 8 * n, "count": 12 * q}
+    if binned:      # (the index and count launches behind the binned design are gated fallbacks that exit at once)
+        alg.pop("index_build"); alg.pop("count")
     alg = {k: b for k, b in alg.items() if ms.get(k)}
     dom = max(alg, key=lambda k: ms[k])
     own = sum(alg.values())

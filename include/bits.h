@@ -25,7 +25,9 @@
  *   - Every function returns a bits_status (0 = BITS_OK); no exceptions, no printing, no exit.
  *     On error no output is defined.  There is no CPU fallback: without a usable CUDA device
  *     the compute entry points return BITS_ERR_CUDA.
- *   - Sizes: n_a, n_b < 2^32.  Degenerate sizes are legal: n_a == 0 or n_b == 0 gives total 0,
+ *   - Sizes: n_a, n_b < 2^28 (268,435,456 intervals per set; larger sets are refused with BITS_ERR_SIZE -- element
+ *     indices inside the kernels are 32-bit and some are scaled by up to 8 before use; the GPU tests go up to 2.5e7
+ *     intervals).  Coordinates use the full uint32 range.  Degenerate sizes are legal: n_a == 0 or n_b == 0 gives total 0,
  *     all per-interval counts 0 and all round counts 0.
  *   - All results are integers: per-interval counts uint32, totals and round counts uint64.
  *   - Threads: the library keeps no state between calls except (a) the tuning knobs of
@@ -49,7 +51,7 @@ extern "C" {
 typedef enum {
   BITS_OK = 0,
   BITS_ERR_NULL = 1,          /* a required pointer is NULL */
-  BITS_ERR_SIZE = 2,          /* n_a or n_b >= 2^32, or n_rounds / round_begin overflow uint32 */
+  BITS_ERR_SIZE = 2,          /* n_a or n_b >= 2^28, or n_rounds / round_begin overflow uint32 */
   BITS_ERR_GENOME = 3,        /* offset table: off[0] != 0, not strictly ascending, or n_chrom == 0 */
   BITS_ERR_NO_PLACEMENT = 4,  /* an interval of the permuted set is as long as every chromosome */
   BITS_ERR_WORKSPACE = 5,     /* workspace NULL, misaligned (256 B) or smaller than required */
@@ -258,7 +260,7 @@ double bits_enrichment(uint64_t observed, const uint64_t* round_counts, uint32_t
 /* The many-pair screen as one device job (Sec. 3.3: every pairwise comparison of K interval
  * sets by the Monte Carlo simulation; Fig. 3 caption :224: score = log2(observed / median of the simulated counts)).
  * The K tracks are passed concatenated: track t = starts/ends[track_offsets[t] .. track_offsets[t+1]) (dev uint32;
- * track_offsets: HOST uint64[n_tracks + 1], [0] = 0, non-decreasing, last < 2^32; n_tracks <= 65535).
+ * track_offsets: HOST uint64[n_tracks + 1], [0] = 0, non-decreasing, last < 2^28; n_tracks <= 65535).
  * For every ORDERED pair (i, j), p = i * n_tracks + j:
  *   observed_out[p] = |I(T_i, T_j)|                                            (dev uint64[n_tracks^2])
  *   round_counts_out[p * n_rounds + k] = total(T_i', T_j), k in [0, n_rounds)     (dev uint64[n_tracks^2 * n_rounds])
@@ -297,7 +299,10 @@ int bits_profile_read(int cls, double* ms_out, uint64_t* launches_out);
 
 /* Tuning knobs for design studies (bench.py --opt NAME=VALUE); returns BITS_ERR_FLAGS for an unknown
  * name or a value out of range.  They never change results.  Thread-local (see "Threads" above).
- * Names are listed in DESIGN.md "Knobs". */
+ * Names, values, defaults and measured effects are tabulated in DESIGN.md section 10 ("Knobs").
+ * Two names are TEST HOOKS, not tuning knobs -- "mc_force_redo" (every n-th fused Monte Carlo round is redone by
+ * the general path as if its overflow flag had been raised) and "mc_shift_bias" (bins widened until they overflow on
+ * the device): they let the parity tests reach the overflow branches through this ABI and have no use in production. */
 int bits_set_option(const char* name, int64_t value);
 
 const char* bits_strerror(int status);

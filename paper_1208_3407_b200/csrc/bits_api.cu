@@ -49,6 +49,10 @@ struct Options {
 static thread_local Options g_opt;
 
 constexpr int kSMs = 148;
+// Largest interval set an entry point accepts (bits.h, "Sizes").  Element indices inside the kernels are 32-bit, and some
+// are scaled before use (four positions per thread: t << 2; tile index x tile size; counts padded by kPad): below 2^28
+// every such product stays under 2^31.  The largest sets the GPU tests run are 2.5e7 intervals.
+constexpr uint64_t kMaxIntervals = 1ull << 28;
 constexpr size_t kMaxSmemPerBlock = 232448 - 2048;   // 227 KB opt-in limit of shared memory per block on sm_100, less room for static shared memory
 
 // ---------------------------------------------------------------------------------------------
@@ -638,7 +642,7 @@ static int validate_inputs(const uint32_t* a_start, const uint32_t* a_end, uint3
 
 static int check_common(const void* a_start, const void* a_end, uint64_t n_a, const void* b_start, const void* b_end,
                         uint64_t n_b, uint32_t flags) {
-  if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (n_a >= kMaxIntervals || n_b >= kMaxIntervals) return BITS_ERR_SIZE;
   if (flags & ~(uint32_t)(BITS_B_SORTED | BITS_VALIDATE)) return BITS_ERR_FLAGS;
   if (n_a && (!a_start || !a_end)) return BITS_ERR_NULL;
   if (n_b && (!b_start || !b_end)) return BITS_ERR_NULL;
@@ -1182,7 +1186,7 @@ static int check_tracks(const uint64_t* toff, uint32_t K) {
   if (toff[0] != 0) return BITS_ERR_SIZE;
   for (uint32_t t = 0; t < K; ++t)
     if (toff[t + 1] < toff[t]) return BITS_ERR_SIZE;
-  if (toff[K] >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (toff[K] >= kMaxIntervals) return BITS_ERR_SIZE;
   return BITS_OK;
 }
 
@@ -1351,7 +1355,7 @@ extern "C" {
 size_t bits_workspace_bytes(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_chrom, int which, uint32_t flags) {
   (void)flags;
   if (fn < BITS_FN_COUNT || fn > BITS_FN_ENUMERATE) return 0;
-  if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return 0;
+  if (n_a >= kMaxIntervals || n_b >= kMaxIntervals) return 0;
   return make_layout(nullptr, fn, n_a, n_b, n_chrom, which, flags).bytes;
 }
 
@@ -1359,7 +1363,7 @@ int bits_workspace_sorted_offset(int fn, uint64_t n_a, uint64_t n_b, uint32_t n_
                                  size_t* offset_out) {
   if (!offset_out) return BITS_ERR_NULL;
   if (fn < BITS_FN_COUNT || fn > BITS_FN_MC_ROUNDS || (array != 0 && array != 1)) return BITS_ERR_FLAGS;
-  if (n_a >= (1ull << 32) || n_b >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (n_a >= kMaxIntervals || n_b >= kMaxIntervals) return BITS_ERR_SIZE;
   char* const base = reinterpret_cast<char*>(uintptr_t(1) << 20);   // any non-null base: only differences are used
   const Layout L = make_layout(base, fn, n_a, n_b, n_chrom, which);
   *offset_out = (size_t)(reinterpret_cast<char*>(L.b.buf[array][0]) - base);
@@ -1475,7 +1479,7 @@ int bits_place(const uint32_t* spans, uint64_t n, const uint32_t* chrom_offsets,
                uint32_t round, uint32_t tag, void* workspace, size_t workspace_bytes, uint32_t* start_out,
                uint32_t* end_out, void* stream) {
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  if (n >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (n >= kMaxIntervals) return BITS_ERR_SIZE;
   if (n && (!spans || !start_out || !end_out)) return BITS_ERR_NULL;
   ChromTable chrom;
   uint32_t l_max = 0;
@@ -1492,7 +1496,7 @@ int bits_place(const uint32_t* spans, uint64_t n, const uint32_t* chrom_offsets,
 int bits_sort_u32(const uint32_t* keys_in, uint32_t* keys_out, uint64_t n, void* workspace, size_t workspace_bytes,
                   void* stream) {
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  if (n >= (1ull << 32)) return BITS_ERR_SIZE;
+  if (n >= kMaxIntervals) return BITS_ERR_SIZE;
   if (n && (!keys_in || !keys_out)) return BITS_ERR_NULL;
   const Layout L = make_layout(workspace, BITS_FN_SORT, 0, n, 0, 0);
   if (!ws_ok(workspace, workspace_bytes, L.bytes)) return BITS_ERR_WORKSPACE;
@@ -1646,7 +1650,7 @@ const char* bits_strerror(int status) {
   switch (status) {
     case BITS_OK: return "ok";
     case BITS_ERR_NULL: return "a required pointer is NULL";
-    case BITS_ERR_SIZE: return "size out of range (n_a, n_b < 2^32; round_begin + n_rounds <= 2^32)";
+    case BITS_ERR_SIZE: return "size out of range (n_a, n_b < 2^28; round_begin + n_rounds <= 2^32)";
     case BITS_ERR_GENOME: return "bad chromosome offset table";
     case BITS_ERR_NO_PLACEMENT: return "an interval of the permuted set is as long as every chromosome";
     case BITS_ERR_WORKSPACE: return "workspace NULL, misaligned or too small";

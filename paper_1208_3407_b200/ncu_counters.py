@@ -39,8 +39,11 @@ METRICS = {
     "l1tex__lsu_writeback_active_mem_lg.avg.pct_of_peak_sustained_elapsed": "l1_lsu_writeback_pct",
     "l1tex__throughput.avg.pct_of_peak_sustained_active": "l1tex_throughput_pct",
     "lts__throughput.avg.pct_of_peak_sustained_elapsed": "l2_throughput_pct",
-    "lts__t_sectors_op_read.sum": "l2_sectors_read",
-    "lts__t_sectors_op_write.sum": "l2_sectors_write",
+    "lts__t_sectors_srcunit_tex_op_read.sum": "l2_sectors_read",          # sectors the SMs read from L2 (hits and misses)
+    "lts__t_sectors_srcunit_tex_op_write.sum": "l2_sectors_write",
+    "lts__t_sectors_srcunit_tex_op_red.sum": "l2_sectors_red",
+    "lts__t_requests_srcunit_tex_op_read.sum": "l2_read_requests",
+    "lts__t_sectors_srcunit_tex_op_read_lookup_miss.sum": "l2_sectors_read_miss",
     "lts__t_sector_hit_rate.pct": "l2_hit_rate_pct",
     "l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum": "l1_global_load_sectors",
     "l1tex__t_requests_pipe_lsu_mem_global_op_ld.sum": "l1_global_load_requests",
@@ -86,10 +89,12 @@ def read_report(report: str):
 
 
 def to_number(x: str):
+    """None for text and for the nan ncu prints when a counter could not be collected (very long kernels)."""
     try:
-        return float(x.replace(",", ""))
+        v = float(x.replace(",", ""))
     except ValueError:
         return None
+    return v if v == v and abs(v) != float("inf") else None
 
 
 def summarise(report: str) -> dict:
@@ -116,7 +121,7 @@ def summarise(report: str) -> dict:
                 scale = {"ns": 1e-3, "us": 1.0, "usecond": 1.0, "ms": 1e3, "msecond": 1e3, "nsecond": 1e-3, "s": 1e6, "second": 1e6}.get(unit, None)
                 d["duration_us_under_ncu"] = v * scale if scale else v
                 continue
-            if key.startswith("dram_bytes") or key.startswith("l2_sectors") or key.endswith("instructions") or key.endswith("wavefronts"):
+            if key.startswith("dram_bytes") or key.startswith("l2_sectors") or key.endswith("requests") or key.endswith("instructions") or key.endswith("wavefronts"):
                 mult = {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "byte": 1.0}.get(unit, 1.0)
                 d[key] = int(round(v * mult))
             else:

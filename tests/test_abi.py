@@ -41,6 +41,8 @@ def test_workspace_sizes():
     w = bits.workspace_bytes
     assert w(99, 1, 1) == 0
     assert w(bits.FN_COUNT, 2**32, 1) == 0
+    assert w(bits.FN_COUNT, 2**28, 1) == 0 and w(bits.FN_COUNT, 1, 2**28) == 0      # the documented bound: n < 2^28
+    assert w(bits.FN_COUNT, 2**28 - 1, 2**28 - 1) > 16 * (2**28 - 1)
     small, big = w(bits.FN_COUNT, 10, 1000), w(bits.FN_COUNT, 10, 10_000_000)
     assert 0 < small < big
     assert big >= 4 * 4 * 10_000_000                      # two arrays, ping + pong

@@ -1025,6 +1025,89 @@ def test_cli_on_bed_files(tmp_path, capsys):
     assert cli.main(["count", "-a", str(tmp_path / "nope.bed"), "-b", str(tmp_path / "b.bed"), "-g", str(tmp_path / "g.txt")]) == 2
 
 
+# ------------------------------------------------------------------------------------- input checking, large sizes
+def test_validate_flag_through_every_entry_point():
+    """BITS_VALIDATE through bits_mc_rounds (both kinds), bits_enumerate and bits_screen: a set with one start > end is
+    refused with status 7 (BITS_ERR_MALFORMED), well-formed sets give the oracle's integers with the flag on."""
+    rng = np.random.default_rng(41)
+    off = W.genome_offsets([3_000_000, 2_000_000, 1_200_000])
+    tracks = _screen_tracks(rng, off, ((3000, 400), (20_000, 900)))
+    (a_s, a_e), (b_s, b_e) = tracks
+    i_a = int(np.argmax(a_s > 0))
+    bad_e = a_e.copy(); bad_e[i_a] = a_s[i_a] - 1                        # a malformed interval in A
+    assert b_s[-1] > 0
+    bad_be = b_e.copy(); bad_be[-1] = b_s[-1] - 1                        # ... and one in B (the last element)
+    for which in (0, 1):
+        obs, rc = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, which, 3, 0, 7, flags=bits.VALIDATE)
+        sync()
+        o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, which, 3, 0, 7)
+        assert int(host_u64(obs)[0]) == o_obs and np.array_equal(host_u64(rc), o_rc)
+        for args in ((a_s, bad_e, b_s, b_e), (a_s, a_e, b_s, bad_be)):
+            with pytest.raises(bits.BitsError) as e:
+                bits.mc_rounds(*[dev(x) for x in args], off, which, 3, 0, 7, flags=bits.VALIDATE)
+            assert e.value.status == 7
+    pa, pb, n = bits.enumerate_pairs(dev(a_s), dev(a_e), dev(b_s), dev(b_e), flags=bits.VALIDATE)
+    sync()
+    want = oracle.enumerate_pairs(a_s, a_e, b_s, b_e)
+    got = np.stack([host_u32(pa), host_u32(pb)], axis=1)
+    assert n == len(want) and np.array_equal(got[np.lexsort((got[:, 1], got[:, 0]))], want)
+    for args in ((a_s, bad_e, b_s, b_e), (a_s, a_e, b_s, bad_be)):
+        with pytest.raises(bits.BitsError) as e:
+            bits.enumerate_pairs(*[dev(x) for x in args], flags=bits.VALIDATE)
+        assert e.value.status == 7
+    toff = np.array([0, a_s.size, a_s.size + b_s.size], dtype=np.uint64)
+    cat = lambda x, y: dev(np.concatenate([x, y]))
+    obs, rc = bits.screen_concat(cat(a_s, b_s), cat(a_e, b_e), toff, off, 5, 4, flags=bits.VALIDATE)
+    sync()
+    o_obs, o_rc, _ = oracle.screen(tracks, off, 5, 0, 4)
+    assert np.array_equal(obs.cpu().numpy().view(np.uint64), o_obs) and np.array_equal(rc.cpu().numpy().view(np.uint64), o_rc)
+    with pytest.raises(bits.BitsError) as e:
+        bits.screen_concat(cat(a_s, b_s), cat(a_e, bad_be), toff, off, 5, 4, flags=bits.VALIDATE)
+    assert e.value.status == 7
+
+
+def test_count_per_interval_host_config4_full_size():
+    """The host-buffer entry point at a size where the staging matters (160 MB in, 40 MB out): every one of the 10^7
+    per-interval counts and the total against the oracle."""
+    w = W.make_config(4)
+    o_total, o_counts = oracle.count_per_interval(w.a_start, w.a_end, w.b_start, w.b_end)
+    counts, total = bits.count_per_interval_host(w.a_start, w.a_end, w.b_start, w.b_end)
+    assert total == o_total
+    bad = np.nonzero(counts != o_counts)[0]
+    assert bad.size == 0, (bad.size, bad[:5])
+    assert bits.count_host(w.a_start, w.a_end, w.b_start, w.b_end) == o_total
+
+
+def test_mc_permute_b_above_the_fused_limit():
+    """A re-placed set of 25M intervals (above the 24M the fused bins hold): every round goes through the general path
+    (placement kernel, MSD sort of both arrays, search with the sorted queries).  Two rounds against the oracle, and the
+    sorted arrays of the last round."""
+    rng = np.random.default_rng(43)
+    off = W.genome_offsets(W.GENOME24_LENGTHS)
+    n_b, n_a = 25_000_000, 200_000
+    def draw(n, max_len):
+        c = rng.integers(0, 24, n); ln = rng.integers(1, max_len, n)
+        lo, hi = off[:-1][c].astype(np.int64), off[1:][c].astype(np.int64)
+        st = lo + (rng.random(n) * (hi - lo - ln)).astype(np.int64)
+        return st.astype(np.uint32), (st + ln - 1).astype(np.uint32)
+    b_s, b_e = draw(n_b, 500)
+    a_s, a_e = draw(n_a, 3000)
+    ws = torch.empty(bits.workspace_bytes(bits.FN_MC_ROUNDS, n_a, n_b, 24, 1), dtype=torch.uint8, device=DEV)
+    bits.set_option("profile", 2); bits.set_option("profile", 1)
+    try:
+        obs, rc = bits.mc_rounds(dev(a_s), dev(a_e), dev(b_s), dev(b_e), off, 1, 9, 3, 2, workspace=ws)
+        sync()
+        prof = bits.profile_read()
+    finally:
+        bits.set_option("profile", 0)
+    assert prof["place_scatter"][1] == 0 and prof["place"][1] == 2          # the general path ran, twice
+    o_obs, o_rc = oracle.mc_rounds(a_s, a_e, b_s, b_e, off, 1, 9, 3, 2)
+    assert int(host_u64(obs)[0]) == o_obs and np.array_equal(host_u64(rc), o_rc)
+    g_s, g_e = bits.sorted_arrays_in_workspace(ws, bits.FN_MC_ROUNDS, n_a, n_b, 24, 1)
+    p_s, p_e = oracle.place_round((b_e - b_s).astype(np.uint32), off, 9, 4, 1)
+    assert np.array_equal(host_u32(g_s), oracle.sort_u32(p_s)) and np.array_equal(host_u32(g_e), oracle.sort_u32(p_e))
+
+
 # ------------------------------------------------------------------------------------- host-buffer entry points
 def test_host_variants_config1():
     w = W.make_config(1)
