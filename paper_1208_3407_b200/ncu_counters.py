@@ -171,5 +171,86 @@ def main(argv=None) -> int:
     return 0
 
 
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Per-phase instruction budget of bin_sort_search_kernel from the source page of an `--import-source on` capture:
+#     python -m paper_1208_3407_b200.ncu_counters --phases OUT.md REPORT.ncu-rep --keys N
+# Every source line's counters (warp instructions executed, shared-memory wavefronts, excess wavefronts = bank
+# conflicts, stall samples) are summed over the phase the line belongs to.  Phases are line ranges of mc_tile.cuh found
+# from the marker strings below, so the table follows the file as it changes.
+PHASE_MARKERS = (      # (phase, first-line marker, last-line marker) in mc_tile.cuh; helper functions count for their phase
+    ("count (count_key)", "__device__ __forceinline__ void count_key(", "// position of the next key of sub-bucket sb"),
+    ("scatter (take_slot)", "__device__ __forceinline__ uint32_t take_slot(", "// Counts -> exclusive prefixes, in place"),
+    ("scan of the cursors (scan_cursors)", "__device__ __forceinline__ void scan_cursors(", "// Counting-sort scatter of buf[0..m) in place"),
+    ("scatter (scatter_in_place)", "__device__ __forceinline__ void scatter_in_place(", "// Write buf[0..mv) (ordered by sub-bucket)"),
+    ("write-out + tie rank (write_and_rank, first loop)", "__device__ __forceinline__ uint64_t write_and_rank(", "  uint64_t qsum = 0;\n  for (uint32_t qi"),
+    ("query rank (write_and_rank, second loop)", "  uint64_t qsum = 0;\n  for (uint32_t qi", "template <class C, bool kSlots = false>"),
+    ("per-bin prologue: ticket, segment words, scans, cursor clear", "bin_sort_search_kernel(BinSortArgs a) {", "    // gather: a group of lanes per segment"),
+    ("gather (cp.async of the pairs and the hand-over list)", "    // gather: a group of lanes per segment", "    // Algorithm 2's Sort(B_S), Sort(B_E) for this bin"),
+    ("count (loop in the kernel body)", "    // Algorithm 2's Sort(B_S), Sort(B_E) for this bin", "    uint32_t total[2];"),
+    ("calls + block reduce (kernel body tail)", "    uint32_t total[2];", "// Query ranges per bin, once per call"),
+)
+
+
+def phase_budget(report: str, n_keys: float, kernel_regex: str = "bin_sort_search_kernel") -> str:
+    import os
+    text = open(os.path.join(B.CSRC, "mc_tile.cuh")).read()
+    line_of = lambda marker: text[:text.index(marker)].count("\n") + 1
+    ranges = [(name, line_of(a), line_of(b) - 1) for name, a, b in PHASE_MARKERS]
+    raw = subprocess.run(["ncu", "-i", report, "--page", "source", "--csv", "--print-source", "cuda,sass", "--kernel-name",
+                          f"regex:{kernel_regex}"], check=True, capture_output=True, text=True).stdout
+    cur_file, cols, kernel = None, None, ""
+    agg: dict[str, list[float]] = {}
+    fields = ("Instructions Executed", "L1 Wavefronts Shared", "L1 Wavefronts Shared Excessive", "# Samples", "stall_barrier",
+              "stall_long_sb", "stall_short_sb", "stall_mio")
+    for r in csv.reader(io.StringIO(raw)):
+        if len(r) == 2 and r[0] == "File Path":
+            cur_file = os.path.basename(r[1]); continue
+        if len(r) == 2 and r[0] == "Function Name":
+            kernel = r[1]; continue
+        if r and r[0] == "Line No":
+            cols = {}
+            for i, n in enumerate(r):
+                cols.setdefault(n, i)
+            continue
+        if not cols or len(r) < len(cols) or r[cols["Address"]] != "-":
+            continue                                  # SASS rows repeat what the line's own row already sums
+        try:
+            line = int(r[0])
+        except ValueError:
+            continue
+        phase = f"other files ({cur_file})"
+        if cur_file == "mc_tile.cuh":
+            phase = next((name for name, lo, hi in ranges if lo <= line <= hi), "mc_tile.cuh, other lines (sub_of, ...)")
+        a = agg.setdefault(phase, [0.0] * len(fields))
+        for j, f in enumerate(fields):
+            a[j] += to_number(r[cols[f]]) or 0.0
+    tot = [sum(a[j] for a in agg.values()) for j in range(len(fields))]
+    out = [f"Kernel: `{kernel}`", "",
+           f"Source-page counters summed per phase; per key = divided by {n_keys:.0f} keys per launch (both arrays). "
+           "One warp instruction = up to 32 thread instructions.", "",
+           "| phase | mc_tile.cuh lines | warp instr | share | thread instr per key (x32) | shared wavefronts | excess (bank conflicts) | stall samples | of which barrier | long_sb | short_sb | mio |",
+           "|---|---|---|---|---|---|---|---|---|---|---|---|"]
+    lines_of = {name: f"{lo}-{hi}" for name, lo, hi in ranges}
+    for name, a in sorted(agg.items(), key=lambda kv: -kv[1][0]):
+        out.append(f"| {name} | {lines_of.get(name, '')} | {a[0]:,.0f} | {a[0] / tot[0]:.3f} | {32 * a[0] / n_keys:.1f} | {a[1]:,.0f} | {a[2]:,.0f} | "
+                   f"{a[3]:,.0f} | {a[4]:,.0f} | {a[5]:,.0f} | {a[6]:,.0f} | {a[7]:,.0f} |")
+    out.append(f"| **total** | | {tot[0]:,.0f} | 1.000 | {32 * tot[0] / n_keys:.1f} | {tot[1]:,.0f} | {tot[2]:,.0f} | {tot[3]:,.0f} | {tot[4]:,.0f} | {tot[5]:,.0f} | {tot[6]:,.0f} | {tot[7]:,.0f} |")
+    return "\n".join(out) + "\n"
+
+
+def phases_main(argv) -> int:
+    p = argparse.ArgumentParser()
+    p.add_argument("out"); p.add_argument("report"); p.add_argument("--keys", type=float, default=2e7)
+    p.add_argument("--kernel", default="bin_sort_search_kernel")
+    a = p.parse_args(argv)
+    body = phase_budget(a.report, a.keys, a.kernel)
+    with open(a.out, "w") as f:
+        f.write(f"<!-- written by: python -m paper_1208_3407_b200.ncu_counters --phases {a.out} {a.report} --keys {a.keys:.0f}; csrc {B.csrc_hash()} -->\n\n" + body)
+    print(body)
+    return 0
+
+
 if __name__ == "__main__":
-    sys.exit(main())
+    sys.exit(phases_main(sys.argv[2:]) if len(sys.argv) > 1 and sys.argv[1] == "--phases" else main())
